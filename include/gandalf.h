@@ -1,0 +1,139 @@
+/* gandalf.h -- C ABI of the B200-native GANDALF KRMHD hot path (arXiv 2511.21891).
+ *
+ * The library evaluates the pseudo-spectral right-hand side of the Kinetic Reduced MHD
+ * equations and advances them with the integrating-factor RK2 step, entirely in hand-written
+ * sm_100a CUDA kernels (no cuFFT, no CPU fallback).  Citations are PAPER.md line numbers with
+ * the section / equation they fall in; readings of ambiguous passages are DESIGN.md Q1-Q24.
+ *
+ * Conventions
+ *  - All functions return GANDALF_OK (0) or a negative error code; they never throw or abort.
+ *    gandalf_last_error(ctx) returns a ctx-owned, NUL-terminated message for the last failure.
+ *  - The handle owns every device buffer.  Caller arrays are only read / written during a call.
+ *    `on_device` says whether caller array pointers are HOST (0) or DEVICE (1) pointers on the
+ *    ctx's device.  Host-pointer calls synchronise the ctx's stream before returning; device-
+ *    pointer calls are stream-ordered on the ctx's stream and do not synchronise.
+ *  - No global state; contexts are independent; one context must not be used from two threads
+ *    at once.
+ *
+ * Boundary array layout ("half-plane"): complex fp64, interleaved (re,im) doubles,
+ *    a[field][kz][ky][kx],  kx = 0..nx/2 fastest (nx/2+1 entries), ky and kz in FFT order
+ *    (0..N/2-1, -N/2..-1), physical normalisation  f(x) = sum_k fhat(k) exp(+i k.x),
+ *    fhat(k) = (1/(nx ny nz)) sum_x f(x) exp(-i k.x)            [PAPER.md:125-130, Eq. 9]
+ *    with k_j = 2 pi n_j / L_j                                   [PAPER.md:128].
+ *    Bytes per field: 16 * (nx/2+1) * ny * nz.
+ */
+#ifndef GANDALF_H_
+#define GANDALF_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GANDALF_OK               0
+#define GANDALF_ERR_INVALID     -1   /* NULL pointer, bad size or parameter                     */
+#define GANDALF_ERR_CUDA        -2   /* a CUDA runtime call or kernel launch failed             */
+#define GANDALF_ERR_NONFINITE   -3   /* NaN/Inf seen in the energy reduction of the last step   */
+#define GANDALF_ERR_UNSUPPORTED -4   /* e.g. M > 0 with vA != 1 (Eq. 6 is written for v_A = 1)  */
+
+typedef struct gandalf_ctx gandalf_ctx;   /* opaque */
+
+typedef struct gandalf_params {
+  int    nx, ny, nz;      /* grid; powers of two, 8 <= nx,ny <= 512, 2 <= nz <= 512               */
+  int    M;               /* number of Hermite moments g_0..g_{M-1}; 0 = RMHD only (Q10)          */
+  double Lx, Ly, Lz;      /* box lengths (> 0)                                                    */
+  double vA;              /* Alfven speed in exp(+-i kz vA dt)  [Eq. 12-13, PAPER.md:154-158]     */
+  double eta;             /* (hyper)resistivity coefficient on w+-  [Eq. 17-18, PAPER.md:230-236] */
+  int    r;               /* hyper order r >= 1                                                   */
+  int    eta_normalized;  /* 1: exp(-eta (kperp^2/kperp_max^2)^r dt) [Eq. 18]; 0: exp(-eta kperp^(2r) dt) */
+  double eta_z;           /* k_z hyperdissipation exp(-eta_z (kz^2/kz_max^2)^r_z dt); 0 = off (Q9) */
+  int    r_z;
+  double eta_g;           /* same perpendicular (and k_z) factor applied to g_m; 0 = paper-literal */
+  double nu_coll;         /* exp(-nu_coll (m/M)^(2p) dt) on g_m  [Eq. 19, PAPER.md:240]            */
+  double p;               /* hyper-collision exponent p >= 1/2                                    */
+  int    closure;         /* 0: g_M = 0 (absorbing); 1: g_M = g_{M-2} (reflecting) [PAPER.md:105]  */
+  int    if_variant;      /* 0: paper-literal double phase [Eq. 15, Alg. 1]; 1: standard IF midpoint (Q6) */
+  int    g_sign;          /* +1: upper signs of Eq. 6 (g^+), -1: lower signs (g^-)                */
+  int    nonlinear;       /* 1: brackets on; 0: brackets replaced by zero (linear tests)          */
+  int    hermite_coeff;   /* 0: sqrt(m/2), sqrt((m+1)/2) for every m [Eq. 6c]; 1: literal sqrt(2), sqrt(3/2) of Eq. 6a/6b (Q24) */
+  double force_eps;       /* energy injection rate of the white-noise forcing; 0 = off [Eq. 25]   */
+  int    force_nperp_min, force_nperp_max, force_nz_max;  /* forced shell in mode numbers          */
+  unsigned long long seed;/* forcing RNG key (counter-based, Q17)                       */
+  double cfl;             /* C of Eq. 16, used when gandalf_step gets dt <= 0      */
+  int    device;          /* CUDA device ordinal                                                  */
+  void*  stream;          /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
+} gandalf_params;
+
+/* Fill *p with defaults: M=0, L=2pi, vA=1, no dissipation, r=r_z=1, p=1, absorbing closure,
+ * paper-literal IF, g_sign=+1, nonlinear=1, no forcing (shell 1..2, |nz|<=1), cfl=0.3, device 0. */
+int gandalf_default_params(gandalf_params* p);
+
+/* Allocate a context (all device buffers, FFT twiddle tables) for the given problem.
+ * Errors: INVALID for NULL / non-power-of-two / out-of-range sizes, M < 0, L <= 0;
+ * UNSUPPORTED for M > 0 with vA != 1 (Q12); CUDA if allocation fails (nothing is leaked). */
+int gandalf_create(const gandalf_params* p, gandalf_ctx** out);
+int gandalf_destroy(gandalf_ctx* ctx);
+
+/* State exchange.  zeta_hat: the Elsasser POTENTIALS xi^+ then xi^- (2 fields, not the
+ * vorticities; w = -kperp^2 xi is formed inside).  g_hat: M fields (may be NULL
+ * when M = 0).  gandalf_set_state PROJECTS its input: it applies the Eq. 20 mask (a mode is
+ * kept iff 3|n| <= N on every axis), zeroes kperp = 0 for zeta, and replaces
+ * the kx = 0 plane by (a(0,ky,kz) + conj a(0,-ky,-kz))/2 so the real-space field is real.
+ * It also resets time, step counter and energy history.  gandalf_get_state returns the current
+ * (projected) state with zeros at removed modes. */
+int gandalf_set_state(gandalf_ctx* ctx, const double* zeta_hat, const double* g_hat, int on_device);
+int gandalf_get_state(gandalf_ctx* ctx, double* zeta_hat, double* g_hat, int on_device);
+
+/* Right-hand side at the current state, boundary layout, without advancing it:
+ *   dw_hat[2] = N^+, N^-  : -1/2 [ {xi+,w-} + {xi-,w+} -+ lap_perp {xi+,xi-} ]  (Eq. 1 / Eq. 12 RHS,
+ *               vorticity units, the linear -+ i kz vA w term is NOT included -- the integrating
+ *               factor carries it), each bracket evaluated pseudo-spectrally and dealiased
+ *               [PAPER.md:49, 140-142, 154, 251-257];
+ *   dg_hat[M] = H_m = -{Phi,g_m} + sqrt(m/2){Psi,g_{m-1}} + sqrt((m+1)/2){Psi,g_{m+1}}
+ *               + s i kz [ g_m - sqrt(m/2) g_{m-1} - sqrt((m+1)/2) g_{m+1} ]   (Eq. 6, no collisions)
+ *               [PAPER.md:89-93]. */
+int gandalf_rhs(gandalf_ctx* ctx, double* dw_hat, double* dg_hat, int on_device);
+
+/* Advance nsteps complete steps of Algorithm 2 [PAPER.md:297-315]: (CFL dt) -> RHS -> half-step
+ * predictor with integrating factors (Eq. 15) and plain RK2 for g_m -> midpoint RHS -> full-step
+ * corrector (Alg. 1 l.8-9) -> exponential dissipation (Eq. 17-19) -> forcing increment (Eq. 25).
+ * dt > 0: fixed step.  dt <= 0: dt = cfl * min(Lx/nx, Ly/ny) / max|grad_perp Phi| recomputed every
+ * step ON THE DEVICE from the state at t_n (Eq. 16), no host synchronisation.
+ * One energy record is appended per step to the device-resident history.  The call is
+ * asynchronous on the ctx's stream; errors detected on the device (non-finite energy) are
+ * reported by gandalf_energy_history / gandalf_energy / gandalf_get_time, which synchronise. */
+int gandalf_step(gandalf_ctx* ctx, double dt, int nsteps);
+
+/* Energies of the current state (host output, synchronises):
+ * out = { E_A, E_plus, E_minus, E_kin, E_mag, W_g } with E_+- = 1/4 sum_k kperp^2 |xi+-|^2,
+ * E_A = E_plus + E_minus, E_kin = 1/2 sum kperp^2 |Phi|^2, E_mag = 1/2 sum kperp^2 |Psi|^2,
+ * W_g = 1/2 sum_m sum_k |g_m|^2, sums over the full spectrum [PAPER.md:115, 383, 442; Q14]. */
+int gandalf_energy(gandalf_ctx* ctx, double out[6]);
+
+/* Perpendicular shell spectrum [Eq. 26; Q15]: bin j = floor(kperp/dk + 1/2),
+ * dk = 2 pi / max(Lx, Ly), summed over kz.  literal_eq26 = 0: mode energy 1/4 kperp^2 (|xi+|^2 +
+ * |xi-|^2) (bins sum to E_A); 1: |xi+|^2 + |xi-|^2 as printed.  out: nbins doubles on the HOST. */
+int gandalf_kperp_spectrum(gandalf_ctx* ctx, int nbins, int literal_eq26, double* out);
+
+/* Copy up to max_records of the per-step records {t, E_A, E_plus, E_minus, E_kin, E_mag, W_g}
+ * (7 doubles each, oldest first, host output) and the count.  Returns GANDALF_ERR_NONFINITE
+ * if any recorded energy is NaN/Inf (records are still copied). */
+int gandalf_energy_history(gandalf_ctx* ctx, int max_records, double* t_and_E, int* n);
+
+/* Simulation time, number of completed steps and the last dt used (host output, synchronises). */
+int gandalf_get_time(gandalf_ctx* ctx, double* t, long long* step, double* last_dt);
+
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+long long gandalf_launch_count(const gandalf_ctx* ctx);
+
+/* Event-timed average duration (ms) of one named kernel class since the last reset; used by
+ * bench.py for the roofline line.  which: 0 z-inverse, 1 y-inverse (P1), 2 x-pass (P2),
+ * 3 y-forward (P3), 4 z-forward, 5 update.  Timing is off unless enabled (it inserts events). */
+int gandalf_kernel_timing(gandalf_ctx* ctx, int enable);
+int gandalf_kernel_time_ms(gandalf_ctx* ctx, int which, double* avg_ms, long long* launches);
+
+const char* gandalf_last_error(const gandalf_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif  /* GANDALF_H_ */

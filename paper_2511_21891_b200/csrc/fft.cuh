@@ -1,0 +1,208 @@
+// fft.cuh -- register-resident radix-2/4/8/16 butterflies and a lane-group cooperative FFT.
+//
+// One FFT of length N is computed by a group of T = N/E consecutive lanes of ONE warp; each lane
+// keeps E complex doubles in registers.  Distribution contract (same on input and output):
+//     lane t (0..T-1) holds   v[q] = x[t + T*q],  q = 0..E-1.
+// The transform is a Stockham autosort with radices {r_1,..,r_S} (product N).  Between stages the
+// data crosses lanes through a padded shared-memory line buffer; the last stage needs no exchange
+// because its natural output index  j + i*N/r  is again  t + T*(b + i*E/r).  All synchronisation is
+// __syncwarp(): every lane of the warp must call the routine (idle groups transform zeros).
+//
+// The phases (compute / scatter / gather) are separate HD functions so that a host test can
+// emulate the T lanes sequentially (tests/test_fft_host.py compiles this header with g++).
+//
+// Sign convention: DIR = -1 forward kernel exp(-2 pi i jk/N), DIR = +1 inverse; no scaling.
+#pragma once
+
+#if defined(__CUDACC__)
+#define GD_HD __host__ __device__ __forceinline__
+#else
+#define GD_HD inline
+#endif
+
+struct alignas(16) cd {   // complex double
+  double x, y;
+};
+
+GD_HD cd cmake(double a, double b) { cd r; r.x = a; r.y = b; return r; }
+GD_HD cd operator+(cd a, cd b) { return cmake(a.x + b.x, a.y + b.y); }
+GD_HD cd operator-(cd a, cd b) { return cmake(a.x - b.x, a.y - b.y); }
+GD_HD cd cmul(cd a, cd b) { return cmake(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+GD_HD cd cconj(cd a) { return cmake(a.x, -a.y); }
+GD_HD cd cscale(cd a, double s) { return cmake(a.x * s, a.y * s); }
+// multiply by DIR*i : forward (-1) -> -i, inverse (+1) -> +i
+template <int DIR> GD_HD cd mul_dir_i(cd a) { return DIR < 0 ? cmake(a.y, -a.x) : cmake(-a.y, a.x); }
+// multiply by i (always +i)
+GD_HD cd mul_i(cd a) { return cmake(-a.y, a.x); }
+
+#define GD_SQRT1_2 0.70710678118654752440
+#define GD_COS_PI_8 0.92387953251128675613
+#define GD_SIN_PI_8 0.38268343236508977173
+
+// multiply by exp(DIR * 2 pi i * P / 16), P in 0..15, with the cheap cases special-cased
+template <int P, int DIR> GD_HD cd mul_w16(cd a) {
+  if constexpr (P == 0) return a;
+  else if constexpr (P == 4) return mul_dir_i<DIR>(a);
+  else if constexpr (P == 8) return cmake(-a.x, -a.y);
+  else if constexpr (P == 12) return mul_dir_i<-DIR>(a);
+  else if constexpr (P == 2) return cmake(GD_SQRT1_2 * (a.x - DIR * a.y), GD_SQRT1_2 * (DIR * a.x + a.y));
+  else if constexpr (P == 6) return mul_w16<2, DIR>(mul_dir_i<DIR>(a));
+  else if constexpr (P == 10) return mul_w16<2, DIR>(cmake(-a.x, -a.y));
+  else if constexpr (P == 14) return mul_w16<2, DIR>(mul_dir_i<-DIR>(a));
+  else {
+    // odd P: general rotation by angle P*pi/8
+    constexpr double c = (P == 1 || P == 15) ? GD_COS_PI_8 : (P == 3 || P == 13) ? GD_SIN_PI_8
+                        : (P == 5 || P == 11) ? -GD_SIN_PI_8 : -GD_COS_PI_8;          // 7, 9
+    constexpr double s0 = (P == 1 || P == 7) ? GD_SIN_PI_8 : (P == 3 || P == 5) ? GD_COS_PI_8
+                         : (P == 9 || P == 15) ? -GD_SIN_PI_8 : -GD_COS_PI_8;        // 11, 13
+    constexpr double s = DIR * s0;
+    return cmake(a.x * c - a.y * s, a.x * s + a.y * c);
+  }
+}
+
+// ---- in-register butterflies: natural order in, natural order out -----------------------------
+template <int DIR> GD_HD void bf2(cd (&x)[2]) {
+  cd a = x[0], b = x[1];
+  x[0] = a + b; x[1] = a - b;
+}
+template <int DIR> GD_HD void bf4(cd& x0, cd& x1, cd& x2, cd& x3) {
+  cd a0 = x0 + x2, a1 = x0 - x2, a2 = x1 + x3, a3 = mul_dir_i<DIR>(x1 - x3);
+  x0 = a0 + a2; x1 = a1 + a3; x2 = a0 - a2; x3 = a1 - a3;
+}
+template <int DIR> GD_HD void bf4(cd (&x)[4]) { bf4<DIR>(x[0], x[1], x[2], x[3]); }
+template <int DIR> GD_HD void bf8(cd (&x)[8]) {
+  cd e0 = x[0], e1 = x[2], e2 = x[4], e3 = x[6];
+  cd o0 = x[1], o1 = x[3], o2 = x[5], o3 = x[7];
+  bf4<DIR>(e0, e1, e2, e3);
+  bf4<DIR>(o0, o1, o2, o3);
+  o1 = mul_w16<2, DIR>(o1);
+  o2 = mul_w16<4, DIR>(o2);
+  o3 = mul_w16<6, DIR>(o3);
+  x[0] = e0 + o0; x[4] = e0 - o0;
+  x[1] = e1 + o1; x[5] = e1 - o1;
+  x[2] = e2 + o2; x[6] = e2 - o2;
+  x[3] = e3 + o3; x[7] = e3 - o3;
+}
+template <int DIR> GD_HD void bf16(cd (&x)[16]) {
+  // n = 4*n1 + n2 ; k = k1 + 4*k2.  Y[n2][k1] = FFT4 over n1; twiddle w16^(n2*k1); FFT4 over n2.
+  cd y0[4] = {x[0], x[4], x[8], x[12]};
+  cd y1[4] = {x[1], x[5], x[9], x[13]};
+  cd y2[4] = {x[2], x[6], x[10], x[14]};
+  cd y3[4] = {x[3], x[7], x[11], x[15]};
+  bf4<DIR>(y0); bf4<DIR>(y1); bf4<DIR>(y2); bf4<DIR>(y3);
+  y1[1] = mul_w16<1, DIR>(y1[1]); y1[2] = mul_w16<2, DIR>(y1[2]); y1[3] = mul_w16<3, DIR>(y1[3]);
+  y2[1] = mul_w16<2, DIR>(y2[1]); y2[2] = mul_w16<4, DIR>(y2[2]); y2[3] = mul_w16<6, DIR>(y2[3]);
+  y3[1] = mul_w16<3, DIR>(y3[1]); y3[2] = mul_w16<6, DIR>(y3[2]); y3[3] = mul_w16<9, DIR>(y3[3]);
+#pragma unroll
+  for (int k1 = 0; k1 < 4; ++k1) {
+    cd a = y0[k1], b = y1[k1], c = y2[k1], d = y3[k1];
+    bf4<DIR>(a, b, c, d);
+    x[k1] = a; x[k1 + 4] = b; x[k1 + 8] = c; x[k1 + 12] = d;
+  }
+}
+template <int R, int DIR> GD_HD void butterfly(cd (&x)[R]) {
+  if constexpr (R == 2) bf2<DIR>(x);
+  else if constexpr (R == 4) bf4<DIR>(x);
+  else if constexpr (R == 8) bf8<DIR>(x);
+  else bf16<DIR>(x);
+}
+
+// ---- plan: N -> lanes per FFT, elements per lane, stage radices -------------------------------
+template <int N> struct FftPlan;
+template <> struct FftPlan<2>   { static constexpr int T = 1,  E = 2,  S = 1, R0 = 2,  R1 = 1,  R2 = 1; };
+template <> struct FftPlan<4>   { static constexpr int T = 1,  E = 4,  S = 1, R0 = 4,  R1 = 1,  R2 = 1; };
+template <> struct FftPlan<8>   { static constexpr int T = 1,  E = 8,  S = 1, R0 = 8,  R1 = 1,  R2 = 1; };
+template <> struct FftPlan<16>  { static constexpr int T = 1,  E = 16, S = 1, R0 = 16, R1 = 1,  R2 = 1; };
+template <> struct FftPlan<32>  { static constexpr int T = 4,  E = 8,  S = 2, R0 = 8,  R1 = 4,  R2 = 1; };
+template <> struct FftPlan<64>  { static constexpr int T = 8,  E = 8,  S = 2, R0 = 8,  R1 = 8,  R2 = 1; };
+template <> struct FftPlan<128> { static constexpr int T = 8,  E = 16, S = 2, R0 = 16, R1 = 8,  R2 = 1; };
+template <> struct FftPlan<256> { static constexpr int T = 16, E = 16, S = 2, R0 = 16, R1 = 16, R2 = 1; };
+template <> struct FftPlan<512> { static constexpr int T = 32, E = 16, S = 3, R0 = 8,  R1 = 8,  R2 = 8; };
+
+template <int N> struct FftGeom {
+  using P = FftPlan<N>;
+  static constexpr int T = P::T, E = P::E, S = P::S;
+  static constexpr int PADDIV = P::R0;                     // pad(idx) = idx + idx / R0
+  static constexpr int BUF = (S > 1) ? (N + N / PADDIV) : 0;  // complex entries of the line buffer
+  GD_HD static int pad(int idx) { return idx + idx / PADDIV; }
+  template <int s> static constexpr int radix() { return s == 0 ? P::R0 : (s == 1 ? P::R1 : P::R2); }
+  template <int s> static constexpr int ns() { return s == 0 ? 1 : (s == 1 ? P::R0 : P::R0 * P::R1); }
+};
+
+// Stage s, compute phase: twiddle (table tw[p] = exp(-2 pi i p / N), conjugated for DIR=+1) and
+// radix butterflies on the lane's own registers.  Results stay at v[b + i*B].
+template <int N, int DIR, int s> GD_HD void fft_stage_compute(cd (&v)[FftPlan<N>::E], int t, const cd* __restrict__ tw) {
+  using G = FftGeom<N>;
+  constexpr int R = G::template radix<s>();
+  constexpr int NS = G::template ns<s>();
+  constexpr int B = G::E / R;                 // butterflies per lane in this stage
+  constexpr int STRIDE = N / (NS * R);        // table stride of w_{NS*R}
+#pragma unroll
+  for (int b = 0; b < B; ++b) {
+    cd x[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) x[i] = v[b + i * B];
+    if constexpr (NS > 1) {
+      const int k = (t + G::T * b) % NS;
+#pragma unroll
+      for (int i = 1; i < R; ++i) {
+#if defined(__CUDA_ARCH__)
+        const double2 w2 = __ldg(reinterpret_cast<const double2*>(tw) + i * k * STRIDE);
+        cd w = cmake(w2.x, w2.y);
+#else
+        cd w = tw[i * k * STRIDE];
+#endif
+        if (DIR > 0) w.y = -w.y;
+        x[i] = cmul(x[i], w);
+      }
+    }
+    butterfly<R, DIR>(x);
+#pragma unroll
+    for (int i = 0; i < R; ++i) v[b + i * B] = x[i];
+  }
+}
+
+// Stage s, scatter phase: write the lane's results to the line buffer at the Stockham positions.
+template <int N, int s> GD_HD void fft_stage_scatter(const cd (&v)[FftPlan<N>::E], int t, cd* buf) {
+  using G = FftGeom<N>;
+  constexpr int R = G::template radix<s>();
+  constexpr int NS = G::template ns<s>();
+  constexpr int B = G::E / R;
+#pragma unroll
+  for (int b = 0; b < B; ++b) {
+    const int j = t + G::T * b;
+    const int j0 = (j / NS) * NS * R + (j % NS);
+#pragma unroll
+    for (int i = 0; i < R; ++i) buf[G::pad(j0 + i * NS)] = v[b + i * B];
+  }
+}
+
+// Gather phase: read back the lane's own distribution v[q] = buf[t + T q].
+template <int N> GD_HD void fft_gather(cd (&v)[FftPlan<N>::E], int t, const cd* buf) {
+  using G = FftGeom<N>;
+#pragma unroll
+  for (int q = 0; q < G::E; ++q) v[q] = buf[G::pad(t + G::T * q)];
+}
+
+#if defined(__CUDACC__)
+// The cooperative transform.  buf: this line's shared buffer (FftGeom<N>::BUF entries; unused if S==1).
+template <int N, int DIR> __device__ __forceinline__ void fft_lanes(cd (&v)[FftPlan<N>::E], int t, cd* buf,
+                                                                     const cd* __restrict__ tw) {
+  using G = FftGeom<N>;
+  fft_stage_compute<N, DIR, 0>(v, t, tw);
+  if constexpr (G::S > 1) {
+    fft_stage_scatter<N, 0>(v, t, buf);
+    __syncwarp();
+    fft_gather<N>(v, t, buf);
+    __syncwarp();
+    fft_stage_compute<N, DIR, 1>(v, t, tw);
+  }
+  if constexpr (G::S > 2) {
+    fft_stage_scatter<N, 1>(v, t, buf);
+    __syncwarp();
+    fft_gather<N>(v, t, buf);
+    __syncwarp();
+    fft_stage_compute<N, DIR, 2>(v, t, tw);
+  }
+}
+#endif

@@ -1,0 +1,189 @@
+// pass_x.cu -- P2, the fused row pass of the RHS pipeline (one lane group per (y,z) line).
+//
+// For every source field f in {xi+, xi-, w+, w-, g_m} the pass reads the two half-lines
+// f~(kx; y,z) and (df/dy)~(kx; y,z) that P1 wrote (retained kx only), forms
+//     Z(kx) = i kx f~(kx) + i (df/dy)~(kx)          for kx >= 0       (Eq. 10)
+//     Z(-kx) = conj(i kx f~) + i conj((df/dy)~)                        (Hermitian completion)
+// and ONE complex inverse FFT of length nx returns (df/dx) + i (df/dy) on the real line -- the
+// derivative fields exist only in registers.  Bracket products:
+//     A = {xi+,w-} + {xi-,w+},  B = {xi+,xi-}                          (Eq. 1)
+//     P_m = {Phi,g_m}, Q_m = {Psi,g_m},  R_m = -P_m + dn_m Q_{m-1} + up_m Q_{m+1}   (Eq. 6)
+// with {P,Q} = Px Qy - Py Qx.  R_m is combined in real space with a sliding window over m (linear,
+// so one forward transform per moment instead of two).  Pairs of real lines (A,B), (R_m,R_{m+1}) go
+// through ONE complex forward FFT and are separated by Hermitian symmetry; only kx <= nx/3 is
+// written (kx part of Eq. 20).  The CFL quantity max (dPhi/dx)^2+(dPhi/dy)^2
+// (Eq. 16) rides on the Elsasser part.
+#include "common.cuh"
+
+template <int NX>
+struct XGeom {
+  using G = FftGeom<NX>;
+  static constexpr int T = G::T, E = G::E;
+  static constexpr int LB = NX + NX / G::PADDIV + 1;        // line buffer (FFT exchange + unpack), complex entries
+  static constexpr int PER_GROUP = LB + 2 * NX;             // + (Phi_x,Phi_y) and (Psi_x,Psi_y) lines
+  static constexpr int GROUPS = GD_FFT_THREADS / T;
+  static constexpr size_t SMEM = (size_t)GROUPS * PER_GROUP * sizeof(cd);
+};
+
+template <int NX>
+__global__ void __launch_bounds__(GD_FFT_THREADS) k_xpass(Dims d, const cd* __restrict__ D, cd* __restrict__ Eo,
+                                                        const cd* __restrict__ tw, const double* __restrict__ cdn,
+                                                        const double* __restrict__ cup,
+                                                        unsigned long long* __restrict__ maxbits, int nlines) {
+  using X = XGeom<NX>;
+  using G = FftGeom<NX>;
+  constexpr int T = X::T, E = X::E;
+  extern __shared__ cd smem[];
+  const int grp = threadIdx.x / T, t = threadIdx.x % T;
+  const int line = blockIdx.x * X::GROUPS + grp;
+  cd* buf = smem + (size_t)grp * X::PER_GROUP;
+  cd* sPhi = buf + X::LB;          // first xi+ then Phi derivatives, layout [q][t]
+  cd* sPsi = sPhi + NX;            // first xi- then Psi derivatives
+  const bool active = line < nlines;
+  const size_t base = (size_t)(active ? line : 0) * d.Kx;     // (z*ny + y)*Kx
+  const int hx3 = d.hx3;
+  cd v[E];
+
+  // load the pair (f, df/dy) of array a, a+1 and pack Z = Fx + i Fy on the full kx line
+  auto load_pack = [&](int a) {
+    const cd* pf = D + (size_t)a * d.PD + base;
+    const cd* pfy = pf + d.PD;
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+      const int n = t + T * q;
+      cd z = cmake(0.0, 0.0);
+      if (active) {
+        if (n <= hx3) {
+          cd f = ldg_cd(pf + n), fy = ldg_cd(pfy + n);
+          if (n == 0) { f.y = 0.0; fy.y = 0.0; }
+          const double kx = d.kx0 * n;
+          // Fx = i kx f = (-kx f.y, kx f.x);  Z = Fx + i Fy
+          z = cmake(-kx * f.y - fy.y, kx * f.x + fy.x);
+        } else if (n >= NX - hx3) {
+          const int c = NX - n;
+          const cd f = ldg_cd(pf + c), fy = ldg_cd(pfy + c);
+          const double kx = d.kx0 * c;
+          // conj(Fx) + i conj(Fy) = (-kx f.y + fy.y, -kx f.x + fy.x)
+          z = cmake(-kx * f.y + fy.y, -kx * f.x + fy.x);
+        }
+      }
+      v[q] = z;
+    }
+  };
+  // forward-transform v = (U + i V) of two real lines and store U~, V~ (kx <= nx/3) to arrays e0, e1 (e1 < 0: skip)
+  auto fwd_store = [&](int e0, int e1) {
+    fft_lanes<NX, -1>(v, t, buf, tw);
+#pragma unroll
+    for (int q = 0; q < E; ++q) buf[G::pad(t + T * q)] = v[q];
+    __syncwarp();
+    if (active) {
+      cd* p0 = Eo + (size_t)e0 * d.PD + base;
+      cd* p1 = Eo + (size_t)(e1 < 0 ? e0 : e1) * d.PD + base;
+#pragma unroll
+      for (int q = 0; q < E; ++q) {
+        const int c = t + T * q;
+        if (c <= hx3) {
+          const cd z1 = buf[G::pad(c)], z2 = buf[G::pad((NX - c) & (NX - 1))];
+          st_cd(p0 + c, cmake(0.5 * (z1.x + z2.x), 0.5 * (z1.y - z2.y)));
+          if (e1 >= 0) st_cd(p1 + c, cmake(0.5 * (z1.y + z2.y), -0.5 * (z1.x - z2.x)));
+        }
+      }
+    }
+    __syncwarp();
+  };
+
+  // ---- Elsasser part: A, B --------------------------------------------------------------------
+  load_pack(0);                                   // xi+
+  fft_lanes<NX, +1>(v, t, buf, tw);
+#pragma unroll
+  for (int q = 0; q < E; ++q) sPhi[q * T + t] = v[q];
+  load_pack(2);                                   // xi-
+  fft_lanes<NX, +1>(v, t, buf, tw);
+#pragma unroll
+  for (int q = 0; q < E; ++q) sPsi[q * T + t] = v[q];
+  double A[E];
+  load_pack(6);                                   // w-
+  fft_lanes<NX, +1>(v, t, buf, tw);
+#pragma unroll
+  for (int q = 0; q < E; ++q) {
+    const cd xp = sPhi[q * T + t];
+    A[q] = xp.x * v[q].y - xp.y * v[q].x;         // {xi+, w-}
+  }
+  load_pack(4);                                   // w+
+  fft_lanes<NX, +1>(v, t, buf, tw);
+  double gmax = 0.0;
+#pragma unroll
+  for (int q = 0; q < E; ++q) {
+    const cd xp = sPhi[q * T + t], xm = sPsi[q * T + t];
+    const double a = A[q] + (xm.x * v[q].y - xm.y * v[q].x);      // + {xi-, w+}
+    const double b = xp.x * xm.y - xp.y * xm.x;                   // {xi+, xi-}
+    v[q] = cmake(a, b);
+    const cd phi = cmake(0.5 * (xp.x + xm.x), 0.5 * (xp.y + xm.y));   // grad Phi, Phi = (xi+ + xi-)/2
+    const cd psi = cmake(0.5 * (xp.x - xm.x), 0.5 * (xp.y - xm.y));   // grad Psi
+    sPhi[q * T + t] = phi;
+    sPsi[q * T + t] = psi;
+    gmax = fmax(gmax, phi.x * phi.x + phi.y * phi.y);
+  }
+  if (maxbits != nullptr) {
+    if (!active) gmax = 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) gmax = fmax(gmax, __shfl_xor_sync(0xffffffffu, gmax, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(maxbits, (unsigned long long)__double_as_longlong(gmax));
+  }
+  fwd_store(0, 1);
+
+  // ---- Hermite part: R_m with a sliding window over m ------------------------------------------
+  const int M = d.M;
+  if (M > 0) {
+    double Qp[E], Ra[E], Rd[E];
+#pragma unroll
+    for (int q = 0; q < E; ++q) { Qp[q] = 0.0; Ra[q] = 0.0; Rd[q] = 0.0; }
+    for (int m = 0; m < M; ++m) {
+      load_pack(8 + 2 * m);
+      fft_lanes<NX, +1>(v, t, buf, tw);
+      const double dn = cdn[m];
+      const double upp = (m > 0) ? cup[m - 1] : 0.0;
+      const bool emit = (m >= 1) && (((m - 1) & 1) == 1);     // R_{m-1} completes the pair (R_{m-2}, R_{m-1})
+#pragma unroll
+      for (int q = 0; q < E; ++q) {
+        const cd ph = sPhi[q * T + t], ps = sPsi[q * T + t];
+        const double gx = v[q].x, gy = v[q].y;
+        const double P = ph.x * gy - ph.y * gx;               // {Phi, g_m}
+        const double Q = ps.x * gy - ps.y * gx;               // {Psi, g_m}
+        const double rfin = Ra[q] + upp * Q;                  // R_{m-1} complete
+        Ra[q] = dn * Qp[q] - P;
+        Qp[q] = Q;
+        if (emit) v[q] = cmake(Rd[q], rfin);
+        else Rd[q] = rfin;
+      }
+      if (emit) fwd_store(2 + m - 2, 2 + m - 1);
+    }
+    // R_{M-1} is complete (up_{M-1} = 0 after the closure was folded into dn)
+    if (((M - 1) & 1) == 1) {
+#pragma unroll
+      for (int q = 0; q < E; ++q) v[q] = cmake(Rd[q], Ra[q]);
+      fwd_store(2 + M - 2, 2 + M - 1);
+    } else {
+#pragma unroll
+      for (int q = 0; q < E; ++q) v[q] = cmake(Ra[q], 0.0);
+      fwd_store(2 + M - 1, -1);
+    }
+  }
+}
+
+cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
+                         unsigned long long* maxbits, cudaStream_t st, bool prepare_only) {
+  const int nlines = d.ny * d.nz;
+#define XCASE(NN)                                                                                             \
+  {                                                                                                           \
+    using X = XGeom<NN>;                                                                                      \
+    if (prepare_only) return cudaFuncSetAttribute(k_xpass<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X::SMEM); \
+    k_xpass<NN><<<(nlines + X::GROUPS - 1) / X::GROUPS, GD_FFT_THREADS, X::SMEM, st>>>(d, D, Eo, tw, cdn, cup, maxbits, nlines); \
+  }
+  switch (d.nx) {
+    case 8: XCASE(8) break; case 16: XCASE(16) break; case 32: XCASE(32) break; case 64: XCASE(64) break;
+    case 128: XCASE(128) break; case 256: XCASE(256) break; case 512: XCASE(512) break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaGetLastError();
+}

@@ -1,0 +1,208 @@
+"""Thin Python binding over the C-ABI CUDA library (include/gandalf.h).  Argument marshalling only:
+every step of the hot path runs in the library's own sm_100a kernels.  PyTorch supplies device
+memory and streams when the caller wants device-resident arrays; numpy arrays go through the
+host-pointer entry points.  There is no CPU fallback: a missing library is a hard error.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libgandalf.so")
+
+OK, ERR_INVALID, ERR_CUDA, ERR_NONFINITE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4
+KERNEL_CLASSES = ("z_inverse", "y_inverse_P1", "x_pass_P2", "y_forward_P3", "z_forward", "update")
+
+
+class GandalfParams(C.Structure):
+    """Mirror of `gandalf_params` (include/gandalf.h)."""
+    _fields_ = [
+        ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("M", C.c_int),
+        ("Lx", C.c_double), ("Ly", C.c_double), ("Lz", C.c_double), ("vA", C.c_double),
+        ("eta", C.c_double), ("r", C.c_int), ("eta_normalized", C.c_int),
+        ("eta_z", C.c_double), ("r_z", C.c_int),
+        ("eta_g", C.c_double),
+        ("nu_coll", C.c_double), ("p", C.c_double),
+        ("closure", C.c_int), ("if_variant", C.c_int), ("g_sign", C.c_int), ("nonlinear", C.c_int),
+        ("hermite_coeff", C.c_int),
+        ("force_eps", C.c_double), ("force_nperp_min", C.c_int), ("force_nperp_max", C.c_int),
+        ("force_nz_max", C.c_int),
+        ("seed", C.c_ulonglong),
+        ("cfl", C.c_double),
+        ("device", C.c_int),
+        ("stream", C.c_void_p),
+    ]
+
+
+class GandalfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"gandalf error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libgandalf.so (built in-tree by csrc/build.py).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2511_21891_b200.csrc.build` "
+                          "(__graft_entry__.build()); there is no CPU fallback")
+    lib = C.CDLL(LIB_PATH)
+    V, D, I = C.c_void_p, C.c_double, C.c_int
+    PD = C.POINTER(C.c_double)
+    lib.gandalf_default_params.argtypes = [C.POINTER(GandalfParams)]
+    lib.gandalf_create.argtypes = [C.POINTER(GandalfParams), C.POINTER(V)]
+    lib.gandalf_destroy.argtypes = [V]
+    lib.gandalf_set_state.argtypes = [V, V, V, I]
+    lib.gandalf_get_state.argtypes = [V, V, V, I]
+    lib.gandalf_rhs.argtypes = [V, V, V, I]
+    lib.gandalf_step.argtypes = [V, D, I]
+    lib.gandalf_energy.argtypes = [V, PD]
+    lib.gandalf_kperp_spectrum.argtypes = [V, I, I, PD]
+    lib.gandalf_energy_history.argtypes = [V, I, PD, C.POINTER(I)]
+    lib.gandalf_get_time.argtypes = [V, PD, C.POINTER(C.c_longlong), PD]
+    lib.gandalf_launch_count.argtypes = [V]
+    lib.gandalf_launch_count.restype = C.c_longlong
+    lib.gandalf_kernel_timing.argtypes = [V, I]
+    lib.gandalf_kernel_time_ms.argtypes = [V, I, PD, C.POINTER(C.c_longlong)]
+    lib.gandalf_last_error.argtypes = [V]
+    lib.gandalf_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _is_torch(x):
+    return type(x).__module__.startswith("torch")
+
+
+class Gandalf:
+    """One solver context.  Boundary arrays: complex128, shape (fields, nz, ny, nx//2+1); zeta = the
+    Elsasser potentials xi^+, xi^- (2 fields), g = Hermite moments g_0..g_{M-1}.
+    numpy arrays use the host entry points; torch CUDA tensors are passed as device pointers."""
+
+    def __init__(self, nx, ny, nz, M=0, device=0, stream=None, **kw):
+        self._h = None
+        lib = load_library()
+        p = GandalfParams()
+        lib.gandalf_default_params(C.byref(p))
+        p.nx, p.ny, p.nz, p.M, p.device = nx, ny, nz, M, device
+        names = {f[0] for f in GandalfParams._fields_}
+        for k, v in kw.items():
+            if k not in names:
+                raise TypeError(f"unknown gandalf parameter {k!r}")
+            setattr(p, k, v)
+        if stream is not None:
+            p.stream = int(stream)
+        self.params = p
+        self.nx, self.ny, self.nz, self.M, self.hx = nx, ny, nz, M, nx // 2 + 1
+        h = C.c_void_p()
+        rc = lib.gandalf_create(C.byref(p), C.byref(h))
+        if rc != OK:
+            raise GandalfError(rc, "gandalf_create failed (invalid parameters, unsupported combination or CUDA error)")
+        self._h, self._lib = h, lib
+
+    # -- plumbing -------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.gandalf_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ck(self, rc):
+        if rc != OK:
+            raise GandalfError(rc, self._lib.gandalf_last_error(self._h).decode())
+
+    def _shape(self, nf):
+        return (nf, self.nz, self.ny, self.hx)
+
+    def _in_ptr(self, a, nf):
+        """(pointer, on_device, keepalive) for an input array."""
+        if a is None:
+            return None, None, None
+        if _is_torch(a):
+            import torch
+            assert a.is_cuda and a.dtype == torch.complex128 and a.is_contiguous() and tuple(a.shape) == self._shape(nf)
+            return C.c_void_p(a.data_ptr()), 1, a
+        arr = np.ascontiguousarray(a, dtype=np.complex128)
+        assert arr.shape == self._shape(nf), (arr.shape, self._shape(nf))
+        return C.c_void_p(arr.ctypes.data), 0, arr
+
+    # -- API ------------------------------------------------------------------------------------
+    def set_state(self, zeta_hat, g_hat=None):
+        zp, dev, k1 = self._in_ptr(zeta_hat, 2)
+        gp, dev2, k2 = self._in_ptr(g_hat, self.M) if self.M > 0 else (None, dev, None)
+        assert dev == dev2, "zeta and g must both be host or both be device arrays"
+        self._ck(self._lib.gandalf_set_state(self._h, zp, gp, dev))
+
+    def _out(self, like_torch, nf):
+        if like_torch:
+            import torch
+            t = torch.empty(self._shape(max(nf, 1)), dtype=torch.complex128, device=f"cuda:{self.params.device}")
+            return t, C.c_void_p(t.data_ptr())
+        a = np.empty(self._shape(max(nf, 1)), dtype=np.complex128)
+        return a, C.c_void_p(a.ctypes.data)
+
+    def get_state(self, device=False):
+        z, zp = self._out(device, 2)
+        g, gp = self._out(device, self.M)
+        self._ck(self._lib.gandalf_get_state(self._h, zp, gp, int(bool(device))))
+        return z, g[: self.M]
+
+    def rhs(self, device=False):
+        dw, wp = self._out(device, 2)
+        dg, gp = self._out(device, self.M)
+        self._ck(self._lib.gandalf_rhs(self._h, wp, gp, int(bool(device))))
+        return dw, dg[: self.M]
+
+    def step(self, dt, nsteps=1):
+        self._ck(self._lib.gandalf_step(self._h, float(dt), int(nsteps)))
+
+    def energy(self):
+        out = np.zeros(6)
+        self._ck(self._lib.gandalf_energy(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def kperp_spectrum(self, nbins, literal_eq26=False):
+        out = np.zeros(nbins)
+        self._ck(self._lib.gandalf_kperp_spectrum(self._h, nbins, int(literal_eq26), out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def energy_history(self, max_records=None):
+        _, nstep, _ = self.time()
+        k = nstep if max_records is None else min(nstep, max_records)
+        buf = np.zeros((max(k, 1), 7))
+        n = C.c_int(0)
+        self._ck(self._lib.gandalf_energy_history(self._h, k, buf.ctypes.data_as(C.POINTER(C.c_double)), C.byref(n)))
+        return buf[: n.value].copy()
+
+    def time(self):
+        t, s, d = C.c_double(0), C.c_longlong(0), C.c_double(0)
+        self._ck(self._lib.gandalf_get_time(self._h, C.byref(t), C.byref(s), C.byref(d)))
+        return t.value, s.value, d.value
+
+    def launch_count(self):
+        return int(self._lib.gandalf_launch_count(self._h))
+
+    def kernel_timing(self, enable=True):
+        self._ck(self._lib.gandalf_kernel_timing(self._h, int(bool(enable))))
+
+    def kernel_times(self):
+        """{class name: (average ms per launch, launches)} since timing was enabled."""
+        out = {}
+        for i, name in enumerate(KERNEL_CLASSES):
+            ms, n = C.c_double(0), C.c_longlong(0)
+            self._ck(self._lib.gandalf_kernel_time_ms(self._h, i, C.byref(ms), C.byref(n)))
+            out[name] = (ms.value, n.value)
+        return out

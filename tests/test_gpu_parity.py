@@ -1,0 +1,225 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json north_star's: 1e-12 relative L2 per RHS evaluation,
+1e-10 after 10 steps, 1e-9 on energy histories."""
+import numpy as np
+import pytest
+
+from cases import config0, config1, config2, config3, rel_l2
+from paper_2511_21891_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHS, TOL_10STEPS, TOL_ENERGY = 1e-12, 1e-10, 1e-9
+
+
+def _pair(shape, prm):
+    from oracle import Oracle
+    from paper_2511_21891_b200.gandalf import Gandalf
+    nx, ny, nz = shape
+    o = Oracle(nx, ny, nz, **prm)
+    g = Gandalf(nx, ny, nz, **prm)
+    return o, g
+
+
+def _check_rhs(o, g, tol=TOL_RHS):
+    dw_o, dg_o = o.rhs()
+    dw_g, dg_g = g.rhs()
+    for a in range(2):
+        assert rel_l2(dw_g[a], dw_o[a]) <= tol, ("dw", a, rel_l2(dw_g[a], dw_o[a]))
+    if o.M:
+        # per moment, relative to the largest moment's RHS norm (moments that start at zero have tiny RHS)
+        ref = max(np.linalg.norm(dg_o[m]) for m in range(o.M))
+        for m in range(o.M):
+            assert np.linalg.norm(dg_g[m] - dg_o[m]) <= tol * ref, ("dg", m)
+        assert rel_l2(dg_g, dg_o) <= tol
+    # removed modes are exactly zero on the GPU side too
+    assert np.count_nonzero(dw_g[:, :, :, o.nx // 3 + 1:]) == 0
+
+
+def _check_state(o, g, tol):
+    zo, go = o.get_state()
+    zg, gg = g.get_state()
+    assert rel_l2(zg, zo) <= tol, rel_l2(zg, zo)
+    if o.M:
+        assert rel_l2(gg, go) <= tol, rel_l2(gg, go)
+
+
+def _check_history(o, g, tol=TOL_ENERGY):
+    ho, hg = o.energy_history(), g.energy_history()
+    assert ho.shape == hg.shape and ho.shape[0] > 0
+    assert np.abs(hg[:, 0] - ho[:, 0]).max() <= 1e-12 * max(1.0, abs(ho[-1, 0]))
+    scale = np.abs(ho[:, 1:]).max(axis=0)
+    for k in range(6):
+        if scale[k] > 0:
+            assert np.abs(hg[:, 1 + k] - ho[:, 1 + k]).max() <= tol * scale[k], k
+
+
+def test_config0_rmhd_decay():
+    prm, z, _, run = config0()
+    o, g = _pair(run["shape"], prm)
+    o.set_state(z); g.set_state(z)
+    _check_state(o, g, 1e-14)
+    assert np.abs(g.energy() - o.energy()).max() <= 1e-13
+    _check_rhs(o, g)
+    o.step(run["dt"], 10); g.step(run["dt"], 10)
+    _check_state(o, g, TOL_10STEPS)
+    o.step(run["dt"], 90); g.step(run["dt"], 90)
+    _check_state(o, g, 1e-9)
+    _check_history(o, g)
+    assert g.time()[1] == 100 and abs(g.time()[0] - 0.1) < 1e-12
+
+
+def test_config2_krmhd_hermite():
+    prm, z, gm, run = config2()
+    o, g = _pair(run["shape"], prm)
+    o.set_state(z, gm); g.set_state(z, gm)
+    _check_rhs(o, g)
+    o.step(run["dt"], 10); g.step(run["dt"], 10)
+    _check_state(o, g, TOL_10STEPS)
+    _check_rhs(o, g)                      # RHS on an evolved state (all moments populated up to m=10)
+    o.step(run["dt"], 30); g.step(run["dt"], 30)
+    _check_history(o, g)
+
+
+@pytest.mark.parametrize("shape,M", [((8, 8, 2), 0), ((16, 8, 4), 1), ((8, 16, 8), 2), ((32, 64, 16), 3),
+                                     ((64, 32, 8), 5), ((128, 16, 4), 2), ((16, 128, 4), 2), ((256, 8, 2), 1),
+                                     ((8, 256, 2), 1), ((512, 8, 2), 1), ((8, 512, 2), 2), ((8, 8, 64), 2),
+                                     ((8, 8, 128), 1), ((8, 8, 256), 1), ((8, 8, 512), 1), ((16, 16, 32), 4)])
+def test_rhs_all_transform_sizes_dense_state(shape, M):
+    """Every FFT length on every axis, ragged tails, dense random input incl. modes set_state must project out."""
+    nx, ny, nz = shape
+    prm = dict(M=M)
+    o, g = _pair(shape, prm)
+    z = synth.dense_random(nx, ny, nz, 2, seed=nx + 3 * ny + 7 * nz)
+    gm = synth.dense_random(nx, ny, nz, M, seed=99 + nx) if M else None
+    o.set_state(z, gm); g.set_state(z, gm)
+    _check_state(o, g, 1e-14)
+    _check_rhs(o, g)
+    o.step(1e-3, 2); g.step(1e-3, 2)
+    _check_state(o, g, TOL_10STEPS)
+
+
+@pytest.mark.parametrize("opts", [dict(if_variant=1), dict(closure=1), dict(g_sign=-1), dict(hermite_coeff=1),
+                                  dict(nonlinear=0), dict(eta=0.5, r=3, eta_normalized=1, eta_z=0.2, r_z=2, eta_g=0.3,
+                                                          nu_coll=0.7, p=1.5),
+                                  dict(Lx=3.0, Ly=5.0, Lz=11.0)])
+def test_variants_and_options(opts):
+    shape, M = (32, 16, 8), 4
+    prm = dict(M=M, **opts)
+    o, g = _pair(shape, prm)
+    z = synth.dense_random(*shape, 2, seed=5)
+    gm = synth.dense_random(*shape, M, seed=6)
+    o.set_state(z, gm); g.set_state(z, gm)
+    _check_rhs(o, g)
+    o.step(2e-3, 10); g.step(2e-3, 10)
+    _check_state(o, g, TOL_10STEPS)
+    _check_history(o, g)
+
+
+def test_rmhd_with_va_not_one():
+    shape = (16, 16, 8)
+    o, g = _pair(shape, dict(M=0, vA=2.5))
+    z = synth.dense_random(*shape, 2, seed=8)
+    o.set_state(z); g.set_state(z)
+    o.step(5e-3, 10); g.step(5e-3, 10)
+    _check_state(o, g, TOL_10STEPS)
+
+
+def test_alfven_wave_exact_on_gpu():
+    from paper_2511_21891_b200.gandalf import Gandalf
+    g = Gandalf(32, 32, 16)
+    z0 = synth.single_mode(32, 32, 16, (1, 0, 1), 0.01)
+    g.set_state(z0)
+    T = 2 * np.pi
+    g.step(T / 4, 4)
+    z, _ = g.get_state()
+    assert abs(z[0, 1, 0, 1] - 0.01) <= 1e-16          # one full period: back to the start
+    z[0, 1, 0, 1] = 0
+    assert np.abs(z).max() == 0.0
+
+
+def test_config3_forcing_and_cfl_window():
+    """Scaled-down config 3 (forcing + adaptive CFL dt + k_z and k_perp hyperdissipation): trajectory parity
+    over the first steps (Q20)."""
+    prm, z, gm, run = config3(32, 32, 16, 4, eta=50.0)
+    o, g = _pair(run["shape"], prm)
+    o.set_state(z, gm); g.set_state(z, gm)
+    o.step(0.0, 10); g.step(0.0, 10)
+    to, tg = o.time(), g.time()
+    assert tg[1] == 10 and abs(tg[0] - to[0]) <= 1e-12 * to[0] and abs(tg[2] - to[2]) <= 1e-12 * to[2]
+    _check_state(o, g, TOL_10STEPS)
+    _check_history(o, g)
+    so, sg = o.kperp_spectrum(24), g.kperp_spectrum(24)
+    assert np.abs(sg - so).max() <= 1e-10 * so.max()
+    assert abs(sg.sum() - g.energy()[0]) <= 1e-12 * sg.sum()
+    sl_o, sl_g = o.kperp_spectrum(24, True), g.kperp_spectrum(24, True)
+    assert np.abs(sl_g - sl_o).max() <= 1e-10 * sl_o.max()
+
+
+def test_config1_orszag_tang_energy_history():
+    prm, z, _, run = config1()
+    o, g = _pair(run["shape"], prm)
+    o.set_state(z); g.set_state(z)
+    e0 = g.energy()
+    assert abs(e0[0] - 4.0) <= 1e-13 and abs(e0[3] - 2.0) <= 1e-13 and abs(e0[4] - 2.0) <= 1e-13
+    n = 2000
+    g.step(run["dt"], n)
+    hg = g.energy_history()
+    drift = np.abs(hg[:, 1] / 4.0 - 1.0).max()
+    assert drift <= 1e-5, drift                      # paper: 1.6e-6 at 128^2 x 2
+    o.step(run["dt"], 400)                           # oracle over the first 400 steps (time budget)
+    ho = o.energy_history()
+    assert np.abs(hg[:400, 1:] - ho[:, 1:]).max() <= TOL_ENERGY * 4.0
+    assert hg[-1, 5] / hg[-1, 4] > 1.0               # selective decay direction
+
+
+def test_device_pointer_entry_points():
+    import torch
+    from oracle import Oracle
+    from paper_2511_21891_b200.gandalf import Gandalf
+    shape, M = (32, 32, 8), 3
+    z = synth.dense_random(*shape, 2, seed=1)
+    gm = synth.dense_random(*shape, M, seed=2)
+    g = Gandalf(*shape, M=M)
+    zt = torch.from_numpy(z).cuda(); gt = torch.from_numpy(gm).cuda()
+    g.set_state(zt, gt)
+    dw, dg = g.rhs(device=True)
+    torch.cuda.synchronize()
+    o = Oracle(*shape, M=M)
+    o.set_state(z, gm)
+    dw_o, dg_o = o.rhs()
+    assert rel_l2(dw.cpu().numpy(), dw_o) <= TOL_RHS and rel_l2(dg.cpu().numpy(), dg_o) <= TOL_RHS
+    # a non-default stream supplied by torch
+    s = torch.cuda.Stream()
+    g2 = Gandalf(*shape, M=M, stream=s.cuda_stream)
+    with torch.cuda.stream(s):
+        g2.set_state(zt, gt)
+        g2.step(1e-3, 3)
+    zs, gs = g2.get_state()
+    g.step(1e-3, 3)
+    z1, g1 = g.get_state()
+    assert np.array_equal(zs, z1) and np.array_equal(gs, g1)      # bit-reproducible across contexts/streams
+
+
+def test_nonfinite_is_reported():
+    from paper_2511_21891_b200.gandalf import Gandalf, GandalfError, ERR_NONFINITE
+    g = Gandalf(16, 16, 4)
+    z = synth.dense_random(16, 16, 4, 2, seed=3) * 1e200
+    g.set_state(z)
+    g.step(1.0, 3)
+    with pytest.raises(GandalfError) as ei:
+        g.energy_history()
+    assert ei.value.code == ERR_NONFINITE
+
+
+def test_launch_count_and_kernel_timing():
+    from paper_2511_21891_b200.gandalf import Gandalf
+    prm, z, gm, run = config2(32, 32, 16, 4)
+    g = Gandalf(*run["shape"], **prm)
+    g.set_state(z, gm)
+    n0 = g.launch_count()
+    g.kernel_timing(True)
+    g.step(run["dt"], 2)
+    kt = g.kernel_times()
+    assert g.launch_count() - n0 == 2 * 15
+    assert kt["x_pass_P2"][1] == 4 and kt["x_pass_P2"][0] > 0
