@@ -1,9 +1,9 @@
-"""Workload definitions shared by the parity tests, smoke() and bench.py: the BASELINE.json configs
+"""Workload definitions shared by the parity tests, smoke() and bench.py (no CUDA, no oracle import): the BASELINE.json configs
 as (parameter dict, seeded inputs).  The dicts use the parameter names common to gandalf_params and
 the oracle; nothing here computes any of the method's arithmetic."""
 import numpy as np
 
-from paper_2511_21891_b200 import synth
+from . import synth
 
 
 def config0(nx=32, ny=32, nz=16, seed=1000):
