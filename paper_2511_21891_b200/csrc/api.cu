@@ -73,12 +73,14 @@ static bool pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
 template <class T> static cudaError_t dalloc(T** p, size_t count) { return cudaMalloc((void**)p, count * sizeof(T)); }
 
+int fft_stage_table_host(int n, std::vector<cd>& out);
+
 static cudaError_t upload_twiddles(cd** dst, int n, cudaStream_t st) {
-  std::vector<cd> h(n);
-  for (int k = 0; k < n; ++k) { h[k].x = std::cos(2.0 * kPi * k / n); h[k].y = -std::sin(2.0 * kPi * k / n); }
-  cudaError_t e = dalloc(dst, (size_t)n);
+  std::vector<cd> h;
+  if (fft_stage_table_host(n, h) != 0) return cudaErrorInvalidValue;
+  cudaError_t e = dalloc(dst, h.size());
   if (e != cudaSuccess) return e;
-  e = cudaMemcpyAsync(*dst, h.data(), n * sizeof(cd), cudaMemcpyHostToDevice, st);
+  e = cudaMemcpyAsync(*dst, h.data(), h.size() * sizeof(cd), cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) return e;
   return cudaStreamSynchronize(st);
 }

@@ -13,6 +13,7 @@
 //
 // Sign convention: DIR = -1 forward kernel exp(-2 pi i jk/N), DIR = +1 inverse; no scaling.
 #pragma once
+#include <cmath>
 
 #if defined(__CUDACC__)
 #define GD_HD __host__ __device__ __forceinline__
@@ -129,14 +130,40 @@ template <int N> struct FftGeom {
   template <int s> static constexpr int ns() { return s == 0 ? 1 : (s == 1 ? P::R0 : P::R0 * P::R1); }
 };
 
-// Stage s, compute phase: twiddle (table tw[p] = exp(-2 pi i p / N), conjugated for DIR=+1) and
-// radix butterflies on the lane's own registers.  Results stay at v[b + i*B].
-template <int N, int DIR, int s> GD_HD void fft_stage_compute(cd (&v)[FftPlan<N>::E], int t, const cd* __restrict__ tw) {
+// Stage twiddles live in a per-N "stage table" (copied to shared memory by every kernel): for each stage
+// s >= 1 the entries  tws[OFF_s + (i-1)*NS_s + k] = exp(-2 pi i * i*k / (NS_s*R_s)),  i = 1..R_s-1, k = 0..NS_s-1,
+// so that consecutive lanes (consecutive k) read consecutive 16-byte words: conflict-free LDS.128.
+template <int N> struct FftTw {
+  using G = FftGeom<N>;
+  static constexpr int CNT1 = (G::S > 1) ? (G::template radix<1>() - 1) * G::template ns<1>() : 0;
+  static constexpr int CNT2 = (G::S > 2) ? (G::template radix<2>() - 1) * G::template ns<2>() : 0;
+  static constexpr int COUNT = CNT1 + CNT2;
+  template <int s> static constexpr int off() { return s == 1 ? 0 : CNT1; }
+};
+
+template <int N> inline void fft_fill_stage_table(cd* out) {   // host side, libm cos/sin per entry
+  using G = FftGeom<N>;
+  const double PI2 = 6.28318530717958647692528676655900577;
+  int o = 0;
+  if constexpr (G::S > 1) {
+    constexpr int R = G::template radix<1>(), NS = G::template ns<1>();
+    for (int i = 1; i < R; ++i)
+      for (int k = 0; k < NS; ++k) { const double a = PI2 * (double)(i * k) / (double)(NS * R); out[o++] = cmake(std::cos(a), -std::sin(a)); }
+  }
+  if constexpr (G::S > 2) {
+    constexpr int R = G::template radix<2>(), NS = G::template ns<2>();
+    for (int i = 1; i < R; ++i)
+      for (int k = 0; k < NS; ++k) { const double a = PI2 * (double)(i * k) / (double)(NS * R); out[o++] = cmake(std::cos(a), -std::sin(a)); }
+  }
+}
+
+// Stage s, compute phase: twiddle (stage table, conjugated for DIR=+1) and radix butterflies on the lane's
+// own registers.  Results stay at v[b + i*B].
+template <int N, int DIR, int s> GD_HD void fft_stage_compute(cd (&v)[FftPlan<N>::E], int t, const cd* __restrict__ tws) {
   using G = FftGeom<N>;
   constexpr int R = G::template radix<s>();
   constexpr int NS = G::template ns<s>();
   constexpr int B = G::E / R;                 // butterflies per lane in this stage
-  constexpr int STRIDE = N / (NS * R);        // table stride of w_{NS*R}
 #pragma unroll
   for (int b = 0; b < B; ++b) {
     cd x[R];
@@ -144,14 +171,10 @@ template <int N, int DIR, int s> GD_HD void fft_stage_compute(cd (&v)[FftPlan<N>
     for (int i = 0; i < R; ++i) x[i] = v[b + i * B];
     if constexpr (NS > 1) {
       const int k = (t + G::T * b) % NS;
+      const cd* tb = tws + FftTw<N>::template off<s>() + k;
 #pragma unroll
       for (int i = 1; i < R; ++i) {
-#if defined(__CUDA_ARCH__)
-        const double2 w2 = __ldg(reinterpret_cast<const double2*>(tw) + i * k * STRIDE);
-        cd w = cmake(w2.x, w2.y);
-#else
-        cd w = tw[i * k * STRIDE];
-#endif
+        cd w = tb[(i - 1) * NS];
         if (DIR > 0) w.y = -w.y;
         x[i] = cmul(x[i], w);
       }
@@ -185,24 +208,30 @@ template <int N> GD_HD void fft_gather(cd (&v)[FftPlan<N>::E], int t, const cd* 
 }
 
 #if defined(__CUDACC__)
-// The cooperative transform.  buf: this line's shared buffer (FftGeom<N>::BUF entries; unused if S==1).
+// The cooperative transform.  buf: this line's shared buffer (FftGeom<N>::BUF entries; unused if S==1);
+// tws: the stage table (FftTw<N>::COUNT entries), normally in shared memory.
+// Copy helper: all threads of the CTA, followed by __syncthreads().
+template <int N> __device__ __forceinline__ void fft_load_table(cd* dst, const cd* __restrict__ src) {
+  for (int i = threadIdx.x; i < FftTw<N>::COUNT; i += blockDim.x) dst[i] = src[i];
+  __syncthreads();
+}
 template <int N, int DIR> __device__ __forceinline__ void fft_lanes(cd (&v)[FftPlan<N>::E], int t, cd* buf,
-                                                                     const cd* __restrict__ tw) {
+                                                                     const cd* __restrict__ tws) {
   using G = FftGeom<N>;
-  fft_stage_compute<N, DIR, 0>(v, t, tw);
+  fft_stage_compute<N, DIR, 0>(v, t, tws);
   if constexpr (G::S > 1) {
     fft_stage_scatter<N, 0>(v, t, buf);
     __syncwarp();
     fft_gather<N>(v, t, buf);
     __syncwarp();
-    fft_stage_compute<N, DIR, 1>(v, t, tw);
+    fft_stage_compute<N, DIR, 1>(v, t, tws);
   }
   if constexpr (G::S > 2) {
     fft_stage_scatter<N, 1>(v, t, buf);
     __syncwarp();
     fft_gather<N>(v, t, buf);
     __syncwarp();
-    fft_stage_compute<N, DIR, 2>(v, t, tw);
+    fft_stage_compute<N, DIR, 2>(v, t, tws);
   }
 }
 #endif

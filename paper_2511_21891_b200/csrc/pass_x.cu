@@ -20,13 +20,16 @@ struct XGeom {
   using G = FftGeom<NX>;
   static constexpr int T = G::T, E = G::E;
   static constexpr int LB = NX + NX / G::PADDIV + 1;        // line buffer (FFT exchange + unpack), complex entries
-  static constexpr int PER_GROUP = LB + 2 * NX;             // + (Phi_x,Phi_y) and (Psi_x,Psi_y) lines
-  static constexpr int GROUPS = GD_FFT_THREADS / T;
-  static constexpr size_t SMEM = (size_t)GROUPS * PER_GROUP * sizeof(cd);
+  static constexpr int KXP = NX / 3 + 1;                    // retained kx count (== Dims::Kx)
+  static constexpr int STG = 2 * KXP;                       // staging buffer: the two half-lines (f, df/dy) of the NEXT field
+  static constexpr int PER_GROUP = LB + 2 * NX + STG;       // + (Phi_x,Phi_y) and (Psi_x,Psi_y) lines + staging
+  static constexpr int THREADS = 224;                       // 7 warps, one CTA per SM: shared memory is the limiter
+  static constexpr int GROUPS = THREADS / T;
+  static constexpr size_t SMEM = ((size_t)GROUPS * PER_GROUP + FftTw<NX>::COUNT) * sizeof(cd);
 };
 
 template <int NX>
-__global__ void __launch_bounds__(GD_FFT_THREADS) k_xpass(Dims d, const cd* __restrict__ D, cd* __restrict__ Eo,
+__global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const cd* __restrict__ D, cd* __restrict__ Eo,
                                                         const cd* __restrict__ tw, const double* __restrict__ cdn,
                                                         const double* __restrict__ cup,
                                                         unsigned long long* __restrict__ maxbits, int nlines) {
@@ -36,7 +39,9 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_xpass(Dims d, const cd* __re
   extern __shared__ cd smem[];
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   const int line = blockIdx.x * X::GROUPS + grp;
-  cd* buf = smem + (size_t)grp * X::PER_GROUP;
+  cd* buf = smem + FftTw<NX>::COUNT + (size_t)grp * X::PER_GROUP;
+  fft_load_table<NX>(smem, tw);
+  const cd* tws = smem;
   cd* sPhi = buf + X::LB;          // first xi+ then Phi derivatives, layout [q][t]
   cd* sPsi = sPhi + NX;            // first xi- then Psi derivatives
   const bool active = line < nlines;
@@ -44,24 +49,39 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_xpass(Dims d, const cd* __re
   const int hx3 = d.hx3;
   cd v[E];
 
-  // load the pair (f, df/dy) of array a, a+1 and pack Z = Fx + i Fy on the full kx line
-  auto load_pack = [&](int a) {
-    const cd* pf = D + (size_t)a * d.PD + base;
-    const cd* pfy = pf + d.PD;
+  cd* sStage = sPsi + NX;          // [0,Kx): f~(kx), [Kx,2Kx): (df/dy)~(kx) of the field being fetched
+  // asynchronous fetch (cp.async, 16 B per lane) of the two half-lines of array a, a+1 into the staging buffer
+  auto fetch = [&](int a) {
+    if (active) {
+      const cd* pf = D + (size_t)a * d.PD + base;
+      const unsigned sbase = (unsigned)__cvta_generic_to_shared(sStage);
+      for (int c = t; c < 2 * d.Kx; c += T) {
+        const cd* src = (c < d.Kx) ? pf + c : pf + d.PD + (c - d.Kx);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sbase + 16u * (unsigned)c), "l"(src) : "memory");
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  // wait for the staged half-lines, pack Z = Fx + i Fy on the full kx line into v, then start fetching array `next`
+  auto load_pack = [&](int next) {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncwarp();
+    const cd* pf = sStage;
+    const cd* pfy = sStage + d.Kx;
 #pragma unroll
     for (int q = 0; q < E; ++q) {
       const int n = t + T * q;
       cd z = cmake(0.0, 0.0);
       if (active) {
         if (n <= hx3) {
-          cd f = ldg_cd(pf + n), fy = ldg_cd(pfy + n);
+          cd f = pf[n], fy = pfy[n];
           if (n == 0) { f.y = 0.0; fy.y = 0.0; }
           const double kx = d.kx0 * n;
           // Fx = i kx f = (-kx f.y, kx f.x);  Z = Fx + i Fy
           z = cmake(-kx * f.y - fy.y, kx * f.x + fy.x);
         } else if (n >= NX - hx3) {
           const int c = NX - n;
-          const cd f = ldg_cd(pf + c), fy = ldg_cd(pfy + c);
+          const cd f = pf[c], fy = pfy[c];
           const double kx = d.kx0 * c;
           // conj(Fx) + i conj(Fy) = (-kx f.y + fy.y, -kx f.x + fy.x)
           z = cmake(-kx * f.y + fy.y, -kx * f.x + fy.x);
@@ -69,10 +89,12 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_xpass(Dims d, const cd* __re
       }
       v[q] = z;
     }
+    __syncwarp();                   // every lane has consumed the staging buffer
+    if (next >= 0) fetch(next);
   };
   // forward-transform v = (U + i V) of two real lines and store U~, V~ (kx <= nx/3) to arrays e0, e1 (e1 < 0: skip)
   auto fwd_store = [&](int e0, int e1) {
-    fft_lanes<NX, -1>(v, t, buf, tw);
+    fft_lanes<NX, -1>(v, t, buf, tws);
 #pragma unroll
     for (int q = 0; q < E; ++q) buf[G::pad(t + T * q)] = v[q];
     __syncwarp();
@@ -93,24 +115,25 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_xpass(Dims d, const cd* __re
   };
 
   // ---- Elsasser part: A, B --------------------------------------------------------------------
-  load_pack(0);                                   // xi+
-  fft_lanes<NX, +1>(v, t, buf, tw);
+  fetch(0);
+  load_pack(2);                                   // xi+   (and start fetching xi-)
+  fft_lanes<NX, +1>(v, t, buf, tws);
 #pragma unroll
   for (int q = 0; q < E; ++q) sPhi[q * T + t] = v[q];
-  load_pack(2);                                   // xi-
-  fft_lanes<NX, +1>(v, t, buf, tw);
+  load_pack(6);                                   // xi-   (fetch w-)
+  fft_lanes<NX, +1>(v, t, buf, tws);
 #pragma unroll
   for (int q = 0; q < E; ++q) sPsi[q * T + t] = v[q];
   double A[E];
-  load_pack(6);                                   // w-
-  fft_lanes<NX, +1>(v, t, buf, tw);
+  load_pack(4);                                   // w-    (fetch w+)
+  fft_lanes<NX, +1>(v, t, buf, tws);
 #pragma unroll
   for (int q = 0; q < E; ++q) {
     const cd xp = sPhi[q * T + t];
     A[q] = xp.x * v[q].y - xp.y * v[q].x;         // {xi+, w-}
   }
-  load_pack(4);                                   // w+
-  fft_lanes<NX, +1>(v, t, buf, tw);
+  load_pack(d.M > 0 ? 8 : -1);                    // w+    (fetch g_0)
+  fft_lanes<NX, +1>(v, t, buf, tws);
   double gmax = 0.0;
 #pragma unroll
   for (int q = 0; q < E; ++q) {
@@ -139,8 +162,8 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_xpass(Dims d, const cd* __re
 #pragma unroll
     for (int q = 0; q < E; ++q) { Qp[q] = 0.0; Ra[q] = 0.0; Rd[q] = 0.0; }
     for (int m = 0; m < M; ++m) {
-      load_pack(8 + 2 * m);
-      fft_lanes<NX, +1>(v, t, buf, tw);
+      load_pack(m + 1 < M ? 8 + 2 * (m + 1) : -1);  // g_m  (fetch g_{m+1})
+      fft_lanes<NX, +1>(v, t, buf, tws);
       const double dn = cdn[m];
       const double upp = (m > 0) ? cup[m - 1] : 0.0;
       const bool emit = (m >= 1) && (((m - 1) & 1) == 1);     // R_{m-1} completes the pair (R_{m-2}, R_{m-1})
@@ -178,7 +201,7 @@ cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const
   {                                                                                                           \
     using X = XGeom<NN>;                                                                                      \
     if (prepare_only) return cudaFuncSetAttribute(k_xpass<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X::SMEM); \
-    k_xpass<NN><<<(nlines + X::GROUPS - 1) / X::GROUPS, GD_FFT_THREADS, X::SMEM, st>>>(d, D, Eo, tw, cdn, cup, maxbits, nlines); \
+    k_xpass<NN><<<(nlines + X::GROUPS - 1) / X::GROUPS, X::THREADS, X::SMEM, st>>>(d, D, Eo, tw, cdn, cup, maxbits, nlines); \
   }
   switch (d.nx) {
     case 8: XCASE(8) break; case 16: XCASE(16) break; case 32: XCASE(32) break; case 64: XCASE(64) break;

@@ -9,6 +9,7 @@
 // Every FFT is fft_lanes<N> (fft.cuh): T lanes of one warp per column, data in registers, one
 // shared-memory exchange per stage boundary.  Adjacent lane groups take adjacent cx so that global
 // accesses of a warp cover contiguous kx runs.
+#include <vector>
 #include "common.cuh"
 
 template <int NZ, int DIR>
@@ -19,7 +20,9 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_zfft(Dims d, const cd* __res
   extern __shared__ cd smem[];
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   const int gid = blockIdx.x * (GD_FFT_THREADS / T) + grp;
-  cd* buf = smem + (size_t)grp * (G::BUF + 1);
+  cd* buf = smem + FftTw<NZ>::COUNT + (size_t)grp * (G::BUF + 1);
+  fft_load_table<NZ>(smem, tw);
+  const cd* tws = smem;
   const bool active = gid < ncols;
   const int plane = d.Ky * d.Kx;
   const int f = active ? gid / plane : 0, rem = active ? gid % plane : 0;
@@ -31,7 +34,7 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_zfft(Dims d, const cd* __res
       const int cz = fft2c(t + T * q, NZ, d.hz3, d.Kz);
       v[q] = (active && cz >= 0) ? ldg_cd(src + (size_t)cz * plane) : cmake(0.0, 0.0);
     }
-    fft_lanes<NZ, +1>(v, t, buf, tw);
+    fft_lanes<NZ, +1>(v, t, buf, tws);
     if (active) {
       cd* dst = out + (size_t)f * d.PH + rem;
 #pragma unroll
@@ -41,7 +44,7 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_zfft(Dims d, const cd* __res
     const cd* src = in + (size_t)f * d.PH + rem;
 #pragma unroll
     for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * plane) : cmake(0.0, 0.0);
-    fft_lanes<NZ, -1>(v, t, buf, tw);
+    fft_lanes<NZ, -1>(v, t, buf, tws);
     if (active) {
       cd* dst = out + (size_t)f * d.PS + rem;
 #pragma unroll
@@ -63,7 +66,9 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_yinv(Dims d, const cd* __res
   extern __shared__ cd smem[];
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   const int gid = blockIdx.x * (GD_FFT_THREADS / T) + grp;
-  cd* buf = smem + (size_t)grp * (G::BUF + 1);
+  cd* buf = smem + FftTw<NY>::COUNT + (size_t)grp * (G::BUF + 1);
+  fft_load_table<NY>(smem, tw);
+  const cd* tws = smem;
   const bool active = gid < ncols;
   const int cx = active ? gid % d.Kx : 0;
   const int sz = active ? gid / d.Kx : 0;
@@ -81,7 +86,7 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_yinv(Dims d, const cd* __res
   }
   const size_t obase = (size_t)z * NY * d.Kx + cx;
   auto emit = [&](int a) {   // inverse transform v and write array a
-    fft_lanes<NY, +1>(v, t, buf, tw);
+    fft_lanes<NY, +1>(v, t, buf, tws);
     if (active) {
       cd* dst = D + (size_t)a * d.PD + obase;
 #pragma unroll
@@ -124,7 +129,9 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_yfwd(Dims d, const cd* __res
   extern __shared__ cd smem[];
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   const int gid = blockIdx.x * (GD_FFT_THREADS / T) + grp;
-  cd* buf = smem + (size_t)grp * (G::BUF + 1);
+  cd* buf = smem + FftTw<NY>::COUNT + (size_t)grp * (G::BUF + 1);
+  fft_load_table<NY>(smem, tw);
+  const cd* tws = smem;
   const bool active = gid < ncols;
   const int cx = active ? gid % d.Kx : 0;
   const int ez = active ? gid / d.Kx : 0;
@@ -136,7 +143,7 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_yfwd(Dims d, const cd* __res
     const cd* src = Ein + (size_t)a * d.PD + ibase;
 #pragma unroll
     for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * d.Kx) : cmake(0.0, 0.0);
-    fft_lanes<NY, -1>(v, t, buf, tw);
+    fft_lanes<NY, -1>(v, t, buf, tws);
   };
   if (e == 0) {
     cd va[E];
@@ -175,7 +182,7 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_yfwd(Dims d, const cd* __res
 }
 
 // ---- launchers ------------------------------------------------------------------------------------
-template <int N> static size_t fft_smem() { return (size_t)(GD_FFT_THREADS / FftGeom<N>::T) * (FftGeom<N>::BUF + 1) * sizeof(cd); }
+template <int N> static size_t fft_smem() { return ((size_t)(GD_FFT_THREADS / FftGeom<N>::T) * (FftGeom<N>::BUF + 1) + FftTw<N>::COUNT) * sizeof(cd); }
 template <int N> static int fft_blocks(long long ncols) { const int gpb = GD_FFT_THREADS / FftGeom<N>::T; return (int)((ncols + gpb - 1) / gpb); }
 
 #define GD_DISPATCH(NVAL, MACRO)                                                      \
@@ -205,4 +212,16 @@ cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, cudaSt
 #define YFCASE(NN) k_yfwd<NN><<<fft_blocks<NN>(ncols), GD_FFT_THREADS, fft_smem<NN>(), st>>>(d, E, Gh, tw, (int)ncols);
   GD_DISPATCH(d.ny, YFCASE)
   return cudaGetLastError();
+}
+
+// Host: the stage twiddle table of length-n transforms (fft.cuh layout); empty for single-stage sizes.
+int fft_stage_table_host(int n, std::vector<cd>& out) {
+#define TCASE(NN) out.assign(FftTw<NN>::COUNT + 1, cmake(0.0, 0.0)); fft_fill_stage_table<NN>(out.data());
+  switch (n) {
+    case 2: TCASE(2) break; case 4: TCASE(4) break; case 8: TCASE(8) break; case 16: TCASE(16) break;
+    case 32: TCASE(32) break; case 64: TCASE(64) break; case 128: TCASE(128) break; case 256: TCASE(256) break;
+    case 512: TCASE(512) break;
+    default: return -1;
+  }
+  return 0;
 }

@@ -9,9 +9,8 @@
 template <int N, int DIR> static void run(const double* in, double* out) {
   using G = FftGeom<N>;
   constexpr int T = G::T, E = G::E;
-  std::vector<cd> tw(N);
-  const double PI = 3.14159265358979323846;
-  for (int p = 0; p < N; ++p) tw[p] = cmake(std::cos(2 * PI * p / N), -std::sin(2 * PI * p / N));
+  std::vector<cd> tw(FftTw<N>::COUNT + 1);
+  fft_fill_stage_table<N>(tw.data());
   std::vector<cd> buf(G::BUF + 1);
   cd v[T][E];
   for (int t = 0; t < T; ++t)
