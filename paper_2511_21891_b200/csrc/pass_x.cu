@@ -22,11 +22,41 @@ struct XGeom {
   static constexpr int LB = NX + NX / G::PADDIV + 1;        // line buffer (FFT exchange + unpack), complex entries
   static constexpr int KXP = NX / 3 + 1;                    // retained kx count (== Dims::Kx)
   static constexpr int STG = 2 * KXP;                       // staging buffer: the two half-lines (f, df/dy) of the NEXT field
-  static constexpr int PER_GROUP = LB + 2 * NX + STG;       // + (Phi_x,Phi_y) and (Psi_x,Psi_y) lines + staging
-  static constexpr int THREADS = 224;                       // 7 warps, one CTA per SM: shared memory is the limiter
+  static constexpr int PER_GROUP = LB + STG;
+  static constexpr int THREADS = 256;                       // 8 warps, one CTA per SM (it owns all 512 TMEM columns)
   static constexpr int GROUPS = THREADS / T;
   static constexpr size_t SMEM = ((size_t)GROUPS * PER_GROUP + FftTw<NX>::COUNT) * sizeof(cd);
+  // Tensor memory as a thread-private scratchpad (tcgen05.ld/st, shape 32x32b: lane i of a warp owns TMEM lane
+  // 32*(warp%4)+i).  Per thread: 8 words per x-point for (Phi_x,Phi_y,Psi_x,Psi_y) and 2 words per x-point for the
+  // parked R_{m-2}.  Warps sharing a lane quarter take consecutive column slots.
+  static constexpr int TM_PHI = 0, TM_RD = 8 * E, TM_SLOT = 10 * E;
+  static_assert(TM_SLOT * (THREADS / 128) <= 512, "TMEM columns");
 };
+
+// ---- tensor-memory helpers (b32 columns <-> doubles) ------------------------------------------------------
+__device__ __forceinline__ void tm_st2(unsigned a, double x) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(a), "r"(__double2loint(x)), "r"(__double2hiint(x)) : "memory");
+}
+__device__ __forceinline__ void tm_st4(unsigned a, double x, double y) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(__double2loint(x)), "r"(__double2hiint(x)),
+               "r"(__double2loint(y)), "r"(__double2hiint(y)) : "memory");
+}
+struct TmRaw2 { unsigned w[2]; };
+struct TmRaw4 { unsigned w[4]; };
+struct TmRaw8 { unsigned w[8]; };
+__device__ __forceinline__ void tm_ld2(unsigned a, TmRaw2& r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r.w[0]), "=r"(r.w[1]) : "r"(a) : "memory");
+}
+__device__ __forceinline__ void tm_ld4(unsigned a, TmRaw4& r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(r.w[0]), "=r"(r.w[1]), "=r"(r.w[2]), "=r"(r.w[3]) : "r"(a) : "memory");
+}
+__device__ __forceinline__ void tm_ld8(unsigned a, TmRaw8& r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(r.w[0]), "=r"(r.w[1]), "=r"(r.w[2]), "=r"(r.w[3]), "=r"(r.w[4]), "=r"(r.w[5]), "=r"(r.w[6]), "=r"(r.w[7]) : "r"(a) : "memory");
+}
+__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ double tm_d(const unsigned* w) { return __hiloint2double((int)w[1], (int)w[0]); }
 
 template <int NX>
 __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const cd* __restrict__ D, cd* __restrict__ Eo,
@@ -40,16 +70,24 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   const int line = blockIdx.x * X::GROUPS + grp;
   cd* buf = smem + FftTw<NX>::COUNT + (size_t)grp * X::PER_GROUP;
-  fft_load_table<NX>(smem, tw);
+  __shared__ unsigned s_tmem_base;
+  const int warp = threadIdx.x >> 5;
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&s_tmem_base)), "r"(512) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  fft_load_table<NX>(smem, tw);      // ends with __syncthreads()
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const cd* tws = smem;
-  cd* sPhi = buf + X::LB;          // first xi+ then Phi derivatives, layout [q][t]
-  cd* sPsi = sPhi + NX;            // first xi- then Psi derivatives
+  // this warp's TMEM window: lane quarter warp%4, column slot warp/4
+  const unsigned tm = s_tmem_base + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * X::TM_SLOT);
   const bool active = line < nlines;
   const size_t base = (size_t)(active ? line : 0) * d.Kx;     // (z*ny + y)*Kx
   const int hx3 = d.hx3;
   cd v[E];
 
-  cd* sStage = sPsi + NX;          // [0,Kx): f~(kx), [Kx,2Kx): (df/dy)~(kx) of the field being fetched
+  cd* sStage = buf + X::LB;        // [0,Kx): f~(kx), [Kx,2Kx): (df/dy)~(kx) of the field being fetched
   // asynchronous fetch (cp.async, 16 B per lane) of the two half-lines of array a, a+1 into the staging buffer
   auto fetch = [&](int a) {
     if (active) {
@@ -119,33 +157,49 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   load_pack(2);                                   // xi+   (and start fetching xi-)
   fft_lanes<NX, +1>(v, t, buf, tws);
 #pragma unroll
-  for (int q = 0; q < E; ++q) sPhi[q * T + t] = v[q];
+  for (int q = 0; q < E; ++q) tm_st4(tm + X::TM_PHI + 8 * q, v[q].x, v[q].y);
   load_pack(6);                                   // xi-   (fetch w-)
   fft_lanes<NX, +1>(v, t, buf, tws);
 #pragma unroll
-  for (int q = 0; q < E; ++q) sPsi[q * T + t] = v[q];
+  for (int q = 0; q < E; ++q) tm_st4(tm + X::TM_PHI + 8 * q + 4, v[q].x, v[q].y);
   double A[E];
   load_pack(4);                                   // w-    (fetch w+)
   fft_lanes<NX, +1>(v, t, buf, tws);
+  tm_wait_st();
 #pragma unroll
-  for (int q = 0; q < E; ++q) {
-    const cd xp = sPhi[q * T + t];
-    A[q] = xp.x * v[q].y - xp.y * v[q].x;         // {xi+, w-}
+  for (int q0 = 0; q0 < E; q0 += 4) {
+    TmRaw4 r[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) tm_ld4(tm + X::TM_PHI + 8 * (q0 + j), r[j]);
+    tm_wait_ld();
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const double xpx = tm_d(r[j].w), xpy = tm_d(r[j].w + 2);
+      A[q0 + j] = xpx * v[q0 + j].y - xpy * v[q0 + j].x;          // {xi+, w-}
+    }
   }
   load_pack(d.M > 0 ? 8 : -1);                    // w+    (fetch g_0)
   fft_lanes<NX, +1>(v, t, buf, tws);
   double gmax = 0.0;
 #pragma unroll
-  for (int q = 0; q < E; ++q) {
-    const cd xp = sPhi[q * T + t], xm = sPsi[q * T + t];
-    const double a = A[q] + (xm.x * v[q].y - xm.y * v[q].x);      // + {xi-, w+}
-    const double b = xp.x * xm.y - xp.y * xm.x;                   // {xi+, xi-}
-    v[q] = cmake(a, b);
-    const cd phi = cmake(0.5 * (xp.x + xm.x), 0.5 * (xp.y + xm.y));   // grad Phi, Phi = (xi+ + xi-)/2
-    const cd psi = cmake(0.5 * (xp.x - xm.x), 0.5 * (xp.y - xm.y));   // grad Psi
-    sPhi[q * T + t] = phi;
-    sPsi[q * T + t] = psi;
-    gmax = fmax(gmax, phi.x * phi.x + phi.y * phi.y);
+  for (int q0 = 0; q0 < E; q0 += 4) {
+    TmRaw8 r[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) tm_ld8(tm + X::TM_PHI + 8 * (q0 + j), r[j]);
+    tm_wait_ld();
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int q = q0 + j;
+      const cd xp = cmake(tm_d(r[j].w), tm_d(r[j].w + 2)), xm = cmake(tm_d(r[j].w + 4), tm_d(r[j].w + 6));
+      const double a = A[q] + (xm.x * v[q].y - xm.y * v[q].x);      // + {xi-, w+}
+      const double b = xp.x * xm.y - xp.y * xm.x;                   // {xi+, xi-}
+      v[q] = cmake(a, b);
+      const cd phi = cmake(0.5 * (xp.x + xm.x), 0.5 * (xp.y + xm.y));   // grad Phi, Phi = (xi+ + xi-)/2
+      const cd psi = cmake(0.5 * (xp.x - xm.x), 0.5 * (xp.y - xm.y));   // grad Psi
+      tm_st4(tm + X::TM_PHI + 8 * q, phi.x, phi.y);
+      tm_st4(tm + X::TM_PHI + 8 * q + 4, psi.x, psi.y);
+      gmax = fmax(gmax, phi.x * phi.x + phi.y * phi.y);
+    }
   }
   if (maxbits != nullptr) {
     if (!active) gmax = 0.0;
@@ -158,33 +212,55 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   // ---- Hermite part: R_m with a sliding window over m ------------------------------------------
   const int M = d.M;
   if (M > 0) {
-    double Qp[E], Ra[E], Rd[E];
+    double Qp[E], Ra[E];
 #pragma unroll
-    for (int q = 0; q < E; ++q) { Qp[q] = 0.0; Ra[q] = 0.0; Rd[q] = 0.0; }
+    for (int q = 0; q < E; ++q) { Qp[q] = 0.0; Ra[q] = 0.0; }
     for (int m = 0; m < M; ++m) {
       load_pack(m + 1 < M ? 8 + 2 * (m + 1) : -1);  // g_m  (fetch g_{m+1})
       fft_lanes<NX, +1>(v, t, buf, tws);
       const double dn = cdn[m];
       const double upp = (m > 0) ? cup[m - 1] : 0.0;
       const bool emit = (m >= 1) && (((m - 1) & 1) == 1);     // R_{m-1} completes the pair (R_{m-2}, R_{m-1})
+      tm_wait_st();                                           // earlier tensor-memory stores are visible
 #pragma unroll
-      for (int q = 0; q < E; ++q) {
-        const cd ph = sPhi[q * T + t], ps = sPsi[q * T + t];
-        const double gx = v[q].x, gy = v[q].y;
-        const double P = ph.x * gy - ph.y * gx;               // {Phi, g_m}
-        const double Q = ps.x * gy - ps.y * gx;               // {Psi, g_m}
-        const double rfin = Ra[q] + upp * Q;                  // R_{m-1} complete
-        Ra[q] = dn * Qp[q] - P;
-        Qp[q] = Q;
-        if (emit) v[q] = cmake(Rd[q], rfin);
-        else Rd[q] = rfin;
+      for (int q0 = 0; q0 < E; q0 += 4) {
+        TmRaw8 r[4];
+        TmRaw2 rd[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) tm_ld8(tm + X::TM_PHI + 8 * (q0 + j), r[j]);
+        if (emit) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) tm_ld2(tm + X::TM_RD + 2 * (q0 + j), rd[j]);
+        }
+        tm_wait_ld();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int q = q0 + j;
+          const double phx = tm_d(r[j].w), phy = tm_d(r[j].w + 2), psx = tm_d(r[j].w + 4), psy = tm_d(r[j].w + 6);
+          const double gx = v[q].x, gy = v[q].y;
+          const double P = phx * gy - phy * gx;               // {Phi, g_m}
+          const double Q = psx * gy - psy * gx;               // {Psi, g_m}
+          const double rfin = Ra[q] + upp * Q;                // R_{m-1} complete
+          Ra[q] = dn * Qp[q] - P;
+          Qp[q] = Q;
+          if (emit) v[q] = cmake(tm_d(rd[j].w), rfin);
+          else tm_st2(tm + X::TM_RD + 2 * q, rfin);
+        }
       }
       if (emit) fwd_store(2 + m - 2, 2 + m - 1);
     }
     // R_{M-1} is complete (up_{M-1} = 0 after the closure was folded into dn)
     if (((M - 1) & 1) == 1) {
+      tm_wait_st();
 #pragma unroll
-      for (int q = 0; q < E; ++q) v[q] = cmake(Rd[q], Ra[q]);
+      for (int q0 = 0; q0 < E; q0 += 4) {
+        TmRaw2 rd[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) tm_ld2(tm + X::TM_RD + 2 * (q0 + j), rd[j]);
+        tm_wait_ld();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) v[q0 + j] = cmake(tm_d(rd[j].w), Ra[q0 + j]);
+      }
       fwd_store(2 + M - 2, 2 + M - 1);
     } else {
 #pragma unroll
@@ -192,6 +268,9 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
       fwd_store(2 + M - 1, -1);
     }
   }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem_base), "r"(512) : "memory");
 }
 
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
