@@ -60,16 +60,18 @@ __device__ __forceinline__ double tm_d(const unsigned* w) { return __hiloint2dou
 
 template <int NX>
 __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const cd* __restrict__ D, cd* __restrict__ Eo,
-                                                        const cd* __restrict__ tw, const double* __restrict__ cdn,
-                                                        const double* __restrict__ cup,
-                                                        unsigned long long* __restrict__ maxbits, int nlines) {
+                                                           const cd* __restrict__ tw, const double* __restrict__ cdn,
+                                                           const double* __restrict__ cup,
+                                                           unsigned long long* __restrict__ maxbits, int nlines) {
   using X = XGeom<NX>;
   using G = FftGeom<NX>;
   constexpr int T = X::T, E = X::E;
+  constexpr int HX3 = NX / 3, KX = X::KXP;        // == d.hx3, d.Kx (compile-time so per-q range tests fold)
   extern __shared__ cd smem[];
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   const int line = blockIdx.x * X::GROUPS + grp;
   cd* buf = smem + FftTw<NX>::COUNT + (size_t)grp * X::PER_GROUP;
+  cd* sStage = buf + X::LB;        // [0,KX): f~(kx), [KX,2KX): (df/dy)~(kx) of the field being fetched
   __shared__ unsigned s_tmem_base;
   const int warp = threadIdx.x >> 5;
   if (warp == 0) {
@@ -83,190 +85,192 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   // this warp's TMEM window: lane quarter warp%4, column slot warp/4
   const unsigned tm = s_tmem_base + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * X::TM_SLOT);
   const bool active = line < nlines;
-  const size_t base = (size_t)(active ? line : 0) * d.Kx;     // (z*ny + y)*Kx
-  const int hx3 = d.hx3;
+  const size_t base = (size_t)(active ? line : 0) * KX;       // (z*ny + y)*Kx
+  const int M = d.M;
   cd v[E];
+  double Qp[E], Ra[E];             // Hermite sliding window; Qp doubles as the {xi+,w-} accumulator of the Elsasser part
 
-  cd* sStage = buf + X::LB;        // [0,Kx): f~(kx), [Kx,2Kx): (df/dy)~(kx) of the field being fetched
   // asynchronous fetch (cp.async, 16 B per lane) of the two half-lines of array a, a+1 into the staging buffer
   auto fetch = [&](int a) {
     if (active) {
       const cd* pf = D + (size_t)a * d.PD + base;
       const unsigned sbase = (unsigned)__cvta_generic_to_shared(sStage);
-      for (int c = t; c < 2 * d.Kx; c += T) {
-        const cd* src = (c < d.Kx) ? pf + c : pf + d.PD + (c - d.Kx);
+      for (int c = t; c < 2 * KX; c += T) {
+        const cd* src = (c < KX) ? pf + c : pf + d.PD + (c - KX);
         asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sbase + 16u * (unsigned)c), "l"(src) : "memory");
       }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
   };
-  // wait for the staged half-lines, pack Z = Fx + i Fy on the full kx line into v, then start fetching array `next`
-  auto load_pack = [&](int next) {
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-    __syncwarp();
-    const cd* pf = sStage;
-    const cd* pfy = sStage + d.Kx;
-#pragma unroll
-    for (int q = 0; q < E; ++q) {
-      const int n = t + T * q;
-      cd z = cmake(0.0, 0.0);
-      if (active) {
-        if (n <= hx3) {
-          cd f = pf[n], fy = pfy[n];
-          if (n == 0) { f.y = 0.0; fy.y = 0.0; }
-          const double kx = d.kx0 * n;
-          // Fx = i kx f = (-kx f.y, kx f.x);  Z = Fx + i Fy
-          z = cmake(-kx * f.y - fy.y, kx * f.x + fy.x);
-        } else if (n >= NX - hx3) {
-          const int c = NX - n;
-          const cd f = pf[c], fy = pfy[c];
-          const double kx = d.kx0 * c;
-          // conj(Fx) + i conj(Fy) = (-kx f.y + fy.y, -kx f.x + fy.x)
-          z = cmake(-kx * f.y + fy.y, -kx * f.x + fy.x);
-        }
-      }
-      v[q] = z;
-    }
-    __syncwarp();                   // every lane has consumed the staging buffer
-    if (next >= 0) fetch(next);
-  };
-  // forward-transform v = (U + i V) of two real lines and store U~, V~ (kx <= nx/3) to arrays e0, e1 (e1 < 0: skip)
-  auto fwd_store = [&](int e0, int e1) {
-    fft_lanes<NX, -1>(v, t, buf, tws);
-#pragma unroll
-    for (int q = 0; q < E; ++q) buf[G::pad(t + T * q)] = v[q];
-    __syncwarp();
-    if (active) {
-      cd* p0 = Eo + (size_t)e0 * d.PD + base;
-      cd* p1 = Eo + (size_t)(e1 < 0 ? e0 : e1) * d.PD + base;
-#pragma unroll
-      for (int q = 0; q < E; ++q) {
-        const int c = t + T * q;
-        if (c <= hx3) {
-          const cd z1 = buf[G::pad(c)], z2 = buf[G::pad((NX - c) & (NX - 1))];
-          st_cd(p0 + c, cmake(0.5 * (z1.x + z2.x), 0.5 * (z1.y - z2.y)));
-          if (e1 >= 0) st_cd(p1 + c, cmake(0.5 * (z1.y + z2.y), -0.5 * (z1.x - z2.x)));
-        }
-      }
-    }
-    __syncwarp();
-  };
-
-  // ---- Elsasser part: A, B --------------------------------------------------------------------
-  fetch(0);
-  load_pack(2);                                   // xi+   (and start fetching xi-)
-  fft_lanes<NX, +1>(v, t, buf, tws);
-#pragma unroll
-  for (int q = 0; q < E; ++q) tm_st4(tm + X::TM_PHI + 8 * q, v[q].x, v[q].y);
-  load_pack(6);                                   // xi-   (fetch w-)
-  fft_lanes<NX, +1>(v, t, buf, tws);
-#pragma unroll
-  for (int q = 0; q < E; ++q) tm_st4(tm + X::TM_PHI + 8 * q + 4, v[q].x, v[q].y);
-  double A[E];
-  load_pack(4);                                   // w-    (fetch w+)
-  fft_lanes<NX, +1>(v, t, buf, tws);
-  tm_wait_st();
-#pragma unroll
-  for (int q0 = 0; q0 < E; q0 += 4) {
-    TmRaw4 r[4];
-#pragma unroll
-    for (int j = 0; j < 4; ++j) tm_ld4(tm + X::TM_PHI + 8 * (q0 + j), r[j]);
-    tm_wait_ld();
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const double xpx = tm_d(r[j].w), xpy = tm_d(r[j].w + 2);
-      A[q0 + j] = xpx * v[q0 + j].y - xpy * v[q0 + j].x;          // {xi+, w-}
-    }
-  }
-  load_pack(d.M > 0 ? 8 : -1);                    // w+    (fetch g_0)
-  fft_lanes<NX, +1>(v, t, buf, tws);
+  // Job list of one line.  Kinds 0..3 are the inverse transforms of xi+, xi-, w-, w+; kind 4+m that of g_m.
+  // After kind 3 and after every second moment a forward job (pair of real lines) follows.  Inverse transforms
+  // run as conj(FFT(conj Z)) so that ONE forward-FFT code instance serves every job (instruction cache).
+  auto src_array = [&](int kind) { return kind == 0 ? 0 : kind == 1 ? 2 : kind == 2 ? 6 : kind == 3 ? 4 : 8 + 2 * (kind - 4); };
+  const int nkinds = 4 + M;
+  int kind = 0;
+  bool fwd = false;                // the job about to run is a forward transform of the pair held in v
+  bool tail_done = (M == 0);
+  int e0 = 0, e1 = 1;
   double gmax = 0.0;
+  fetch(src_array(0));
+  for (;;) {
+    if (!fwd) {
+      if (kind == nkinds) {
+        if (tail_done) break;
+        // R_{M-1} is complete (up_{M-1} = 0 after the closure was folded into dn): flush the last pair / single
+        tail_done = true;
+        fwd = true;
+        if (((M - 1) & 1) == 1) {
+          tm_wait_st();
 #pragma unroll
-  for (int q0 = 0; q0 < E; q0 += 4) {
-    TmRaw8 r[4];
+          for (int q0 = 0; q0 < E; q0 += 4) {
+            TmRaw2 rd[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) tm_ld8(tm + X::TM_PHI + 8 * (q0 + j), r[j]);
-    tm_wait_ld();
+            for (int jj = 0; jj < 4; ++jj) tm_ld2(tm + X::TM_RD + 2 * (q0 + jj), rd[jj]);
+            tm_wait_ld();
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const int q = q0 + j;
-      const cd xp = cmake(tm_d(r[j].w), tm_d(r[j].w + 2)), xm = cmake(tm_d(r[j].w + 4), tm_d(r[j].w + 6));
-      const double a = A[q] + (xm.x * v[q].y - xm.y * v[q].x);      // + {xi-, w+}
-      const double b = xp.x * xm.y - xp.y * xm.x;                   // {xi+, xi-}
-      v[q] = cmake(a, b);
-      const cd phi = cmake(0.5 * (xp.x + xm.x), 0.5 * (xp.y + xm.y));   // grad Phi, Phi = (xi+ + xi-)/2
-      const cd psi = cmake(0.5 * (xp.x - xm.x), 0.5 * (xp.y - xm.y));   // grad Psi
-      tm_st4(tm + X::TM_PHI + 8 * q, phi.x, phi.y);
-      tm_st4(tm + X::TM_PHI + 8 * q + 4, psi.x, psi.y);
-      gmax = fmax(gmax, phi.x * phi.x + phi.y * phi.y);
+            for (int jj = 0; jj < 4; ++jj) v[q0 + jj] = cmake(tm_d(rd[jj].w), Ra[q0 + jj]);
+          }
+          e0 = 2 + M - 2; e1 = 2 + M - 1;
+        } else {
+#pragma unroll
+          for (int q = 0; q < E; ++q) v[q] = cmake(Ra[q], 0.0);
+          e0 = 2 + M - 1; e1 = -1;
+        }
+      } else {
+        // wait for the staged half-lines and pack conj(Z), Z = Fx + i Fy, Fx = i kx f  (Hermitian completion for kx < 0)
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncwarp();
+        const cd* pf = sStage;
+        const cd* pfy = sStage + KX;
+#pragma unroll
+        for (int q = 0; q < E; ++q) {
+          const int n = t + T * q;
+          cd z = cmake(0.0, 0.0);
+          if (T * q <= HX3 && n <= HX3) {                       // first test is compile-time per q
+            cd f = pf[n], fy = pfy[n];
+            if (n == 0) { f.y = 0.0; fy.y = 0.0; }
+            const double kx = d.kx0 * n;
+            z = cmake(-kx * f.y - fy.y, -(kx * f.x + fy.x));    // conj( i kx f + i fy )
+          } else if (T * q + T - 1 >= NX - HX3 && n >= NX - HX3) {
+            const int c = NX - n;
+            const cd f = pf[c], fy = pfy[c];
+            const double kx = d.kx0 * c;
+            z = cmake(-kx * f.y + fy.y, kx * f.x - fy.x);       // conj( conj(i kx f) + i conj(fy) )
+          }
+          v[q] = z;
+        }
+        __syncwarp();                   // every lane has consumed the staging buffer
+        if (kind + 1 < nkinds) fetch(src_array(kind + 1));
+      }
     }
+
+    fft_lanes<NX, -1>(v, t, buf, tws);
+
+    if (fwd) {
+      // separate the two real lines' spectra by Hermitian symmetry, keep kx <= nx/3, store
+      fwd = false;
+#pragma unroll
+      for (int q = 0; q < E; ++q) buf[G::pad(t + T * q)] = v[q];
+      __syncwarp();
+      if (active) {
+        cd* p0 = Eo + (size_t)e0 * d.PD + base;
+        cd* p1 = Eo + (size_t)(e1 < 0 ? e0 : e1) * d.PD + base;
+#pragma unroll
+        for (int q = 0; q < E; ++q) {
+          const int c = t + T * q;
+          if (T * q <= HX3 && c <= HX3) {
+            const cd z1 = buf[G::pad(c)], z2 = buf[G::pad((NX - c) & (NX - 1))];
+            st_cd(p0 + c, cmake(0.5 * (z1.x + z2.x), 0.5 * (z1.y - z2.y)));
+            if (e1 >= 0) st_cd(p1 + c, cmake(0.5 * (z1.y + z2.y), -0.5 * (z1.x - z2.x)));
+          }
+        }
+      }
+      __syncwarp();
+      continue;
+    }
+
+    // inverse job done: v[q] = (df/dx, -df/dy) at x = t + T q   (conjugated output)
+    if (kind == 0 || kind == 1) {          // xi+ / xi-: park the derivative lines in tensor memory
+#pragma unroll
+      for (int q = 0; q < E; ++q) tm_st4(tm + X::TM_PHI + 8 * q + 4 * kind, v[q].x, -v[q].y);
+    } else if (kind == 2) {                // w-: {xi+, w-}
+      tm_wait_st();
+#pragma unroll
+      for (int q0 = 0; q0 < E; q0 += 4) {
+        TmRaw4 r[4];
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) tm_ld4(tm + X::TM_PHI + 8 * (q0 + jj), r[jj]);
+        tm_wait_ld();
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+          const double xpx = tm_d(r[jj].w), xpy = tm_d(r[jj].w + 2);
+          Qp[q0 + jj] = xpx * (-v[q0 + jj].y) - xpy * v[q0 + jj].x;
+        }
+      }
+    } else if (kind == 3) {                // w+: A = {xi+,w-} + {xi-,w+}, B = {xi+,xi-}; Phi/Psi lines; CFL max
+#pragma unroll
+      for (int q0 = 0; q0 < E; q0 += 4) {
+        TmRaw8 r[4];
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) tm_ld8(tm + X::TM_PHI + 8 * (q0 + jj), r[jj]);
+        tm_wait_ld();
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+          const int q = q0 + jj;
+          const cd xp = cmake(tm_d(r[jj].w), tm_d(r[jj].w + 2)), xm = cmake(tm_d(r[jj].w + 4), tm_d(r[jj].w + 6));
+          const double a = Qp[q] + (xm.x * (-v[q].y) - xm.y * v[q].x);
+          const double b = xp.x * xm.y - xp.y * xm.x;
+          v[q] = cmake(a, b);
+          const cd phi = cmake(0.5 * (xp.x + xm.x), 0.5 * (xp.y + xm.y));   // grad Phi, Phi = (xi+ + xi-)/2
+          const cd psi = cmake(0.5 * (xp.x - xm.x), 0.5 * (xp.y - xm.y));   // grad Psi
+          tm_st4(tm + X::TM_PHI + 8 * q, phi.x, phi.y);
+          tm_st4(tm + X::TM_PHI + 8 * q + 4, psi.x, psi.y);
+          gmax = fmax(gmax, phi.x * phi.x + phi.y * phi.y);
+          Qp[q] = 0.0; Ra[q] = 0.0;
+        }
+      }
+      fwd = true; e0 = 0; e1 = 1;
+    } else {                               // g_m: P_m, Q_m and the sliding window R_m = -P_m + dn_m Q_{m-1} + up_m Q_{m+1}
+      const int m = kind - 4;
+      const double dn = cdn[m];
+      const double upp = (m > 0) ? cup[m - 1] : 0.0;
+      const bool emit = (m >= 1) && (((m - 1) & 1) == 1);     // R_{m-1} completes the pair (R_{m-2}, R_{m-1})
+      tm_wait_st();
+#pragma unroll
+      for (int q0 = 0; q0 < E; q0 += 4) {
+        TmRaw8 r[4];
+        TmRaw2 rd[4];
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) tm_ld8(tm + X::TM_PHI + 8 * (q0 + jj), r[jj]);
+        if (emit) {
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj) tm_ld2(tm + X::TM_RD + 2 * (q0 + jj), rd[jj]);
+        }
+        tm_wait_ld();
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+          const int q = q0 + jj;
+          const double phx = tm_d(r[jj].w), phy = tm_d(r[jj].w + 2), psx = tm_d(r[jj].w + 4), psy = tm_d(r[jj].w + 6);
+          const double gx = v[q].x, gy = -v[q].y;
+          const double P = phx * gy - phy * gx;               // {Phi, g_m}
+          const double Q = psx * gy - psy * gx;               // {Psi, g_m}
+          const double rfin = Ra[q] + upp * Q;                // R_{m-1} complete
+          Ra[q] = dn * Qp[q] - P;
+          Qp[q] = Q;
+          if (emit) v[q] = cmake(tm_d(rd[jj].w), rfin);
+          else tm_st2(tm + X::TM_RD + 2 * q, rfin);
+        }
+      }
+      if (emit) { fwd = true; e0 = 2 + m - 2; e1 = 2 + m - 1; }
+    }
+    ++kind;
   }
   if (maxbits != nullptr) {
     if (!active) gmax = 0.0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) gmax = fmax(gmax, __shfl_xor_sync(0xffffffffu, gmax, o));
     if ((threadIdx.x & 31) == 0) atomicMax(maxbits, (unsigned long long)__double_as_longlong(gmax));
-  }
-  fwd_store(0, 1);
-
-  // ---- Hermite part: R_m with a sliding window over m ------------------------------------------
-  const int M = d.M;
-  if (M > 0) {
-    double Qp[E], Ra[E];
-#pragma unroll
-    for (int q = 0; q < E; ++q) { Qp[q] = 0.0; Ra[q] = 0.0; }
-    for (int m = 0; m < M; ++m) {
-      load_pack(m + 1 < M ? 8 + 2 * (m + 1) : -1);  // g_m  (fetch g_{m+1})
-      fft_lanes<NX, +1>(v, t, buf, tws);
-      const double dn = cdn[m];
-      const double upp = (m > 0) ? cup[m - 1] : 0.0;
-      const bool emit = (m >= 1) && (((m - 1) & 1) == 1);     // R_{m-1} completes the pair (R_{m-2}, R_{m-1})
-      tm_wait_st();                                           // earlier tensor-memory stores are visible
-#pragma unroll
-      for (int q0 = 0; q0 < E; q0 += 4) {
-        TmRaw8 r[4];
-        TmRaw2 rd[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) tm_ld8(tm + X::TM_PHI + 8 * (q0 + j), r[j]);
-        if (emit) {
-#pragma unroll
-          for (int j = 0; j < 4; ++j) tm_ld2(tm + X::TM_RD + 2 * (q0 + j), rd[j]);
-        }
-        tm_wait_ld();
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int q = q0 + j;
-          const double phx = tm_d(r[j].w), phy = tm_d(r[j].w + 2), psx = tm_d(r[j].w + 4), psy = tm_d(r[j].w + 6);
-          const double gx = v[q].x, gy = v[q].y;
-          const double P = phx * gy - phy * gx;               // {Phi, g_m}
-          const double Q = psx * gy - psy * gx;               // {Psi, g_m}
-          const double rfin = Ra[q] + upp * Q;                // R_{m-1} complete
-          Ra[q] = dn * Qp[q] - P;
-          Qp[q] = Q;
-          if (emit) v[q] = cmake(tm_d(rd[j].w), rfin);
-          else tm_st2(tm + X::TM_RD + 2 * q, rfin);
-        }
-      }
-      if (emit) fwd_store(2 + m - 2, 2 + m - 1);
-    }
-    // R_{M-1} is complete (up_{M-1} = 0 after the closure was folded into dn)
-    if (((M - 1) & 1) == 1) {
-      tm_wait_st();
-#pragma unroll
-      for (int q0 = 0; q0 < E; q0 += 4) {
-        TmRaw2 rd[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) tm_ld2(tm + X::TM_RD + 2 * (q0 + j), rd[j]);
-        tm_wait_ld();
-#pragma unroll
-        for (int j = 0; j < 4; ++j) v[q0 + j] = cmake(tm_d(rd[j].w), Ra[q0 + j]);
-      }
-      fwd_store(2 + M - 2, 2 + M - 1);
-    } else {
-#pragma unroll
-      for (int q = 0; q < E; ++q) v[q] = cmake(Ra[q], 0.0);
-      fwd_store(2 + M - 1, -1);
-    }
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
