@@ -16,6 +16,7 @@
 cudaError_t launch_zfft(const Dims& d, int dir, const cd* in, cd* out, const cd* tw, int nfields, cudaStream_t st);
 cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStream_t st);
 cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, cudaStream_t st);
+cudaError_t prepare_passes_zy(int ny, int nz);
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
                          unsigned long long* maxbits, cudaStream_t st, bool prepare_only);
 cudaError_t launch_update(const Dims& d, const PhysParams& p, int mode, const cd* G, const cd* Wn, const cd* Ws, cd* Wout,
@@ -178,6 +179,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (e == cudaSuccess) e = upload_twiddles(&c->twy, d.ny, c->st);
   if (e == cudaSuccess) e = upload_twiddles(&c->twz, d.nz, c->st);
   if (e == cudaSuccess) e = launch_xpass(d, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, c->st, true);
+  if (e == cudaSuccess) e = prepare_passes_zy(d.ny, d.nz);
 
   // Hermite coupling coefficients with the closure folded in (Q10, Q23, Q24)
   std::vector<double> dn(M + 1, 0.0), up(M + 1, 0.0), cr(M + 1, 0.0);

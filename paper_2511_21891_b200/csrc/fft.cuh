@@ -207,6 +207,31 @@ template <int N> GD_HD void fft_gather(cd (&v)[FftPlan<N>::E], int t, const cd* 
   for (int q = 0; q < G::E; ++q) v[q] = buf[G::pad(t + G::T * q)];
 }
 
+// Split exchange: the real parts cross the lanes first, then the imaginary parts, through a buffer of doubles
+// (FftGeom<N>::BUF entries of 8 bytes -- half the shared memory of the complex exchange; in place, because a lane's
+// .x registers can be overwritten by the gather while its .y registers still wait to be scattered).
+template <int N, int s, int C> GD_HD void fft_stage_scatter_c(const cd (&v)[FftPlan<N>::E], int t, double* buf) {
+  using G = FftGeom<N>;
+  constexpr int R = G::template radix<s>();
+  constexpr int NS = G::template ns<s>();
+  constexpr int B = G::E / R;
+#pragma unroll
+  for (int b = 0; b < B; ++b) {
+    const int j = t + G::T * b;
+    const int j0 = (j / NS) * NS * R + (j % NS);
+#pragma unroll
+    for (int i = 0; i < R; ++i) buf[G::pad(j0 + i * NS)] = C ? v[b + i * B].y : v[b + i * B].x;
+  }
+}
+template <int N, int C> GD_HD void fft_gather_c(cd (&v)[FftPlan<N>::E], int t, const double* buf) {
+  using G = FftGeom<N>;
+#pragma unroll
+  for (int q = 0; q < G::E; ++q) {
+    if (C) v[q].y = buf[G::pad(t + G::T * q)];
+    else v[q].x = buf[G::pad(t + G::T * q)];
+  }
+}
+
 #if defined(__CUDACC__)
 // The cooperative transform.  buf: this line's shared buffer (FftGeom<N>::BUF entries; unused if S==1);
 // tws: the stage table (FftTw<N>::COUNT entries), normally in shared memory.
@@ -231,6 +256,30 @@ template <int N, int DIR> __device__ __forceinline__ void fft_lanes(cd (&v)[FftP
     __syncwarp();
     fft_gather<N>(v, t, buf);
     __syncwarp();
+    fft_stage_compute<N, DIR, 2>(v, t, tws);
+  }
+}
+template <int N, int s> __device__ __forceinline__ void fft_exchange_split(cd (&v)[FftPlan<N>::E], int t, double* buf) {
+  fft_stage_scatter_c<N, s, 0>(v, t, buf);
+  __syncwarp();
+  fft_gather_c<N, 0>(v, t, buf);
+  __syncwarp();
+  fft_stage_scatter_c<N, s, 1>(v, t, buf);
+  __syncwarp();
+  fft_gather_c<N, 1>(v, t, buf);
+  __syncwarp();
+}
+// Same transform with the split exchange; buf: FftGeom<N>::BUF doubles per lane group.
+template <int N, int DIR> __device__ __forceinline__ void fft_lanes_split(cd (&v)[FftPlan<N>::E], int t, double* buf,
+                                                                           const cd* __restrict__ tws) {
+  using G = FftGeom<N>;
+  fft_stage_compute<N, DIR, 0>(v, t, tws);
+  if constexpr (G::S > 1) {
+    fft_exchange_split<N, 0>(v, t, buf);
+    fft_stage_compute<N, DIR, 1>(v, t, tws);
+  }
+  if constexpr (G::S > 2) {
+    fft_exchange_split<N, 1>(v, t, buf);
     fft_stage_compute<N, DIR, 2>(v, t, tws);
   }
 }

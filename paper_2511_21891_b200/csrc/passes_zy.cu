@@ -3,7 +3,8 @@
 //   k_zinv : S[f][cz][cy][cx] -> H[f][z][cy][cx]      inverse c2c along z, zero-padded
 //   k_zfwd : H -> S                                   forward c2c along z, kz part of Eq. 20, 1/N scale
 //   k_yinv : P1.  H -> D: for w+- also xi = -w/kperp^2; for every source field f the
-//            pair ( f , d f/dy = IFFT_y(i ky f) )  (Eq. 10), inverse c2c along y
+//            pair ( f , d f/dy = IFFT_y(i ky f) )  (Eq. 10), inverse c2c along y;
+//            the two arrays of a pair are transformed by sibling warps (no second copy of the input in registers)
 //   k_yfwd : P3.  E -> H: forward c2c along y, ky part of Eq. 20; the Elsasser pair is assembled as
 //            N+- = -1/2 A -+ 1/2 kperp^2 B  (Eq. 1 with Eq. 11)
 // Every FFT is fft_lanes<N> (fft.cuh): T lanes of one warp per column, data in registers, one
@@ -13,13 +14,13 @@
 #include "common.cuh"
 
 template <int NZ, int DIR>
-__global__ void __launch_bounds__(GD_FFT_THREADS) k_zfft(Dims d, const cd* __restrict__ in, cd* __restrict__ out,
+__global__ void __launch_bounds__(GD_Z_THREADS) k_zfft(Dims d, const cd* __restrict__ in, cd* __restrict__ out,
                                                        const cd* __restrict__ tw, int ncols) {
   using G = FftGeom<NZ>;
   constexpr int T = G::T, E = G::E;
   extern __shared__ cd smem[];
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
-  const int gid = blockIdx.x * (GD_FFT_THREADS / T) + grp;
+  const int gid = blockIdx.x * (GD_Z_THREADS / T) + grp;
   cd* buf = smem + FftTw<NZ>::COUNT + (size_t)grp * (G::BUF + 1);
   fft_load_table<NZ>(smem, tw);
   const cd* tws = smem;
@@ -56,122 +57,220 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_zfft(Dims d, const cd* __res
   }
 }
 
-// P1.  One lane group per (source field s, z, cx) column.  Sources: s = 0,1 -> w+, w-;  s = 2+m -> g_m.
-// D array order: 0/1 xi+ , 2/3 xi- , 4/5 w+ , 6/7 w- , 8+2m / 9+2m g_m   (even: f, odd: df/dy).
-template <int NY>
-__global__ void __launch_bounds__(GD_FFT_THREADS) k_yinv(Dims d, const cd* __restrict__ H, cd* __restrict__ D,
-                                                       const cd* __restrict__ tw, int ncols) {
+// Geometry of the y passes: GD_Y_THREADS lanes per CTA = GROUPS lane groups = GROUPS adjacent columns of ONE array,
+// so a CTA covers GROUPS*16 B contiguous per row (256 B at ny = 256: strided row segments narrower than that lose
+// HBM efficiency, profiles/r01_stride_microbench.md) and two CTAs fit on an SM (<= 128 registers per lane).
+#define GD_Y_THREADS 256
+template <int NY> struct YGeom {
   using G = FftGeom<NY>;
-  constexpr int T = G::T, E = G::E;
-  extern __shared__ cd smem[];
-  const int grp = threadIdx.x / T, t = threadIdx.x % T;
-  const int gid = blockIdx.x * (GD_FFT_THREADS / T) + grp;
-  cd* buf = smem + FftTw<NY>::COUNT + (size_t)grp * (G::BUF + 1);
-  fft_load_table<NY>(smem, tw);
-  const cd* tws = smem;
-  const bool active = gid < ncols;
-  const int cx = active ? gid % d.Kx : 0;
-  const int sz = active ? gid / d.Kx : 0;
-  const int z = sz % d.nz, s = sz / d.nz;
-  const cd* src = H + (size_t)s * d.PH + (size_t)z * d.Ky * d.Kx + cx;
-  const double kx = d.kx0 * cx;
-  cd v0[E], v[E];
-  double ky[E];
-#pragma unroll
-  for (int q = 0; q < E; ++q) {
-    const int iy = t + T * q;
-    const int cy = fft2c(iy, NY, d.hy3, d.Ky);
-    v0[q] = (active && cy >= 0) ? ldg_cd(src + (size_t)cy * d.Kx) : cmake(0.0, 0.0);
-    ky[q] = d.ky0 * fft2n(iy, NY);
-  }
-  const size_t obase = (size_t)z * NY * d.Kx + cx;
-  auto emit = [&](int a) {   // inverse transform v and write array a
-    fft_lanes<NY, +1>(v, t, buf, tws);
-    if (active) {
-      cd* dst = D + (size_t)a * d.PD + obase;
-#pragma unroll
-      for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * d.Kx, v[q]);
-    }
-  };
-  if (s < 2) {
-    // potentials: xi = -w / kperp^2, zero at kperp = 0
-#pragma unroll
-    for (int q = 0; q < E; ++q) {
-      const double k2 = kx * kx + ky[q] * ky[q];
-      const double inv = k2 > 0.0 ? -1.0 / k2 : 0.0;
-      v[q] = cscale(v0[q], inv);
-    }
-    emit(2 * s);
-#pragma unroll
-    for (int q = 0; q < E; ++q) {
-      const double k2 = kx * kx + ky[q] * ky[q];
-      const double inv = k2 > 0.0 ? -1.0 / k2 : 0.0;
-      v[q] = cscale(mul_i(v0[q]), inv * ky[q]);
-    }
-    emit(2 * s + 1);
-  }
-  const int a0 = (s < 2) ? 4 + 2 * s : 8 + 2 * (s - 2);
-#pragma unroll
-  for (int q = 0; q < E; ++q) v[q] = v0[q];
-  emit(a0);
-#pragma unroll
-  for (int q = 0; q < E; ++q) v[q] = cscale(mul_i(v0[q]), ky[q]);
-  emit(a0 + 1);
-}
+  static constexpr int T = G::T, E = G::E;
+  static constexpr int GROUPS = GD_Y_THREADS / T;            // columns per CTA
+  static constexpr int YBUF = (G::S > 1 ? G::BUF : NY) + 1;  // per-group buffer (FFT exchange; A/B hand-over in P3)
+  static constexpr int REGION = (GROUPS * YBUF > NY * (GROUPS + 1)) ? GROUPS * YBUF : NY * (GROUPS + 1);   // also holds a padded [NY][GROUPS] tile
+  static constexpr size_t SMEM = ((size_t)REGION + FftTw<NY>::COUNT) * sizeof(cd);
+};
 
-// P3.  One lane group per (task e, z, cx): e = 0 handles A and B together, e = 1+m handles R_m.
-// E array order: 0 A, 1 B, 2+m R_m.  Output hybrid fields: 0 N+, 1 N-, 2+m R_m.
+// P1.  Persistent CTAs over the work items (source field s, z, block of GROUPS columns).  Sources: s = 0,1 -> w+, w-;
+// s = 2+m -> g_m.  D array order: 0/1 xi+ , 2/3 xi- , 4/5 w+ , 6/7 w- , 8+2m / 9+2m g_m  (even: f, odd: df/dy).
+// The [Ky][GROUPS] tile of retained modes arrives by one bulk async copy per row (TMA engine) into a padded
+// shared-memory tile; every lane group then reads its column once per output array (f, then i ky f, Eq. 10; the
+// Elsasser sources first give xi = -w/kperp^2, then w) -- no second copy of the column in registers.
+// The next item's tile is requested as soon as the last read of the current one is done.
+template <int NY> struct YInvGeom {
+  using Y = YGeom<NY>;
+  static constexpr int LD = Y::GROUPS + 1;
+  static constexpr int KYMAX = 2 * (NY / 3) + 1;
+  static constexpr int XB = (FftGeom<NY>::S > 1 ? FftGeom<NY>::BUF : 0) + 2;            // doubles per group
+  static constexpr size_t SMEM = ((size_t)FftTw<NY>::COUNT + (size_t)KYMAX * LD) * sizeof(cd) + (size_t)Y::GROUPS * XB * sizeof(double);
+};
 template <int NY>
-__global__ void __launch_bounds__(GD_FFT_THREADS) k_yfwd(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
-                                                       const cd* __restrict__ tw, int ncols) {
+__global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __restrict__ H, cd* __restrict__ D,
+                                                        const cd* __restrict__ tw, int ncb, int nitems) {
+  using Y = YGeom<NY>;
   using G = FftGeom<NY>;
-  constexpr int T = G::T, E = G::E;
+  using YI = YInvGeom<NY>;
+  constexpr int T = G::T, E = G::E, LD = YI::LD;
   extern __shared__ cd smem[];
+  __shared__ unsigned long long bar;
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
-  const int gid = blockIdx.x * (GD_FFT_THREADS / T) + grp;
-  cd* buf = smem + FftTw<NY>::COUNT + (size_t)grp * (G::BUF + 1);
-  fft_load_table<NY>(smem, tw);
+  cd* tile = smem + FftTw<NY>::COUNT;
+  double* xbuf = reinterpret_cast<double*>(tile + (size_t)YI::KYMAX * LD) + (size_t)grp * YI::XB;
+  if (threadIdx.x == 0) mbar_init(&bar, 1);
+  fft_load_table<NY>(smem, tw);                  // ends with __syncthreads()
   const cd* tws = smem;
-  const bool active = gid < ncols;
-  const int cx = active ? gid % d.Kx : 0;
-  const int ez = active ? gid / d.Kx : 0;
-  const int z = ez % d.nz, e = ez / d.nz;
-  const size_t ibase = (size_t)z * NY * d.Kx + cx;
-  const size_t obase = (size_t)z * d.Ky * d.Kx + cx;
-  cd v[E];
-  auto load = [&](int a) {
-    const cd* src = Ein + (size_t)a * d.PD + ibase;
-#pragma unroll
-    for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * d.Kx) : cmake(0.0, 0.0);
-    fft_lanes<NY, -1>(v, t, buf, tws);
+  auto issue = [&](int item) {                   // all threads: one bulk copy per tile row (row = retained ky)
+    const int cb = item % ncb, sz = item / ncb;
+    const int z = sz % d.nz, s = sz / d.nz;
+    const int cx0 = cb * Y::GROUPS;
+    const int ncol = min(Y::GROUPS, d.Kx - cx0);
+    if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(d.Ky * ncol * sizeof(cd)));
+    for (int r = threadIdx.x; r < d.Ky; r += GD_Y_THREADS)
+      bulk_g2s(tile + (size_t)r * LD, H + (size_t)s * d.PH + ((size_t)z * d.Ky + r) * d.Kx + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
   };
-  if (e == 0) {
-    cd va[E];
-    load(0);
-#pragma unroll
-    for (int q = 0; q < E; ++q) va[q] = v[q];
-    load(1);
-    if (active) {
-      const double kx = d.kx0 * cx;
+  int item = blockIdx.x;
+  if (item < nitems) issue(item);
+  unsigned phase = 0;
+  while (item < nitems) {
+    const int cb = item % ncb, sz = item / ncb;
+    const int z = sz % d.nz, s = sz / d.nz;
+    const int cx = cb * Y::GROUPS + grp;
+    const bool active = cx < d.Kx;
+    const double kx = d.kx0 * cx;
+    const size_t obase = (size_t)z * NY * d.Kx + (active ? cx : 0);
+    const int rounds = (s < 2) ? 4 : 2;
+    mbar_wait(&bar, phase);
+    phase ^= 1u;
+    item += gridDim.x;
+    for (int r = 0; r < rounds; ++r) {
+      const bool pot = (s < 2) && (r < 2);       // rounds 0,1 of an Elsasser source: the potential xi = -w/kperp^2
+      const int which = r & 1;                   // 0: f, 1: df/dy
+      const int a = (s < 2 ? (pot ? 2 * s : 4 + 2 * s) : 8 + 2 * (s - 2)) + which;
+      cd v[E];
 #pragma unroll
       for (int q = 0; q < E; ++q) {
-        const int iy = t + T * q;
-        const int cy = fft2c(iy, NY, d.hy3, d.Ky);
-        if (cy >= 0) {
-          const double ky = d.ky0 * fft2n(iy, NY);
-          const double hk2 = 0.5 * (kx * kx + ky * ky);
-          // N+- = -1/2 A -+ 1/2 kperp^2 B
-          const cd np = cmake(-0.5 * va[q].x - hk2 * v[q].x, -0.5 * va[q].y - hk2 * v[q].y);
-          const cd nm = cmake(-0.5 * va[q].x + hk2 * v[q].x, -0.5 * va[q].y + hk2 * v[q].y);
-          st_cd(Gh + obase + (size_t)cy * d.Kx, np);
-          st_cd(Gh + d.PH + obase + (size_t)cy * d.Kx, nm);
+        const int cy = fft2c(t + T * q, NY, d.hy3, d.Ky);
+        v[q] = (active && cy >= 0) ? tile[(size_t)cy * LD + grp] : cmake(0.0, 0.0);
+      }
+      if (r == rounds - 1) {
+        __syncthreads();                         // last read of the tile by every lane
+        if (item < nitems) issue(item);          // prefetch: overlaps the transform and the stores below
+      }
+      if (pot || which) {
+#pragma unroll
+        for (int q = 0; q < E; ++q) {
+          const double ky = d.ky0 * fft2n(t + T * q, NY);
+          double f = 1.0;
+          if (pot) { const double k2 = kx * kx + ky * ky; f = k2 > 0.0 ? -1.0 / k2 : 0.0; }
+          if (which) v[q] = cscale(mul_i(v[q]), f * ky);
+          else v[q] = cscale(v[q], f);
         }
       }
+      fft_lanes_split<NY, +1>(v, t, xbuf, tws);
+      if (active) {
+        cd* dst = D + (size_t)a * d.PD + obase;
+#pragma unroll
+        for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * d.Kx, v[q]);
+      }
     }
-  } else {
-    load(1 + e);
+  }
+}
+
+// P3.  E arrays: 0 A, 1 B, 2+m R_m.  Output hybrid fields: 0 N+, 1 N-, 2+m R_m.
+// The [ny][GROUPS] input tile of a work item arrives by one bulk async copy per row (TMA engine, mbarrier
+// completion) into a padded shared-memory tile, so the global side moves whole row segments and the lanes then read
+// their own column conflict-free.
+//
+// k_yfwd_pair: work item (z, block of GROUPS/2 columns): the two halves of the CTA transform A and B of the same
+// columns, hand the results over through shared memory and form N+- = -1/2 A -+ 1/2 kperp^2 B  (Eq. 1 with
+// Eq. 11).  The FFT exchange buffers alias the tile once every lane holds its column.
+template <int NY>
+__global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
+                                                             const cd* __restrict__ tw, int ncb) {
+  using Y = YGeom<NY>;
+  using G = FftGeom<NY>;
+  constexpr int T = G::T, E = G::E;
+  constexpr int HG = Y::GROUPS / 2;
+  constexpr int LD = Y::GROUPS + 1;              // padded tile row (complex entries)
+  extern __shared__ cd smem[];
+  __shared__ unsigned long long bar;
+  const int grp = threadIdx.x / T, t = threadIdx.x % T;
+  cd* tile = smem + FftTw<NY>::COUNT;
+  cd* buf = tile + (size_t)grp * Y::YBUF;
+  const int cb = blockIdx.x % ncb, z = blockIdx.x / ncb;
+  const int which = grp / HG;
+  const int cx0 = cb * HG;
+  const int cx = cx0 + grp % HG;
+  const bool active = cx < d.Kx;
+  const int ncol = min(HG, d.Kx - cx0);          // columns of this block that exist
+  if (threadIdx.x == 0) mbar_init(&bar, 1);
+  fft_load_table<NY>(smem, tw);                  // ends with __syncthreads()
+  if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(NY * ncol * 2 * sizeof(cd)));
+  for (int r = threadIdx.x; r < NY; r += GD_Y_THREADS) {
+    const cd* src = Ein + ((size_t)z * NY + r) * d.Kx + cx0;
+    bulk_g2s(tile + (size_t)r * LD, src, (unsigned)(ncol * sizeof(cd)), &bar);
+    bulk_g2s(tile + (size_t)r * LD + HG, src + d.PD, (unsigned)(ncol * sizeof(cd)), &bar);
+  }
+  const cd* tws = smem;
+  mbar_wait(&bar, 0);
+  cd v[E];
+#pragma unroll
+  for (int q = 0; q < E; ++q) v[q] = active ? tile[(size_t)(t + T * q) * LD + grp] : cmake(0.0, 0.0);
+  __syncthreads();                               // tile consumed: the exchange buffers may overwrite it
+  fft_lanes<NY, -1>(v, t, buf, tws);
+  // hand-over: every group publishes its transform, the sibling (other array, same column) reads it
+  __syncwarp();
+#pragma unroll
+  for (int q = 0; q < E; ++q) buf[t + T * q] = v[q];
+  __syncthreads();
+  const cd* sib = tile + (size_t)(grp ^ HG) * Y::YBUF;
+  const double kx = d.kx0 * cx;
+  if (active) {
+    cd* dst = Gh + (size_t)which * d.PH + (size_t)z * d.Ky * d.Kx + cx;
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+      const int cy = fft2c(t + T * q, NY, d.hy3, d.Ky);
+      if (cy >= 0) {
+        const cd o = sib[t + T * q];
+        const cd A = which ? o : v[q], B = which ? v[q] : o;
+        const double ky = d.ky0 * fft2n(t + T * q, NY);
+        const double hk2 = (which ? 0.5 : -0.5) * (kx * kx + ky * ky);
+        st_cd(dst + (size_t)cy * d.Kx, cmake(-0.5 * A.x + hk2 * B.x, -0.5 * A.y + hk2 * B.y));
+      }
+    }
+  }
+}
+
+// k_yfwd: persistent CTAs over the work items (array a >= 2, z, block of GROUPS columns).  The exchange uses its
+// own (split, 8-byte) buffers, so the NEXT item's tile is in flight while the current one is transformed and stored.
+template <int NY> struct YFwdGeom {
+  using Y = YGeom<NY>;
+  static constexpr int LD = Y::GROUPS + 1;
+  static constexpr int XB = (FftGeom<NY>::S > 1 ? FftGeom<NY>::BUF : 0) + 2;            // doubles per group (even: 16-B alignment)
+  static constexpr size_t SMEM = ((size_t)FftTw<NY>::COUNT + (size_t)NY * LD) * sizeof(cd) + (size_t)Y::GROUPS * XB * sizeof(double);
+};
+template <int NY>
+__global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
+                                                        const cd* __restrict__ tw, int ncb, int nitems) {
+  using Y = YGeom<NY>;
+  using G = FftGeom<NY>;
+  using YF = YFwdGeom<NY>;
+  constexpr int T = G::T, E = G::E, LD = YF::LD;
+  extern __shared__ cd smem[];
+  __shared__ unsigned long long bar;
+  const int grp = threadIdx.x / T, t = threadIdx.x % T;
+  cd* tile = smem + FftTw<NY>::COUNT;
+  double* xbuf = reinterpret_cast<double*>(tile + (size_t)NY * LD) + (size_t)grp * YF::XB;
+  if (threadIdx.x == 0) mbar_init(&bar, 1);
+  fft_load_table<NY>(smem, tw);                  // ends with __syncthreads()
+  const cd* tws = smem;
+  auto issue = [&](int item) {                   // all threads: one bulk copy per tile row
+    const int cb = item % ncb, az = item / ncb;
+    const int z = az % d.nz, a = 2 + az / d.nz;
+    const int cx0 = cb * Y::GROUPS;
+    const int ncol = min(Y::GROUPS, d.Kx - cx0);
+    if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(NY * ncol * sizeof(cd)));
+    for (int r = threadIdx.x; r < NY; r += GD_Y_THREADS)
+      bulk_g2s(tile + (size_t)r * LD, Ein + (size_t)a * d.PD + ((size_t)z * NY + r) * d.Kx + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
+  };
+  int item = blockIdx.x;
+  if (item < nitems) issue(item);
+  unsigned phase = 0;
+  while (item < nitems) {
+    const int cb = item % ncb, az = item / ncb;
+    const int z = az % d.nz, a = 2 + az / d.nz;
+    const int cx = cb * Y::GROUPS + grp;
+    const bool active = cx < d.Kx;
+    mbar_wait(&bar, phase);
+    phase ^= 1u;
+    cd v[E];
+#pragma unroll
+    for (int q = 0; q < E; ++q) v[q] = active ? tile[(size_t)(t + T * q) * LD + grp] : cmake(0.0, 0.0);
+    __syncthreads();                             // tile consumed by every lane
+    item += gridDim.x;
+    if (item < nitems) issue(item);              // prefetch: overlaps the transform and the stores below
+    fft_lanes_split<NY, -1>(v, t, xbuf, tws);
     if (active) {
-      cd* dst = Gh + (size_t)(1 + e) * d.PH + obase;
+      cd* dst = Gh + (size_t)a * d.PH + (size_t)z * d.Ky * d.Kx + cx;
 #pragma unroll
       for (int q = 0; q < E; ++q) {
         const int cy = fft2c(t + T * q, NY, d.hy3, d.Ky);
@@ -181,9 +280,11 @@ __global__ void __launch_bounds__(GD_FFT_THREADS) k_yfwd(Dims d, const cd* __res
   }
 }
 
+static int g_num_sms = 148;   // persistent kernels launch 2 CTAs per SM
+
 // ---- launchers ------------------------------------------------------------------------------------
-template <int N> static size_t fft_smem() { return ((size_t)(GD_FFT_THREADS / FftGeom<N>::T) * (FftGeom<N>::BUF + 1) + FftTw<N>::COUNT) * sizeof(cd); }
-template <int N> static int fft_blocks(long long ncols) { const int gpb = GD_FFT_THREADS / FftGeom<N>::T; return (int)((ncols + gpb - 1) / gpb); }
+template <int N> static size_t fft_smem() { return ((size_t)(GD_Z_THREADS / FftGeom<N>::T) * (FftGeom<N>::BUF + 1) + FftTw<N>::COUNT) * sizeof(cd); }
+template <int N> static int fft_blocks(long long ncols) { const int gpb = GD_Z_THREADS / FftGeom<N>::T; return (int)((ncols + gpb - 1) / gpb); }
 
 #define GD_DISPATCH(NVAL, MACRO)                                                      \
   switch (NVAL) {                                                                     \
@@ -196,22 +297,57 @@ template <int N> static int fft_blocks(long long ncols) { const int gpb = GD_FFT
 cudaError_t launch_zfft(const Dims& d, int dir, const cd* in, cd* out, const cd* tw, int nfields, cudaStream_t st) {
   const long long ncols = (long long)nfields * d.Ky * d.Kx;
 #define ZCASE(NN)                                                                                         \
-  if (dir > 0) k_zfft<NN, +1><<<fft_blocks<NN>(ncols), GD_FFT_THREADS, fft_smem<NN>(), st>>>(d, in, out, tw, (int)ncols); \
-  else k_zfft<NN, -1><<<fft_blocks<NN>(ncols), GD_FFT_THREADS, fft_smem<NN>(), st>>>(d, in, out, tw, (int)ncols);
+  if (dir > 0) k_zfft<NN, +1><<<fft_blocks<NN>(ncols), GD_Z_THREADS, fft_smem<NN>(), st>>>(d, in, out, tw, (int)ncols); \
+  else k_zfft<NN, -1><<<fft_blocks<NN>(ncols), GD_Z_THREADS, fft_smem<NN>(), st>>>(d, in, out, tw, (int)ncols);
   GD_DISPATCH(d.nz, ZCASE)
   return cudaGetLastError();
 }
 cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStream_t st) {
-  const long long ncols = (long long)d.F * d.nz * d.Kx;
-#define YICASE(NN) k_yinv<NN><<<fft_blocks<NN>(ncols), GD_FFT_THREADS, fft_smem<NN>(), st>>>(d, H, D, tw, (int)ncols);
+#define YICASE(NN)                                                                                         \
+  {                                                                                                        \
+    const int ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;                                    \
+    const int nitems = d.F * d.nz * ncb;                                                                   \
+    k_yinv<NN><<<nitems < 2 * g_num_sms ? nitems : 2 * g_num_sms, GD_Y_THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, nitems); \
+  }
   GD_DISPATCH(d.ny, YICASE)
   return cudaGetLastError();
 }
 cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, cudaStream_t st) {
-  const long long ncols = (long long)(1 + d.M) * d.nz * d.Kx;
-#define YFCASE(NN) k_yfwd<NN><<<fft_blocks<NN>(ncols), GD_FFT_THREADS, fft_smem<NN>(), st>>>(d, E, Gh, tw, (int)ncols);
+#define YFCASE(NN)                                                                                         \
+  {                                                                                                        \
+    constexpr int HG = YGeom<NN>::GROUPS / 2;                                                              \
+    const int ncb2 = (d.Kx + HG - 1) / HG, ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;       \
+    k_yfwd_pair<NN><<<d.nz * ncb2, GD_Y_THREADS, YGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb2);               \
+    const int nitems = d.M * d.nz * ncb;                                                                   \
+    if (d.M > 0) k_yfwd<NN><<<nitems < 2 * g_num_sms ? nitems : 2 * g_num_sms, GD_Y_THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, nitems); \
+  }
   GD_DISPATCH(d.ny, YFCASE)
   return cudaGetLastError();
+}
+// opt-in dynamic shared memory above 48 KB for every instantiation
+cudaError_t prepare_passes_zy(int ny, int nz) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+  if (g_num_sms <= 0) g_num_sms = 148;
+#define ZPCASE(NN)                                                                                                         \
+  {                                                                                                                        \
+    cudaError_t e = cudaFuncSetAttribute(k_zfft<NN, +1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<NN>());  \
+    if (e != cudaSuccess) return e;                                                                                        \
+    e = cudaFuncSetAttribute(k_zfft<NN, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<NN>());             \
+    if (e != cudaSuccess) return e;                                                                                        \
+  }
+  GD_DISPATCH(nz, ZPCASE)
+#define YPCASE(NN)                                                                                                         \
+  {                                                                                                                        \
+    cudaError_t e = cudaFuncSetAttribute(k_yinv<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YInvGeom<NN>::SMEM); \
+    if (e != cudaSuccess) return e;                                                                                        \
+    e = cudaFuncSetAttribute(k_yfwd_pair<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YGeom<NN>::SMEM);          \
+    if (e != cudaSuccess) return e;                                                                                        \
+    e = cudaFuncSetAttribute(k_yfwd<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YFwdGeom<NN>::SMEM);            \
+    if (e != cudaSuccess) return e;                                                                                        \
+  }
+  GD_DISPATCH(ny, YPCASE)
+  return cudaSuccess;
 }
 
 // Host: the stage twiddle table of length-n transforms (fft.cuh layout); empty for single-stage sizes.
