@@ -17,6 +17,7 @@ cudaError_t launch_zfft(const Dims& d, int dir, const cd* in, cd* out, const cd*
 cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStream_t st);
 cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, cudaStream_t st);
 cudaError_t prepare_passes_zy(int ny, int nz);
+int xpass_lines_per_cta(int nx);
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
                          unsigned long long* maxbits, cudaStream_t st, bool prepare_only);
 cudaError_t launch_update(const Dims& d, const PhysParams& p, int mode, const cd* G, const cd* Wn, const cd* Ws, cd* Wout,
@@ -155,7 +156,10 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   d.Kx = d.hx3 + 1; d.Ky = 2 * d.hy3 + 1; d.Kz = 2 * d.hz3 + 1;
   d.kx0 = 2.0 * kPi / p->Lx; d.ky0 = 2.0 * kPi / p->Ly; d.kz0 = 2.0 * kPi / p->Lz;
   d.inv_n = 1.0 / ((double)p->nx * p->ny * p->nz);
-  d.PS = (size_t)d.Kz * d.Ky * d.Kx; d.PH = (size_t)d.nz * d.Ky * d.Kx; d.PD = (size_t)d.nz * d.ny * d.Kx;
+  d.PS = (size_t)d.Kz * d.Ky * d.Kx; d.PH = (size_t)d.nz * d.Ky * d.Kx; d.PE = (size_t)d.nz * d.ny * d.Kx;
+  d.xl = xpass_lines_per_cta(d.nx);
+  d.xlsh = 0; while ((1 << d.xlsh) < d.xl) ++d.xlsh;
+  { const size_t nlb = ((size_t)d.ny * d.nz + d.xl - 1) / d.xl; d.PD = nlb * d.Kx * (size_t)d.xl; }
   PhysParams& ph = c->ph;
   ph.vA = p->vA; ph.eta = p->eta; ph.r = p->r; ph.eta_normalized = p->eta_normalized;
   ph.eta_z = p->eta_z; ph.r_z = p->r_z; ph.eta_g = p->eta_g;
@@ -168,7 +172,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   A(dalloc(&c->S0, F * d.PS)); A(dalloc(&c->S1, F * d.PS)); A(dalloc(&c->SG, F * d.PS));
   A(dalloc(&c->H, F * d.PH)); A(dalloc(&c->Gh, F * d.PH));
-  A(dalloc(&c->D, (size_t)2 * (F + 2) * d.PD)); A(dalloc(&c->E, F * d.PD));
+  A(dalloc(&c->D, (size_t)2 * (F + 2) * d.PD)); A(dalloc(&c->E, F * d.PE));
   A(dalloc(&c->cdn, (size_t)M + 1)); A(dalloc(&c->cup, (size_t)M + 1)); A(dalloc(&c->crate, (size_t)M + 1));
   A(dalloc(&c->collfac, (size_t)M + 1)); A(dalloc(&c->scal, (size_t)SC_COUNT));
   A(dalloc(&c->partial, (size_t)kEnergyBlocks * 5)); A(dalloc(&c->rec_scratch, (size_t)8));

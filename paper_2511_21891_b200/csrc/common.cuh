@@ -4,7 +4,9 @@
 // the modes Eq. 20 keeps: 3|n| <= N):
 //   compact  S[f][cz][cy][cx]   Kz*Ky*Kx per field   fully spectral state / RHS
 //   hybrid   H[f][z ][cy][cx]   nz*Ky*Kx per field   z in real space, (kx,ky) spectral
-//   xy-real  D[a][z ][y ][cx]   nz*ny*Kx per array   y,z real, kx spectral (retained kx only)
+//   xy-real  D[a][lb][cx][xl]   y,z real, kx spectral (retained kx only); line = z*ny+y = lb*xl + li, stored at slot
+//                               li ^ (cx % xl): the tile of an x-pass CTA (xl lines) is one contiguous run (P1 -> P2)
+//            E[a][z ][y ][cx]   nz*ny*Kx per array   same space, kx fastest (P2 -> P3)
 // cx = 0..Kx-1 is n_x = cx; cy = 0..Ky-1 is n_y = cy (cy <= hy3) or cy-Ky (negative modes);
 // cz likewise.  The zeroed third is never stored or transformed.
 #pragma once
@@ -18,7 +20,8 @@ struct Dims {
   int hx3, hy3, hz3;      // floor(N/3)
   double kx0, ky0, kz0;   // 2 pi / L
   double inv_n;           // 1/(nx ny nz)
-  size_t PS, PH, PD;      // per-field strides (complex elements) of the three spaces
+  int xl, xlsh;           // lines per x-pass CTA (power of two) and its log2: block size of the D layout
+  size_t PS, PH, PD, PE;  // per-field strides (complex elements): compact, hybrid, D (blocked, padded), E
 };
 
 __device__ __forceinline__ int c2n(int c, int h3, int K) { return c <= h3 ? c : c - K; }        // compact -> signed mode

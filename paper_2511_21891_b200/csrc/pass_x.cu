@@ -21,11 +21,13 @@ struct XGeom {
   static constexpr int T = G::T, E = G::E;
   static constexpr int LB = NX + NX / G::PADDIV + 1;        // line buffer (FFT exchange + unpack), complex entries
   static constexpr int KXP = NX / 3 + 1;                    // retained kx count (== Dims::Kx)
-  static constexpr int STG = 2 * KXP;                       // staging buffer: the two half-lines (f, df/dy) of the NEXT field
-  static constexpr int PER_GROUP = LB + STG;
   static constexpr int THREADS = 256;                       // 8 warps, one CTA per SM (it owns all 512 TMEM columns)
-  static constexpr int GROUPS = THREADS / T;
-  static constexpr size_t SMEM = ((size_t)GROUPS * PER_GROUP + FftTw<NX>::COUNT) * sizeof(cd);
+  static constexpr int WARPS = THREADS / 32;
+  static constexpr int GROUPS = THREADS / T;                // lines per CTA: consecutive (z,y), y fastest
+  static constexpr int LD = GROUPS;                         // row of a staged tile [kx][line]; line slot XOR-swizzled with kx
+  static constexpr int STAGE = 2 * KXP * LD;                // one stage: the tiles of f~ and (df/dy)~ for all lines of the CTA
+  static constexpr int NST = 3;                             // stages in flight (full/empty mbarrier ring)
+  static constexpr size_t SMEM = ((size_t)GROUPS * LB + (size_t)NST * STAGE + FftTw<NX>::COUNT) * sizeof(cd);
   // Tensor memory as a thread-private scratchpad (tcgen05.ld/st, shape 32x32b: lane i of a warp owns TMEM lane
   // 32*(warp%4)+i).  Per thread: 8 words per x-point for (Phi_x,Phi_y,Psi_x,Psi_y) and 2 words per x-point for the
   // parked R_{m-2}.  Warps sharing a lane quarter take consecutive column slots.
@@ -70,10 +72,15 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   extern __shared__ cd smem[];
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   const int line = blockIdx.x * X::GROUPS + grp;
-  cd* buf = smem + FftTw<NX>::COUNT + (size_t)grp * X::PER_GROUP;
-  cd* sStage = buf + X::LB;        // [0,KX): f~(kx), [KX,2KX): (df/dy)~(kx) of the field being fetched
+  cd* buf = smem + FftTw<NX>::COUNT + (size_t)grp * X::LB;
+  cd* stages = smem + FftTw<NX>::COUNT + (size_t)X::GROUPS * X::LB;   // NST x [2][KX][LD]: f~ and (df/dy)~ tiles, [kx][line]
   __shared__ unsigned s_tmem_base;
+  __shared__ unsigned long long s_full[X::NST], s_empty[X::NST];
   const int warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int i = 0; i < X::NST; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], X::WARPS); }
+  }
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&s_tmem_base)), "r"(512) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -85,22 +92,26 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   // this warp's TMEM window: lane quarter warp%4, column slot warp/4
   const unsigned tm = s_tmem_base + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * X::TM_SLOT);
   const bool active = line < nlines;
-  const size_t base = (size_t)(active ? line : 0) * KX;       // (z*ny + y)*Kx
+  const size_t base = (size_t)(active ? line : 0) * KX;       // (z*ny + y)*Kx  (output arrays E, kx fastest)
   const int M = d.M;
   cd v[E];
   double Qp[E], Ra[E];             // Hermite sliding window; Qp doubles as the {xi+,w-} accumulator of the Elsasser part
 
-  // asynchronous fetch (cp.async, 16 B per lane) of the two half-lines of array a, a+1 into the staging buffer
-  auto fetch = [&](int a) {
-    if (active) {
-      const cd* pf = D + (size_t)a * d.PD + base;
-      const unsigned sbase = (unsigned)__cvta_generic_to_shared(sStage);
-      for (int c = t; c < 2 * KX; c += T) {
-        const cd* src = (c < KX) ? pf + c : pf + d.PD + (c - KX);
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sbase + 16u * (unsigned)c), "l"(src) : "memory");
-      }
+  // Producer (lane 0 of warp 0): the tiles of arrays a, a+1 for the lines of this CTA.  D[a][line block][kx][LD] is laid
+  // out so that a CTA's tile is ONE contiguous run (line slot XOR-swizzled with kx against bank conflicts): one bulk async copy (TMA engine) per array into
+  // stage kn % NST; completion on s_full, reuse gated by s_empty.
+  auto produce = [&](int kn, int a) {
+    const int sn = kn % X::NST;
+    if (kn >= X::NST) mbar_wait(&s_empty[sn], (unsigned)((kn / X::NST - 1) & 1));
+    if ((threadIdx.x & 31) == 0) {
+      constexpr unsigned TILE_BYTES = (unsigned)(KX * X::LD * sizeof(cd));
+      mbar_arrive_expect_tx(&s_full[sn], 2u * TILE_BYTES);
+      cd* st = stages + (size_t)sn * X::STAGE;
+      const cd* src = D + (size_t)a * d.PD + (size_t)blockIdx.x * (KX * X::LD);
+      bulk_g2s(st, src, TILE_BYTES, &s_full[sn]);
+      bulk_g2s(st + KX * X::LD, src + d.PD, TILE_BYTES, &s_full[sn]);
     }
-    asm volatile("cp.async.commit_group;" ::: "memory");
+    __syncwarp();
   };
   // Job list of one line.  Kinds 0..3 are the inverse transforms of xi+, xi-, w-, w+; kind 4+m that of g_m.
   // After kind 3 and after every second moment a forward job (pair of real lines) follows.  Inverse transforms
@@ -112,7 +123,9 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   bool tail_done = (M == 0);
   int e0 = 0, e1 = 1;
   double gmax = 0.0;
-  fetch(src_array(0));
+  if (warp == 0) {
+    for (int kn = 0; kn < X::NST - 1 && kn < nkinds; ++kn) produce(kn, src_array(kn));
+  }
   for (;;) {
     if (!fwd) {
       if (kind == nkinds) {
@@ -138,30 +151,33 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
           e0 = 2 + M - 1; e1 = -1;
         }
       } else {
-        // wait for the staged half-lines and pack conj(Z), Z = Fx + i Fy, Fx = i kx f  (Hermitian completion for kx < 0)
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncwarp();
-        const cd* pf = sStage;
-        const cd* pfy = sStage + KX;
+        // wait for the staged tiles and pack conj(Z), Z = Fx + i Fy, Fx = i kx f  (Hermitian completion for kx < 0)
+        const int sc = kind % X::NST;
+        mbar_wait(&s_full[sc], (unsigned)((kind / X::NST) & 1));
+        const cd* pf = stages + (size_t)sc * X::STAGE;            // element n of this line: pf[n * LD + (grp ^ (n & (LD-1)))]
+        const cd* pfy = pf + (size_t)KX * X::LD;
 #pragma unroll
         for (int q = 0; q < E; ++q) {
           const int n = t + T * q;
           cd z = cmake(0.0, 0.0);
           if (T * q <= HX3 && n <= HX3) {                       // first test is compile-time per q
-            cd f = pf[n], fy = pfy[n];
+            const int o = n * X::LD + (grp ^ (n & (X::LD - 1)));
+            cd f = pf[o], fy = pfy[o];
             if (n == 0) { f.y = 0.0; fy.y = 0.0; }
             const double kx = d.kx0 * n;
             z = cmake(-kx * f.y - fy.y, -(kx * f.x + fy.x));    // conj( i kx f + i fy )
           } else if (T * q + T - 1 >= NX - HX3 && n >= NX - HX3) {
             const int c = NX - n;
-            const cd f = pf[c], fy = pfy[c];
+            const int o = c * X::LD + (grp ^ (c & (X::LD - 1)));
+            const cd f = pf[o], fy = pfy[o];
             const double kx = d.kx0 * c;
             z = cmake(-kx * f.y + fy.y, kx * f.x - fy.x);       // conj( conj(i kx f) + i conj(fy) )
           }
           v[q] = z;
         }
-        __syncwarp();                   // every lane has consumed the staging buffer
-        if (kind + 1 < nkinds) fetch(src_array(kind + 1));
+        __syncwarp();                   // every lane of the warp has consumed the stage
+        if ((threadIdx.x & 31) == 0) mbar_arrive(&s_empty[sc]);
+        if (warp == 0 && kind + X::NST - 1 < nkinds) produce(kind + X::NST - 1, src_array(kind + X::NST - 1));
       }
     }
 
@@ -174,8 +190,8 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
       for (int q = 0; q < E; ++q) buf[G::pad(t + T * q)] = v[q];
       __syncwarp();
       if (active) {
-        cd* p0 = Eo + (size_t)e0 * d.PD + base;
-        cd* p1 = Eo + (size_t)(e1 < 0 ? e0 : e1) * d.PD + base;
+        cd* p0 = Eo + (size_t)e0 * d.PE + base;
+        cd* p1 = Eo + (size_t)(e1 < 0 ? e0 : e1) * d.PE + base;
 #pragma unroll
         for (int q = 0; q < E; ++q) {
           const int c = t + T * q;
@@ -275,6 +291,16 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem_base), "r"(512) : "memory");
+}
+
+// lines per x-pass CTA (the block size of the D layout)
+int xpass_lines_per_cta(int nx) {
+  switch (nx) {
+    case 8: return XGeom<8>::GROUPS; case 16: return XGeom<16>::GROUPS; case 32: return XGeom<32>::GROUPS;
+    case 64: return XGeom<64>::GROUPS; case 128: return XGeom<128>::GROUPS; case 256: return XGeom<256>::GROUPS;
+    case 512: return XGeom<512>::GROUPS;
+    default: return 0;
+  }
 }
 
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,

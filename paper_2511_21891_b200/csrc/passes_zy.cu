@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
     const int cx = cb * Y::GROUPS + grp;
     const bool active = cx < d.Kx;
     const double kx = d.kx0 * cx;
-    const size_t obase = (size_t)z * NY * d.Kx + (active ? cx : 0);
+    const int cxa = active ? cx : 0;
     const int rounds = (s < 2) ? 4 : 2;
     mbar_wait(&bar, phase);
     phase ^= 1u;
@@ -147,9 +147,15 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
       }
       fft_lanes_split<NY, +1>(v, t, xbuf, tws);
       if (active) {
-        cd* dst = D + (size_t)a * d.PD + obase;
+        // D[a][line block][kx][xl], line = z*ny + y, slot (line % xl) ^ (kx % xl): the lanes of a group fill whole
+        // aligned runs of one block row
+        cd* dst = D + (size_t)a * d.PD;
+        const int sw = cxa & (d.xl - 1);
 #pragma unroll
-        for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * d.Kx, v[q]);
+        for (int q = 0; q < E; ++q) {
+          const int line = z * NY + t + T * q;
+          st_cd(dst + (((size_t)(line >> d.xlsh) * d.Kx + cxa) << d.xlsh) + ((line & (d.xl - 1)) ^ sw), v[q]);
+        }
       }
     }
   }
@@ -188,7 +194,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd_pair(Dims d, const cd*
   for (int r = threadIdx.x; r < NY; r += GD_Y_THREADS) {
     const cd* src = Ein + ((size_t)z * NY + r) * d.Kx + cx0;
     bulk_g2s(tile + (size_t)r * LD, src, (unsigned)(ncol * sizeof(cd)), &bar);
-    bulk_g2s(tile + (size_t)r * LD + HG, src + d.PD, (unsigned)(ncol * sizeof(cd)), &bar);
+    bulk_g2s(tile + (size_t)r * LD + HG, src + d.PE, (unsigned)(ncol * sizeof(cd)), &bar);
   }
   const cd* tws = smem;
   mbar_wait(&bar, 0);
@@ -250,7 +256,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd(Dims d, const cd* __re
     const int ncol = min(Y::GROUPS, d.Kx - cx0);
     if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(NY * ncol * sizeof(cd)));
     for (int r = threadIdx.x; r < NY; r += GD_Y_THREADS)
-      bulk_g2s(tile + (size_t)r * LD, Ein + (size_t)a * d.PD + ((size_t)z * NY + r) * d.Kx + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
+      bulk_g2s(tile + (size_t)r * LD, Ein + (size_t)a * d.PE + ((size_t)z * NY + r) * d.Kx + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
   };
   int item = blockIdx.x;
   if (item < nitems) issue(item);
