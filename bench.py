@@ -55,8 +55,8 @@ def algorithmic_bytes(shape, M):
         "y_inverse_P1": F * S_h + 2 * (F + 2) * S_xy,
         "x_pass_P2": 2 * (F + 2) * S_xy + F * S_xy,
         "y_forward_P3": F * S_xy + F * S_h,
-        "z_forward": F * (S_h + S_c),
-        "update": (3 * F + M / 2) * S_c,          # predictor 3F, corrector 3F + M (stage-state stencil): mean
+        # fused z-forward + update + z-inverse: per step 4F S_h + (3F + 2M) S_c (SURVEY 8(d) "P4"); per launch half of it
+        "z_step_P4": 2 * F * S_h + (1.5 * F + M) * S_c,
     }
     p4 = 4 * F * S_h + (3 * F + 2 * M) * S_c
     step_4pass = 2 * (per_launch["y_inverse_P1"] + per_launch["x_pass_P2"] + per_launch["y_forward_P3"]) + p4

@@ -126,8 +126,9 @@ int gandalf_get_time(gandalf_ctx* ctx, double* t, long long* step, double* last_
 long long gandalf_launch_count(const gandalf_ctx* ctx);
 
 /* Event-timed average duration (ms) of one named kernel class since the last reset; used by
- * bench.py for the roofline line.  which: 0 z-inverse, 1 y-inverse (P1), 2 x-pass (P2),
- * 3 y-forward (P3), 4 z-forward, 5 update.  Timing is off unless enabled (it inserts events). */
+ * bench.py for the roofline line.  which: 0 z-inverse (set_state / after forcing only), 1 y-inverse (P1),
+ * 2 x-pass (P2), 3 y-forward (P3), 4 fused z-forward + stage update + z-inverse (P4).
+ * Timing is off unless enabled (it inserts events). */
 int gandalf_kernel_timing(gandalf_ctx* ctx, int enable);
 int gandalf_kernel_time_ms(gandalf_ctx* ctx, int which, double* avg_ms, long long* launches);
 

@@ -20,8 +20,10 @@ cudaError_t prepare_passes_zy(int ny, int nz);
 int xpass_lines_per_cta(int nx);
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
                          unsigned long long* maxbits, cudaStream_t st, bool prepare_only);
-cudaError_t launch_update(const Dims& d, const PhysParams& p, int mode, const cd* G, const cd* Wn, const cd* Ws, cd* Wout,
-                          const double* scal, const double* cdn, const double* cup, const double* collfac, cudaStream_t st);
+cudaError_t launch_zstep(const Dims& d, int mode, int if_variant, int g_sign, const cd* Gh, const cd* Wn, const cd* Ws, cd* Wout, cd* Hout,
+                         const double* scal, const double* cdn, const double* cup, const double* collfac, const double* tabz,
+                         const double* tabp, const cd* tw, cudaStream_t st);
+cudaError_t launch_tables(const Dims& d, const PhysParams& p, const double* scal, double* tabz, double* tabp, cudaStream_t st);
 cudaError_t launch_prepare_dt(double fixed_dt, double cfl_dxy, const unsigned long long* maxbits, double* scal,
                               const double* crate, double* collfac, int M, cudaStream_t st);
 cudaError_t launch_zero_u64(unsigned long long* p, cudaStream_t st);
@@ -34,7 +36,7 @@ cudaError_t launch_energy(const Dims& d, const cd* S, double* partial, int nbloc
 cudaError_t launch_spectrum(const Dims& d, const cd* S, double* col, int nbins, int literal, double dk, double* out, cudaStream_t st);
 
 static const double kPi = 3.14159265358979323846264338327950288;
-enum { KC_ZINV = 0, KC_YINV = 1, KC_XPASS = 2, KC_YFWD = 3, KC_ZFWD = 4, KC_UPDATE = 5, KC_N = 6 };
+enum { KC_ZINV = 0, KC_YINV = 1, KC_XPASS = 2, KC_YFWD = 3, KC_ZSTEP = 4, KC_N = 5 };
 static const int kEnergyBlocks = 592;   // 4 x 148 SMs
 
 struct gandalf_ctx {
@@ -43,9 +45,9 @@ struct gandalf_ctx {
   PhysParams ph;
   cudaStream_t st;
   // device buffers
-  cd *S0, *S1, *SG, *H, *Gh, *D, *E;
+  cd *S0, *S1, *H, *Gh, *D, *E;
   cd *twx, *twy, *twz;
-  double *cdn, *cup, *crate, *collfac, *scal, *partial, *hist, *rec_scratch, *spec_col, *spec_out;
+  double *cdn, *cup, *crate, *collfac, *scal, *partial, *hist, *rec_scratch, *spec_col, *spec_out, *tabz, *tabp;
   unsigned long long* maxbits;
   int* pairs; int npairs; double force_amp;
   cd* io; size_t io_bytes;
@@ -88,7 +90,7 @@ static cudaError_t upload_twiddles(cd** dst, int n, cudaStream_t st) {
 }
 
 static void free_all(gandalf_ctx* c) {
-  void* ptrs[] = {c->S0, c->S1, c->SG, c->H, c->Gh, c->D, c->E, c->twx, c->twy, c->twz, c->cdn, c->cup, c->crate,
+  void* ptrs[] = {c->tabz, c->tabp, c->S0, c->S1, c->H, c->Gh, c->D, c->E, c->twx, c->twy, c->twz, c->cdn, c->cup, c->crate,
                   c->collfac, c->scal, c->partial, c->hist, c->rec_scratch, c->spec_col, c->spec_out, c->maxbits,
                   c->pairs, c->io};
   for (void* q : ptrs) if (q) cudaFree(q);
@@ -170,7 +172,8 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   const int F = d.F, M = d.M;
   cudaError_t e = cudaSuccess;
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
-  A(dalloc(&c->S0, F * d.PS)); A(dalloc(&c->S1, F * d.PS)); A(dalloc(&c->SG, F * d.PS));
+  A(dalloc(&c->S0, F * d.PS)); A(dalloc(&c->S1, F * d.PS));
+  A(dalloc(&c->tabz, (size_t)6 * d.Kz)); A(dalloc(&c->tabp, (size_t)2 * d.Ky * d.Kx));
   A(dalloc(&c->H, F * d.PH)); A(dalloc(&c->Gh, F * d.PH));
   A(dalloc(&c->D, (size_t)2 * (F + 2) * d.PD)); A(dalloc(&c->E, F * d.PE));
   A(dalloc(&c->cdn, (size_t)M + 1)); A(dalloc(&c->cup, (size_t)M + 1)); A(dalloc(&c->crate, (size_t)M + 1));
@@ -262,25 +265,27 @@ static int make_hybrid(gandalf_ctx* c, const cd* S) {
   return GANDALF_OK;
 }
 
-// bracket terms of the state whose hybrid copy is in H  ->  SG (spectral, masked): N+-, R_m
+// bracket terms of the state whose hybrid copy is in H  ->  Gh (hybrid: z real, (kx,ky) spectral and masked): N+-, R_m
 static int rhs_pipeline(gandalf_ctx* c, bool want_cfl) {
   const Dims& d = c->d;
-  if (!c->p.nonlinear) {
-    GD_CUDA(c, cudaMemsetAsync(c->SG, 0, d.F * d.PS * sizeof(cd), c->st));
-    if (want_cfl) {   // Eq. 16 still needs max|grad Phi|: run P1/P2 on the Elsasser part only is not worth a
-                      // special path -- evaluate the full pipeline and discard the brackets.
-    } else {
-      return GANDALF_OK;
-    }
-  }
+  if (!c->p.nonlinear && !want_cfl) return GANDALF_OK;
+  // nonlinear == 0 with the CFL dt: Eq. 16 still needs max|grad Phi|, so P1/P2 run and the brackets are discarded
   if (want_cfl) GD_CUDA(c, timed(c, -1, 1, [&] { return launch_zero_u64(c->maxbits, c->st); }));
   GD_CUDA(c, timed(c, KC_YINV, 1, [&] { return launch_yinv(d, c->H, c->D, c->twy, c->st); }));
   GD_CUDA(c, timed(c, KC_XPASS, 1, [&] {
     return launch_xpass(d, c->D, c->E, c->twx, c->cdn, c->cup, want_cfl ? c->maxbits : nullptr, c->st, false);
   }));
   if (!c->p.nonlinear) return GANDALF_OK;
-  GD_CUDA(c, timed(c, KC_YFWD, 1, [&] { return launch_yfwd(d, c->E, c->Gh, c->twy, c->st); }));
-  GD_CUDA(c, timed(c, KC_ZFWD, 1, [&] { return launch_zfft(d, -1, c->Gh, c->SG, c->twz, d.F, c->st); }));
+  GD_CUDA(c, timed(c, KC_YFWD, d.M > 0 ? 2 : 1, [&] { return launch_yfwd(d, c->E, c->Gh, c->twy, c->st); }));
+  return GANDALF_OK;
+}
+
+// P4: forward z transform of Gh + stage update (mode 0/1/2) + inverse z transform into the hybrid copy (if wanted)
+static int stage_update(gandalf_ctx* c, int mode, const cd* Wn, const cd* Ws, cd* Wout, bool want_hybrid) {
+  GD_CUDA(c, timed(c, KC_ZSTEP, 1, [&] {
+    return launch_zstep(c->d, mode, c->p.if_variant, c->p.g_sign, c->p.nonlinear ? c->Gh : nullptr, Wn, Ws, Wout,
+                        want_hybrid ? c->H : nullptr, c->scal, c->cdn, c->cup, c->collfac, c->tabz, c->tabp, c->twz, c->st);
+  }));
   return GANDALF_OK;
 }
 
@@ -360,9 +365,8 @@ int gandalf_rhs(gandalf_ctx* c, double* dw_hat, double* dg_hat, int on_device) {
   if (!c->H_valid) { rc = make_hybrid(c, c->S0); if (rc) return rc; c->H_valid = true; }
   rc = rhs_pipeline(c, false);
   if (rc) return rc;
-  GD_CUDA(c, timed(c, KC_UPDATE, 1, [&] {
-    return launch_update(c->d, c->ph, 0, c->SG, c->S0, c->S0, c->S1, c->scal, c->cdn, c->cup, c->collfac, c->st);
-  }));
+  rc = stage_update(c, 0, c->S0, c->S0, c->S1, false);
+  if (rc) return rc;
   return export_fields(c, c->S1, dw_hat, dg_hat, 0, on_device);
 }
 
@@ -376,6 +380,7 @@ int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
   const bool adaptive = !(dt > 0.0);
   const double cfl_dxy = c->p.cfl * std::fmin(c->p.Lx / d.nx, c->p.Ly / d.ny);
   if (!c->H_valid) { rc = make_hybrid(c, c->S0); if (rc) return rc; c->H_valid = true; }
+  const bool need_h = c->p.nonlinear || adaptive;
   for (int i = 0; i < nsteps; ++i) {
     // Alg. 2 l.3-6: RHS at t_n (its x-pass also yields max|grad Phi| for Eq. 16), half-step predictor
     rc = rhs_pipeline(c, adaptive);
@@ -383,28 +388,28 @@ int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
     GD_CUDA(c, timed(c, -1, 1, [&] {
       return launch_prepare_dt(adaptive ? 0.0 : dt, cfl_dxy, c->maxbits, c->scal, c->crate, c->collfac, d.M, c->st);
     }));
-    GD_CUDA(c, timed(c, KC_UPDATE, 1, [&] {
-      return launch_update(d, c->ph, 1, c->SG, c->S0, c->S0, c->S1, c->scal, c->cdn, c->cup, c->collfac, c->st);
-    }));
+    GD_CUDA(c, timed(c, -1, 1, [&] { return launch_tables(d, c->ph, c->scal, c->tabz, c->tabp, c->st); }));
+    rc = stage_update(c, 1, c->S0, c->S0, c->S1, c->p.nonlinear);
+    if (rc) return rc;
     // Alg. 2 l.7-9: midpoint RHS
-    if (c->p.nonlinear) { rc = make_hybrid(c, c->S1); if (rc) return rc; }
     rc = rhs_pipeline(c, false);
     if (rc) return rc;
-    // Alg. 2 l.10-14: full step + dissipation (in place on S0)
-    GD_CUDA(c, timed(c, KC_UPDATE, 1, [&] {
-      return launch_update(d, c->ph, 2, c->SG, c->S0, c->S1, c->S0, c->scal, c->cdn, c->cup, c->collfac, c->st);
-    }));
-    if (c->npairs)
+    // Alg. 2 l.10-14: full step + dissipation (in place on S0: each mode reads only its own S0 entry)
+    rc = stage_update(c, 2, c->S0, c->S1, c->S0, need_h);
+    if (rc) return rc;
+    if (c->npairs) {
       GD_CUDA(c, timed(c, -1, 1, [&] {
         return launch_forcing(d, c->S0, c->pairs, c->npairs, c->force_amp, c->p.seed, c->step, c->scal, c->st);
       }));
+      // the forcing touches w+- only: refresh the hybrid copy of those two fields
+      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, +1, c->S0, c->H, c->twz, 2, c->st); }));
+    }
     GD_CUDA(c, timed(c, -1, 2, [&] {
       return launch_energy(d, c->S0, c->partial, kEnergyBlocks, c->hist + (size_t)c->step * 7, c->scal, 1, c->st);
     }));
     c->step += 1;
-    if (c->p.nonlinear || adaptive) { rc = make_hybrid(c, c->S0); if (rc) return rc; }
   }
-  c->H_valid = true;
+  c->H_valid = need_h;
   return GANDALF_OK;
 }
 

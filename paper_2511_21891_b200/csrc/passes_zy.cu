@@ -57,6 +57,154 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zfft(Dims d, const cd* __restr
   }
 }
 
+// P4.  Fused forward z transform + stage update + inverse z transform: one lane group per (field f, (ky,kx) column).
+//   1. R^(kz) = (1/N) FFT_z of the bracket term Gh[f] (N+-, R_m), kz part of Eq. 20 (only retained kz are used)
+//   2. mode 0: out = RHS (N+-, H_m);  mode 1: half-step predictor (Eq. 15, Alg. 1 l.3-4);  mode 2: full-step corrector
+//      (Alg. 1 l.8-9) followed by the exponential dissipation factors (Eq. 17-19, Alg. 2 l.12-14).
+//      H_m = R_m + s i kz [ g_m - dn_m g_{m-1} - up_m g_{m+1} ]  (Eq. 6) reads the stage state Ws of the neighbours.
+//   3. the new state goes to Wout (compact) and, through an inverse z transform of the same registers, to the hybrid
+//      copy Hout that the next RHS evaluation consumes -- the spectral bracket terms never reach HBM.
+// Tables (k_tables, once per step): tabz[cz] = {cos th/2, sin th/2, cos th, sin th, fz, fzg}, th = kz vA dt;
+// tabp[col] = {fperp, fperp_g}: the separable factors of exp(-(eta P_perp + eta_z P_z) dt).
+// Work items are ordered with f fastest so that the CTAs that read g_{m-1}, g_m, g_{m+1} of the same columns run together.
+template <int NZ> struct ZStepGeom {
+  using G = FftGeom<NZ>;
+  static constexpr int GROUPS = GD_Z_THREADS / G::T;         // columns per CTA
+  static constexpr int KZ = 2 * (NZ / 3) + 1;                // retained kz (== Dims::Kz)
+  static constexpr int LD = GROUPS + 1;                      // padded row of the [kz][column] tile
+  static constexpr int XCH = GROUPS * (G::BUF + 1);          // FFT exchange buffers (alias the tile)
+  static constexpr int REGION = XCH > KZ * LD ? XCH : KZ * LD;
+  static constexpr size_t SMEM = ((size_t)REGION + FftTw<NZ>::COUNT) * sizeof(cd);
+};
+template <int NZ>
+__global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if_variant, double skz_sign, const cd* __restrict__ Gh,
+                                                      const cd* __restrict__ Wn, const cd* __restrict__ Ws, cd* __restrict__ Wout,
+                                                      cd* __restrict__ Hout, const double* __restrict__ scal,
+                                                      const double* __restrict__ cdn, const double* __restrict__ cup,
+                                                      const double* __restrict__ collfac, const double* __restrict__ tabz,
+                                                      const double* __restrict__ tabp, const cd* __restrict__ tw) {
+  using G = FftGeom<NZ>;
+  using Z = ZStepGeom<NZ>;
+  constexpr int T = G::T, E = G::E;
+  constexpr int GROUPS = Z::GROUPS, KZ = Z::KZ, LD = Z::LD;
+  extern __shared__ cd smem[];
+  const int grp = threadIdx.x / T, t = threadIdx.x % T;
+  cd* tile = smem + FftTw<NZ>::COUNT;                          // [KZ][LD], aliases the exchange buffers
+  cd* buf = tile + (size_t)grp * (G::BUF + 1);
+  fft_load_table<NZ>(smem, tw);
+  const cd* tws = smem;
+  const int plane = d.Ky * d.Kx;
+  const int f = blockIdx.x % d.F, cb = blockIdx.x / d.F;
+  const int col0 = cb * GROUPS;
+  const int col = col0 + grp;
+  const bool active = col < plane;
+  const int colc = active ? col : 0;
+  // 1. forward z transform of the bracket term, retained kz -> tile (scaled by 1/N)
+  if (Gh != nullptr) {
+    cd v[E];
+    const cd* src = Gh + (size_t)f * d.PH + colc;
+#pragma unroll
+    for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * plane) : cmake(0.0, 0.0);
+    fft_lanes<NZ, -1>(v, t, buf, tws);
+    __syncthreads();                                           // every group is done with its exchange buffer
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+      const int cz = fft2c(t + T * q, NZ, NZ / 3, KZ);
+      if (cz >= 0) tile[cz * LD + grp] = cscale(v[q], d.inv_n);
+    }
+  } else {
+    for (int e = threadIdx.x; e < KZ * LD; e += GD_Z_THREADS) tile[e] = cmake(0.0, 0.0);
+  }
+  __syncthreads();
+  // 2. pointwise stage update on the tile: thread <-> (kz, column), columns fastest (row-contiguous global accesses);
+  //    the loads of UB modes are issued together
+  {
+    const double dt = scal[SC_DT];
+    const double c = (mode == 1) ? 0.5 * dt : dt;
+    const int m = f - 2;
+    const bool lo = f > 2, hi = f + 1 < d.F;
+    const double dn = f >= 2 ? cdn[m] : 0.0, up = f >= 2 ? cup[m] : 0.0;
+    const double cf = (mode == 2 && f >= 2) ? collfac[m] : 1.0;
+    const int ncolv = min(GROUPS, plane - col0);
+    constexpr int NEL = KZ * GROUPS, UB = 4;
+    for (int e0 = threadIdx.x; e0 < NEL; e0 += UB * GD_Z_THREADS) {
+      cd a0[UB], a1[UB], a2[UB], a3[UB];
+      bool ok[UB];
+#pragma unroll
+      for (int u = 0; u < UB; ++u) {
+        const int e = e0 + u * GD_Z_THREADS;
+        const int cz = e / GROUPS, cl = e % GROUPS;
+        ok[u] = e < NEL && cl < ncolv;
+        const size_t idx = ok[u] ? (size_t)cz * plane + col0 + cl : 0;
+        a0[u] = a1[u] = a2[u] = a3[u] = cmake(0.0, 0.0);
+        if (mode != 0 || f >= 2) {
+          if (f < 2) a0[u] = ldg_cd(Wn + (size_t)f * d.PS + idx);
+          else {
+            a0[u] = ldg_cd(Ws + (size_t)f * d.PS + idx);
+            if (lo) a1[u] = ldg_cd(Ws + (size_t)(f - 1) * d.PS + idx);
+            if (hi) a2[u] = ldg_cd(Ws + (size_t)(f + 1) * d.PS + idx);
+            a3[u] = (Ws == Wn || mode == 0) ? a0[u] : ldg_cd(Wn + (size_t)f * d.PS + idx);
+          }
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < UB; ++u) {
+        if (!ok[u]) continue;
+        const int e = e0 + u * GD_Z_THREADS;
+        const int cz = e / GROUPS, cl = e % GROUPS;
+        const size_t idx = (size_t)cz * plane + col0 + cl;
+        const cd Gv = tile[cz * LD + cl];
+        const double* tz = tabz + 6 * cz;
+        cd out;
+        if (f < 2) {
+          if (mode == 0) out = Gv;
+          else {
+            const double sg = f == 0 ? 1.0 : -1.0;
+            const cd ph_half = cmake(tz[0], sg * tz[1]), ph_full = cmake(tz[2], sg * tz[3]);
+            const cd wn = a0[u];
+            const cd N = cscale(Gv, c);
+            if (mode == 1) {
+              const cd inner = (if_variant == 0) ? wn + cmul(ph_half, N) : wn + N;     // Eq. 15 / standard IF midpoint
+              out = cmul(ph_half, inner);
+            } else {
+              if (if_variant == 0) out = cmul(ph_full, wn + cmul(ph_full, N));
+              else out = cmul(ph_full, wn) + cmul(ph_half, N);
+              out = cscale(out, tabp[2 * (col0 + cl)] * tz[4]);
+            }
+          }
+        } else {
+          const double skz = skz_sign * d.kz0 * c2n(cz, NZ / 3, KZ);
+          const cd lin = cmake(a0[u].x - dn * a1[u].x - up * a2[u].x, a0[u].y - dn * a1[u].y - up * a2[u].y);
+          const cd Hm = cmake(Gv.x - skz * lin.y, Gv.y + skz * lin.x);                 // + i s kz lin  (Eq. 6)
+          if (mode == 0) out = Hm;
+          else {
+            out = cmake(a3[u].x + c * Hm.x, a3[u].y + c * Hm.y);
+            if (mode == 2) out = cscale(out, cf * tabp[2 * (col0 + cl) + 1] * tz[5]);
+          }
+        }
+        st_cd(Wout + (size_t)f * d.PS + idx, out);
+        tile[cz * LD + cl] = out;
+      }
+    }
+  }
+  if (Hout == nullptr) return;
+  __syncthreads();
+  // 3. inverse z transform of the new stage state (zero-padded) -> hybrid copy
+  cd v[E];
+#pragma unroll
+  for (int q = 0; q < E; ++q) {
+    const int cz = fft2c(t + T * q, NZ, NZ / 3, KZ);
+    v[q] = (cz >= 0 && active) ? tile[cz * LD + grp] : cmake(0.0, 0.0);
+  }
+  __syncthreads();                                             // tile read by every group: the exchange may overwrite it
+  fft_lanes<NZ, +1>(v, t, buf, tws);
+  if (active) {
+    cd* dst = Hout + (size_t)f * d.PH + colc;
+#pragma unroll
+    for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * plane, v[q]);
+  }
+}
+
 // Geometry of the y passes: GD_Y_THREADS lanes per CTA = GROUPS lane groups = GROUPS adjacent columns of ONE array,
 // so a CTA covers GROUPS*16 B contiguous per row (256 B at ny = 256: strided row segments narrower than that lose
 // HBM efficiency, profiles/r01_stride_microbench.md) and two CTAs fit on an SM (<= 128 registers per lane).
@@ -308,6 +456,16 @@ cudaError_t launch_zfft(const Dims& d, int dir, const cd* in, cd* out, const cd*
   GD_DISPATCH(d.nz, ZCASE)
   return cudaGetLastError();
 }
+cudaError_t launch_zstep(const Dims& d, int mode, int if_variant, int g_sign, const cd* Gh, const cd* Wn, const cd* Ws, cd* Wout, cd* Hout,
+                         const double* scal, const double* cdn, const double* cup, const double* collfac, const double* tabz,
+                         const double* tabp, const cd* tw, cudaStream_t st) {
+  const long long ncols = (long long)d.Ky * d.Kx;
+#define ZSCASE(NN)                                                                                               \
+  k_zstep<NN><<<fft_blocks<NN>(ncols) * d.F, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, mode, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, \
+                                                                             Hout, scal, cdn, cup, collfac, tabz, tabp, tw);
+  GD_DISPATCH(d.nz, ZSCASE)
+  return cudaGetLastError();
+}
 cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStream_t st) {
 #define YICASE(NN)                                                                                         \
   {                                                                                                        \
@@ -340,6 +498,8 @@ cudaError_t prepare_passes_zy(int ny, int nz) {
     cudaError_t e = cudaFuncSetAttribute(k_zfft<NN, +1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<NN>());  \
     if (e != cudaSuccess) return e;                                                                                        \
     e = cudaFuncSetAttribute(k_zfft<NN, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<NN>());             \
+    if (e != cudaSuccess) return e;                                                                                        \
+    e = cudaFuncSetAttribute(k_zstep<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);           \
     if (e != cudaSuccess) return e;                                                                                        \
   }
   GD_DISPATCH(nz, ZPCASE)

@@ -1,5 +1,5 @@
-// pointwise.cu -- everything that is diagonal in k: the stage update (integrating factor, Hermite
-// streaming stencil, RK2, dissipation), boundary pack/unpack with projection, forcing, CFL dt,
+// pointwise.cu -- the small kernels that are diagonal in k: per-step factor tables of the stage update (the update
+// itself is fused with the z transforms, passes_zy.cu), boundary pack/unpack with projection, forcing, CFL dt,
 // and the energy / shell-spectrum reductions.
 #include "common.cuh"
 
@@ -10,78 +10,31 @@ __device__ __forceinline__ double rate_perp_shape(const PhysParams& p, double k2
   return p.eta_normalized ? ipow_d(k2 / p.k2max_perp, p.r) : ipow_d(k2, p.r);     // Eq. 18 / Eq. 17
 }
 
-// mode: 0 = RHS only (out = N+-, H_m), 1 = predictor (Eq. 15, Alg. 1 l.3-4), 2 = corrector + dissipation
-// (Alg. 1 l.8-9, Alg. 2 l.12-14).  G: spectral bracket terms (N+-, R_m).  Wn: state at t_n.  Ws: the state
-// the RHS was evaluated at (supplies the streaming stencil of Eq. 6).  One thread per retained mode.
-__global__ void __launch_bounds__(256) k_update(Dims d, PhysParams p, int mode, const cd* __restrict__ G,
-                                                const cd* __restrict__ Wn, const cd* __restrict__ Ws, cd* __restrict__ Wout,
-                                                const double* __restrict__ scal, const double* __restrict__ cdn,
-                                                const double* __restrict__ cup, const double* __restrict__ collfac) {
-  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= d.PS) return;
-  const int cx = (int)(idx % d.Kx);
-  const int cy = (int)((idx / d.Kx) % d.Ky);
-  const int cz = (int)(idx / ((size_t)d.Kx * d.Ky));
-  const double kx = d.kx0 * cx, ky = d.ky0 * c2n(cy, d.hy3, d.Ky), kz = d.kz0 * c2n(cz, d.hz3, d.Kz);
+// Per-step factor tables of the fused stage update (k_zstep, passes_zy.cu), separable in (kz) and (kx,ky):
+//   tabz[cz] = { cos th/2, sin th/2, cos th, sin th, fz, fzg },  th = kz vA dt (Eq. 13),
+//              fz = exp(-eta_z (kz^2/kz,max^2)^r_z dt), fzg = fz if eta_g > 0 else 1
+//   tabp[cy][cx] = { exp(-eta P_perp dt), exp(-eta_g P_perp dt) },  P_perp of Eq. 17 / Eq. 18
+__global__ void __launch_bounds__(256) k_tables(Dims d, PhysParams p, const double* __restrict__ scal, double* __restrict__ tabz,
+                                                double* __restrict__ tabp) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const double dt = scal[SC_DT];
-  const double c = (mode == 1) ? 0.5 * dt : dt;
-  double fw = 1.0, fgk = 1.0;
-  if (mode == 2) {
-    const double k2 = kx * kx + ky * ky;
-    const double shape = rate_perp_shape(p, k2);
-    const double zshape = (p.eta_z > 0.0) ? ipow_d(kz * kz / p.kz2max, p.r_z) : 0.0;
-    fw = exp(-(p.eta * shape + p.eta_z * zshape) * dt);
-    if (p.eta_g > 0.0) fgk = exp(-(p.eta_g * shape + p.eta_z * zshape) * dt);
+  const int plane = d.Ky * d.Kx;
+  if (i < plane) {
+    const int cx = i % d.Kx, cy = i / d.Kx;
+    const double kx = d.kx0 * cx, ky = d.ky0 * c2n(cy, d.hy3, d.Ky);
+    const double shape = rate_perp_shape(p, kx * kx + ky * ky);
+    tabp[2 * i] = exp(-(p.eta * shape) * dt);
+    tabp[2 * i + 1] = (p.eta_g > 0.0) ? exp(-(p.eta_g * shape) * dt) : 1.0;
   }
-  // Elsasser vorticities
-  if (mode == 0) {
-    Wout[idx] = G[idx];
-    Wout[d.PS + idx] = G[d.PS + idx];
-  } else {
+  if (i < d.Kz) {
+    const double kz = d.kz0 * c2n(i, d.hz3, d.Kz);
     const double th = kz * p.vA * dt;
     double s1, c1, sh, ch;
     sincos(th, &s1, &c1);
     sincos(0.5 * th, &sh, &ch);
-#pragma unroll
-    for (int f = 0; f < 2; ++f) {
-      const double sg = f == 0 ? 1.0 : -1.0;
-      const cd wn = Wn[(size_t)f * d.PS + idx];
-      const cd N = cscale(G[(size_t)f * d.PS + idx], c);
-      const cd ph_half = cmake(ch, sg * sh), ph_full = cmake(c1, sg * s1);
-      cd w;
-      if (mode == 1) {
-        const cd inner = (p.if_variant == 0) ? wn + cmul(ph_half, N) : wn + N;
-        w = cmul(ph_half, inner);
-      } else {
-        if (p.if_variant == 0) w = cmul(ph_full, wn + cmul(ph_full, N));
-        else w = cmul(ph_full, wn) + cmul(ph_half, N);
-        w = cscale(w, fw);
-      }
-      Wout[(size_t)f * d.PS + idx] = w;
-    }
-  }
-  // Hermite moments: H_m = R_m + s i kz [ g_m - dn_m g_{m-1} - up_m g_{m+1} ]   (Eq. 6)
-  const int M = d.M;
-  if (M > 0) {
-    const double skz = (double)p.g_sign * kz;
-    cd gm1 = cmake(0.0, 0.0);
-    cd g0 = Ws[(size_t)2 * d.PS + idx];
-    for (int m = 0; m < M; ++m) {
-      const cd gp1 = (m + 1 < M) ? Ws[(size_t)(3 + m) * d.PS + idx] : cmake(0.0, 0.0);
-      const double dn = cdn[m], up = cup[m];
-      const cd lin = cmake(g0.x - dn * gm1.x - up * gp1.x, g0.y - dn * gm1.y - up * gp1.y);
-      const cd R = G[(size_t)(2 + m) * d.PS + idx];
-      const cd Hm = cmake(R.x - skz * lin.y, R.y + skz * lin.x);      // + i skz lin
-      cd out;
-      if (mode == 0) out = Hm;
-      else {
-        const cd gn = (Ws == Wn) ? g0 : Wn[(size_t)(2 + m) * d.PS + idx];
-        out = cmake(gn.x + c * Hm.x, gn.y + c * Hm.y);
-        if (mode == 2) out = cscale(out, fgk * collfac[m]);
-      }
-      Wout[(size_t)(2 + m) * d.PS + idx] = out;
-      gm1 = g0; g0 = gp1;
-    }
+    const double fz = (p.eta_z > 0.0) ? exp(-(p.eta_z * ipow_d(kz * kz / p.kz2max, p.r_z)) * dt) : 1.0;
+    double* tz = tabz + 6 * i;
+    tz[0] = ch; tz[1] = sh; tz[2] = c1; tz[3] = s1; tz[4] = fz; tz[5] = (p.eta_g > 0.0) ? fz : 1.0;
   }
 }
 
@@ -293,9 +246,9 @@ __global__ void __launch_bounds__(256) k_spec_bins(Dims d, const double* __restr
 // ---- launchers ---------------------------------------------------------------------------------------------
 static inline int nblk(size_t n, int b) { return (int)((n + b - 1) / b); }
 
-cudaError_t launch_update(const Dims& d, const PhysParams& p, int mode, const cd* G, const cd* Wn, const cd* Ws, cd* Wout,
-                          const double* scal, const double* cdn, const double* cup, const double* collfac, cudaStream_t st) {
-  k_update<<<nblk(d.PS, 256), 256, 0, st>>>(d, p, mode, G, Wn, Ws, Wout, scal, cdn, cup, collfac);
+cudaError_t launch_tables(const Dims& d, const PhysParams& p, const double* scal, double* tabz, double* tabp, cudaStream_t st) {
+  const int n = d.Ky * d.Kx > d.Kz ? d.Ky * d.Kx : d.Kz;
+  k_tables<<<nblk((size_t)n, 256), 256, 0, st>>>(d, p, scal, tabz, tabp);
   return cudaGetLastError();
 }
 cudaError_t launch_prepare_dt(double fixed_dt, double cfl_dxy, const unsigned long long* maxbits, double* scal,

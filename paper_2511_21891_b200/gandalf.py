@@ -14,7 +14,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libgandalf.so")
 
 OK, ERR_INVALID, ERR_CUDA, ERR_NONFINITE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4
-KERNEL_CLASSES = ("z_inverse", "y_inverse_P1", "x_pass_P2", "y_forward_P3", "z_forward", "update")
+KERNEL_CLASSES = ("z_inverse", "y_inverse_P1", "x_pass_P2", "y_forward_P3", "z_step_P4")
 
 
 class GandalfParams(C.Structure):
