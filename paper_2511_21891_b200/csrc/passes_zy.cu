@@ -255,9 +255,11 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
     for (int r = threadIdx.x; r < d.Ky; r += GD_Y_THREADS)
       bulk_g2s(tile + (size_t)r * LD, H + (size_t)s * d.PH + ((size_t)z * d.Ky + r) * d.Kx + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
   };
+  constexpr int HY3 = NY / 3, KY = 2 * HY3 + 1;   // == d.hy3, d.Ky: compile-time so that the per-q mode tests fold
   int item = blockIdx.x;
   if (item < nitems) issue(item);
   unsigned phase = 0;
+  const double kyt = d.ky0 * t, kyT = d.ky0 * T, kyN = d.ky0 * NY;
   while (item < nitems) {
     const int cb = item % ncb, sz = item / ncb;
     const int z = sz % d.nz, s = sz / d.nz;
@@ -266,6 +268,13 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
     const double kx = d.kx0 * cx;
     const int cxa = active ? cx : 0;
     const int rounds = (s < 2) ? 4 : 2;
+    // D[a][line block][kx][xl], line = z*ny + y, slot (line % xl) ^ (kx % xl): the lanes of a group fill whole aligned
+    // runs of one block row.  Offsets of element q: off0 + q*ostr when a block row holds at most T lines.
+    const int lineb = z * NY + t;
+    const bool lin_off = d.xl <= T;
+    const int sw = cxa & (d.xl - 1);
+    const int off0 = ((((lineb >> d.xlsh) * d.Kx + cxa)) << d.xlsh) + ((lineb & (d.xl - 1)) ^ sw);
+    const int ostr = T * d.Kx;
     mbar_wait(&bar, phase);
     phase ^= 1u;
     item += gridDim.x;
@@ -276,8 +285,8 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
       cd v[E];
 #pragma unroll
       for (int q = 0; q < E; ++q) {
-        const int cy = fft2c(t + T * q, NY, d.hy3, d.Ky);
-        v[q] = (active && cy >= 0) ? tile[(size_t)cy * LD + grp] : cmake(0.0, 0.0);
+        const int cy = fft2c(t + T * q, NY, HY3, KY);
+        v[q] = (active && cy >= 0) ? tile[cy * LD + grp] : cmake(0.0, 0.0);
       }
       if (r == rounds - 1) {
         __syncthreads();                         // last read of the tile by every lane
@@ -286,7 +295,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
       if (pot || which) {
 #pragma unroll
         for (int q = 0; q < E; ++q) {
-          const double ky = d.ky0 * fft2n(t + T * q, NY);
+          const double ky = kyt + kyT * q - ((t + T * q) >= NY / 2 ? kyN : 0.0);
           double f = 1.0;
           if (pot) { const double k2 = kx * kx + ky * ky; f = k2 > 0.0 ? -1.0 / k2 : 0.0; }
           if (which) v[q] = cscale(mul_i(v[q]), f * ky);
@@ -295,14 +304,16 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
       }
       fft_lanes_split<NY, +1>(v, t, xbuf, tws);
       if (active) {
-        // D[a][line block][kx][xl], line = z*ny + y, slot (line % xl) ^ (kx % xl): the lanes of a group fill whole
-        // aligned runs of one block row
         cd* dst = D + (size_t)a * d.PD;
-        const int sw = cxa & (d.xl - 1);
+        if (lin_off) {
 #pragma unroll
-        for (int q = 0; q < E; ++q) {
-          const int line = z * NY + t + T * q;
-          st_cd(dst + (((size_t)(line >> d.xlsh) * d.Kx + cxa) << d.xlsh) + ((line & (d.xl - 1)) ^ sw), v[q]);
+          for (int q = 0; q < E; ++q) st_cd(dst + (off0 + q * ostr), v[q]);
+        } else {
+#pragma unroll
+          for (int q = 0; q < E; ++q) {
+            const int line = lineb + T * q;
+            st_cd(dst + (((line >> d.xlsh) * d.Kx + cxa) << d.xlsh) + ((line & (d.xl - 1)) ^ sw), v[q]);
+          }
         }
       }
     }
@@ -389,6 +400,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd(Dims d, const cd* __re
   using G = FftGeom<NY>;
   using YF = YFwdGeom<NY>;
   constexpr int T = G::T, E = G::E, LD = YF::LD;
+  constexpr int HY3 = NY / 3, KY = 2 * HY3 + 1;   // == d.hy3, d.Ky
   extern __shared__ cd smem[];
   __shared__ unsigned long long bar;
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
@@ -418,17 +430,17 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd(Dims d, const cd* __re
     phase ^= 1u;
     cd v[E];
 #pragma unroll
-    for (int q = 0; q < E; ++q) v[q] = active ? tile[(size_t)(t + T * q) * LD + grp] : cmake(0.0, 0.0);
+    for (int q = 0; q < E; ++q) v[q] = active ? tile[(t + T * q) * LD + grp] : cmake(0.0, 0.0);
     __syncthreads();                             // tile consumed by every lane
     item += gridDim.x;
     if (item < nitems) issue(item);              // prefetch: overlaps the transform and the stores below
     fft_lanes_split<NY, -1>(v, t, xbuf, tws);
     if (active) {
-      cd* dst = Gh + (size_t)a * d.PH + (size_t)z * d.Ky * d.Kx + cx;
+      cd* dst = Gh + (size_t)a * d.PH + (size_t)z * KY * d.Kx + cx;
 #pragma unroll
       for (int q = 0; q < E; ++q) {
-        const int cy = fft2c(t + T * q, NY, d.hy3, d.Ky);
-        if (cy >= 0) st_cd(dst + (size_t)cy * d.Kx, v[q]);
+        const int cy = fft2c(t + T * q, NY, HY3, KY);
+        if (cy >= 0) st_cd(dst + cy * d.Kx, v[q]);
       }
     }
   }
