@@ -1,9 +1,9 @@
 // pass_x.cu -- P2, the fused row pass of the RHS pipeline (one lane group per (y,z) line).
 //
 // For every source field f in {xi+, xi-, w+, w-, g_m} the pass reads the two half-lines
-// f~(kx; y,z) and (df/dy)~(kx; y,z) that P1 wrote (retained kx only), forms
-//     Z(kx) = i kx f~(kx) + i (df/dy)~(kx)          for kx >= 0       (Eq. 10)
-//     Z(-kx) = conj(i kx f~) + i conj((df/dy)~)                        (Hermitian completion)
+// U = kx f~ + (df/dy)~ and V = (df/dy)~ - kx f~ of (kx; y,z) that P1 wrote (retained kx only), forms
+//     Z(kx) = i kx f~(kx) + i (df/dy)~(kx) = i U(kx)        for kx >= 0       (Eq. 10)
+//     Z(-kx) = conj(i kx f~) + i conj((df/dy)~) = i conj(V(kx))               (Hermitian completion)
 // and ONE complex inverse FFT of length nx returns (df/dx) + i (df/dy) on the real line -- the
 // derivative fields exist only in registers.  Bracket products:
 //     A = {xi+,w-} + {xi-,w+},  B = {xi+,xi-}                          (Eq. 1)
@@ -151,27 +151,23 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
           e0 = 2 + M - 1; e1 = -1;
         }
       } else {
-        // wait for the staged tiles and pack conj(Z), Z = Fx + i Fy, Fx = i kx f  (Hermitian completion for kx < 0)
+        // wait for the staged tiles and pack conj(Z), Z = Fx + i Fy.  P1 delivers U = kx f~ + (df/dy)~ and
+        // V = (df/dy)~ - kx f~, so that Z(kx) = i U(kx) and Z(-kx) = i conj(V(kx)) (Hermitian completion) need no arithmetic
         const int sc = kind % X::NST;
         mbar_wait(&s_full[sc], (unsigned)((kind / X::NST) & 1));
-        const cd* pf = stages + (size_t)sc * X::STAGE;            // element n of this line: pf[n * LD + (grp ^ (n & (LD-1)))]
-        const cd* pfy = pf + (size_t)KX * X::LD;
+        const cd* pU = stages + (size_t)sc * X::STAGE;            // element n of this line: pU[n * LD + (grp ^ (n & (LD-1)))]
+        const cd* pV = pU + (size_t)KX * X::LD;
 #pragma unroll
         for (int q = 0; q < E; ++q) {
           const int n = t + T * q;
           cd z = cmake(0.0, 0.0);
           if (T * q <= HX3 && n <= HX3) {                       // first test is compile-time per q
-            const int o = n * X::LD + (grp ^ (n & (X::LD - 1)));
-            cd f = pf[o], fy = pfy[o];
-            if (n == 0) { f.y = 0.0; fy.y = 0.0; }
-            const double kx = d.kx0 * n;
-            z = cmake(-kx * f.y - fy.y, -(kx * f.x + fy.x));    // conj( i kx f + i fy )
+            const cd u = pU[n * X::LD + (grp ^ (n & (X::LD - 1)))];
+            z = cmake(n == 0 ? 0.0 : -u.y, -u.x);               // conj(i U); the kx = 0 entry of a real line is real
           } else if (T * q + T - 1 >= NX - HX3 && n >= NX - HX3) {
             const int c = NX - n;
-            const int o = c * X::LD + (grp ^ (c & (X::LD - 1)));
-            const cd f = pf[o], fy = pfy[o];
-            const double kx = d.kx0 * c;
-            z = cmake(-kx * f.y + fy.y, kx * f.x - fy.x);       // conj( conj(i kx f) + i conj(fy) )
+            const cd w = pV[c * X::LD + (grp ^ (c & (X::LD - 1)))];
+            z = cmake(w.y, -w.x);                               // conj(i conj(V)) = -i V
           }
           v[q] = z;
         }

@@ -219,9 +219,10 @@ template <int NY> struct YGeom {
 };
 
 // P1.  Persistent CTAs over the work items (source field s, z, block of GROUPS columns).  Sources: s = 0,1 -> w+, w-;
-// s = 2+m -> g_m.  D array order: 0/1 xi+ , 2/3 xi- , 4/5 w+ , 6/7 w- , 8+2m / 9+2m g_m  (even: f, odd: df/dy).
+// s = 2+m -> g_m.  D array order: 0/1 xi+ , 2/3 xi- , 4/5 w+ , 6/7 w- , 8+2m / 9+2m g_m  (even: U = kx f + df/dy,
+// odd: V = df/dy - kx f: the two combinations the x-pass packs, pass_x.cu).
 // The [Ky][GROUPS] tile of retained modes arrives by one bulk async copy per row (TMA engine) into a padded
-// shared-memory tile; every lane group then reads its column once per output array (f, then i ky f, Eq. 10; the
+// shared-memory tile; every lane group then reads its column once per output array (U, then V, Eq. 10; the
 // Elsasser sources first give xi = -w/kperp^2, then w) -- no second copy of the column in registers.
 // The next item's tile is requested as soon as the last read of the current one is done.
 template <int NY> struct YInvGeom {
@@ -259,7 +260,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
   int item = blockIdx.x;
   if (item < nitems) issue(item);
   unsigned phase = 0;
-  const double kyt = d.ky0 * t, kyT = d.ky0 * T, kyN = d.ky0 * NY;
+  const double kyt = d.ky0 * t, kyT = d.ky0 * T;
   while (item < nitems) {
     const int cb = item % ncb, sz = item / ncb;
     const int z = sz % d.nz, s = sz / d.nz;
@@ -280,7 +281,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
     item += gridDim.x;
     for (int r = 0; r < rounds; ++r) {
       const bool pot = (s < 2) && (r < 2);       // rounds 0,1 of an Elsasser source: the potential xi = -w/kperp^2
-      const int which = r & 1;                   // 0: f, 1: df/dy
+      const int which = r & 1;                   // 0: U, 1: V
       const int a = (s < 2 ? (pot ? 2 * s : 4 + 2 * s) : 8 + 2 * (s - 2)) + which;
       cd v[E];
 #pragma unroll
@@ -292,14 +293,17 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
         __syncthreads();                         // last read of the tile by every lane
         if (item < nitems) issue(item);          // prefetch: overlaps the transform and the stores below
       }
-      if (pot || which) {
+      // which = 0: U = kx f + df/dy -> multiplier (kx + i ky);  which = 1: V = df/dy - kx f -> multiplier (i ky - kx)  (Eq. 10)
+      {
+        const double skx = which ? -kx : kx;
 #pragma unroll
         for (int q = 0; q < E; ++q) {
-          const double ky = kyt + kyT * q - ((t + T * q) >= NY / 2 ? kyN : 0.0);
-          double f = 1.0;
-          if (pot) { const double k2 = kx * kx + ky * ky; f = k2 > 0.0 ? -1.0 / k2 : 0.0; }
-          if (which) v[q] = cscale(mul_i(v[q]), f * ky);
-          else v[q] = cscale(v[q], f);
+          if (T * q <= HY3 || T * q + T - 1 >= NY - HY3) {      // compile-time: some lane of this q holds a retained ky
+            const double ky = fma(kyT, (double)(q < E / 2 ? q : q - E), kyt);     // ky0 * signed mode number of t + T q
+            double ar = skx, ai = ky;
+            if (pot) { const double k2 = kx * kx + ky * ky; const double f = k2 > 0.0 ? -1.0 / k2 : 0.0; ar *= f; ai *= f; }   // xi = -w/kperp^2
+            v[q] = cmake(ar * v[q].x - ai * v[q].y, ar * v[q].y + ai * v[q].x);
+          }
         }
       }
       fft_lanes_split<NY, +1>(v, t, xbuf, tws);
