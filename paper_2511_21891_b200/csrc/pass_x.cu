@@ -180,25 +180,30 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
     fft_lanes<NX, -1>(v, t, buf, tws);
 
     if (fwd) {
-      // separate the two real lines' spectra by Hermitian symmetry, keep kx <= nx/3, store
+      // separate the two real lines' spectra by Hermitian symmetry, keep kx <= nx/3, store.  The partner X[nx - c] of
+      // c = t + T q sits in lane (T - t) % T of the same group at register E-1-q (lane 0: its own register (E - q) % E),
+      // so it comes by warp shuffles -- no shared-memory round trip.
       fwd = false;
-#pragma unroll
-      for (int q = 0; q < E; ++q) buf[G::pad(t + T * q)] = v[q];
-      __syncwarp();
-      if (active) {
+      {
         cd* p0 = Eo + (size_t)e0 * d.PE + base;
         cd* p1 = Eo + (size_t)(e1 < 0 ? e0 : e1) * d.PE + base;
+        const int partner = (T - t) & (T - 1);
 #pragma unroll
         for (int q = 0; q < E; ++q) {
-          const int c = t + T * q;
-          if (T * q <= HX3 && c <= HX3) {
-            const cd z1 = buf[G::pad(c)], z2 = buf[G::pad((NX - c) & (NX - 1))];
-            st_cd(p0 + c, cmake(0.5 * (z1.x + z2.x), 0.5 * (z1.y - z2.y)));
-            if (e1 >= 0) st_cd(p1 + c, cmake(0.5 * (z1.y + z2.y), -0.5 * (z1.x - z2.x)));
+          if (T * q <= HX3) {                                   // compile-time: some lane of this q holds a retained kx
+            const int c = t + T * q;
+            cd z2;
+            z2.x = __shfl_sync(0xffffffffu, v[E - 1 - q].x, partner, T);
+            z2.y = __shfl_sync(0xffffffffu, v[E - 1 - q].y, partner, T);
+            if (t == 0) z2 = v[(E - q) & (E - 1)];
+            const cd z1 = v[q];
+            if (active && c <= HX3) {
+              st_cd(p0 + c, cmake(0.5 * (z1.x + z2.x), 0.5 * (z1.y - z2.y)));
+              if (e1 >= 0) st_cd(p1 + c, cmake(0.5 * (z1.y + z2.y), -0.5 * (z1.x - z2.x)));
+            }
           }
         }
       }
-      __syncwarp();
       continue;
     }
 
