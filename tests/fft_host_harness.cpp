@@ -30,6 +30,41 @@ template <int N, int DIR> static void run(const double* in, double* out) {
     for (int q = 0; q < E; ++q) { out[2 * (t + T * q)] = v[t][q].x; out[2 * (t + T * q) + 1] = v[t][q].y; }
 }
 
+// Same transform with the split (real parts, then imaginary parts) exchange through a buffer of doubles.
+template <int N, int s> static void exchange_split(cd (*v)[FftPlan<N>::E], double* buf) {
+  constexpr int T = FftGeom<N>::T;
+  for (int t = 0; t < T; ++t) fft_stage_scatter_c<N, s, 0>(v[t], t, buf);
+  for (int t = 0; t < T; ++t) fft_gather_c<N, 0>(v[t], t, buf);
+  for (int t = 0; t < T; ++t) fft_stage_scatter_c<N, s, 1>(v[t], t, buf);
+  for (int t = 0; t < T; ++t) fft_gather_c<N, 1>(v[t], t, buf);
+}
+template <int N, int DIR> static void run_split(const double* in, double* out) {
+  using G = FftGeom<N>;
+  constexpr int T = G::T, E = G::E;
+  std::vector<cd> tw(FftTw<N>::COUNT + 1);
+  fft_fill_stage_table<N>(tw.data());
+  std::vector<double> buf(G::BUF + 2);
+  cd v[T][E];
+  for (int t = 0; t < T; ++t)
+    for (int q = 0; q < E; ++q) v[t][q] = cmake(in[2 * (t + T * q)], in[2 * (t + T * q) + 1]);
+  for (int t = 0; t < T; ++t) fft_stage_compute<N, DIR, 0>(v[t], t, tw.data());
+  if constexpr (G::S > 1) {
+    exchange_split<N, 0>(v, buf.data());
+    for (int t = 0; t < T; ++t) fft_stage_compute<N, DIR, 1>(v[t], t, tw.data());
+  }
+  if constexpr (G::S > 2) {
+    exchange_split<N, 1>(v, buf.data());
+    for (int t = 0; t < T; ++t) fft_stage_compute<N, DIR, 2>(v[t], t, tw.data());
+  }
+  for (int t = 0; t < T; ++t)
+    for (int q = 0; q < E; ++q) { out[2 * (t + T * q)] = v[t][q].x; out[2 * (t + T * q) + 1] = v[t][q].y; }
+}
+extern "C" int host_fft_split(int n, int dir, const double* in, double* out) {
+#define SCASE(NN) case NN: if (dir < 0) run_split<NN, -1>(in, out); else run_split<NN, +1>(in, out); return 0;
+  switch (n) { SCASE(2) SCASE(4) SCASE(8) SCASE(16) SCASE(32) SCASE(64) SCASE(128) SCASE(256) SCASE(512) }
+  return -1;
+}
+
 extern "C" int host_fft(int n, int dir, const double* in, double* out) {
 #define CASE(NN) case NN: if (dir < 0) run<NN, -1>(in, out); else run<NN, +1>(in, out); return 0;
   switch (n) { CASE(2) CASE(4) CASE(8) CASE(16) CASE(32) CASE(64) CASE(128) CASE(256) CASE(512) }

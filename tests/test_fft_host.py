@@ -24,9 +24,10 @@ def test_lane_group_fft_matches_numpy(lib, n):
     x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
     out = np.empty_like(x)
     P = C.POINTER(C.c_double)
-    for d, ref in ((-1, np.fft.fft(x)), (+1, np.fft.ifft(x) * n)):
-        assert lib.host_fft(n, d, x.view(np.float64).ctypes.data_as(P), out.view(np.float64).ctypes.data_as(P)) == 0
-        assert np.linalg.norm(out - ref) <= 1e-14 * np.sqrt(n) * np.linalg.norm(ref)
+    for fn in (lib.host_fft, lib.host_fft_split):       # complex exchange / split (re, im) exchange
+        for d, ref in ((-1, np.fft.fft(x)), (+1, np.fft.ifft(x) * n)):
+            assert fn(n, d, x.view(np.float64).ctypes.data_as(P), out.view(np.float64).ctypes.data_as(P)) == 0
+            assert np.linalg.norm(out - ref) <= 1e-14 * np.sqrt(n) * np.linalg.norm(ref)
 
 
 @pytest.mark.parametrize("n", [32, 64, 128, 256, 512])

@@ -1,0 +1,106 @@
+"""-m gpu: parity at BASELINE config 4(a)'s FULL size (256x256x128, M=32) in the launch configuration bench.py times.
+
+The oracle cannot run the full grid in seconds, but the workload's initial state is band limited (|n_perp| <= 4,
+|n_z| <= 2), and a dealiased pseudo-spectral bracket of band-limited fields is the truncated
+convolution sum -- independent of the grid it is evaluated on as long as every product
+mode is retained.  So the oracle on a 64x64x32 grid, fed the SAME Fourier coefficients, must reproduce every
+non-zero coefficient of the full-size GPU result (RHS, and one complete Algorithm-2 step: two nested RHS evaluations
+reach |n| <= 16, |n_z| <= 8, still inside the small grid's retained band), and the GPU result must vanish elsewhere.
+The k_perp-normalised dissipation of Eq. 18 depends on the grid's k_max, so it is switched off for this comparison
+(collisions, Eq. 19, stay on).  A second test checks the ideal invariants at full size on a dense
+spectrum, a property that holds at any size.
+"""
+import numpy as np
+import pytest
+
+from paper_2511_21891_b200.workloads import config4a, rel_l2
+from paper_2511_21891_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+BIG = (256, 256, 128)
+SMALL = (64, 64, 32)
+
+
+def _idx(n_small, n_big):
+    """FFT-order indices of the small grid's modes inside the big grid (Nyquist excluded)."""
+    m = synth.mode_numbers(n_small)
+    keep = np.abs(m) < n_small // 2
+    return np.nonzero(keep)[0], (m[keep] % n_big)
+
+
+def _to_small(a_big):
+    """(fields, nz, ny, hx) big half-spectrum -> the same coefficients on the small grid."""
+    nxs, nys, nzs = SMALL
+    out = np.zeros((a_big.shape[0], nzs, nys, nxs // 2 + 1), dtype=np.complex128)
+    zs, zb = _idx(nzs, BIG[2])
+    ys, yb = _idx(nys, BIG[1])
+    kx = nxs // 2          # kx = 0 .. nxs/2-1
+    out[np.ix_(np.arange(a_big.shape[0]), zs, ys, np.arange(kx))] = a_big[np.ix_(np.arange(a_big.shape[0]), zb, yb, np.arange(kx))]
+    return out
+
+
+def _split(a_big):
+    """(coefficients inside the small band as a small-grid array, largest |coefficient| outside it)."""
+    inside = _to_small(a_big)
+    rest = a_big.copy()
+    zs, zb = _idx(SMALL[2], BIG[2])
+    ys, yb = _idx(SMALL[1], BIG[1])
+    rest[np.ix_(np.arange(a_big.shape[0]), zb, yb, np.arange(SMALL[0] // 2))] = 0.0
+    return inside, float(np.abs(rest).max())
+
+
+def test_config4a_full_size_rhs_and_step_vs_small_grid_oracle():
+    from oracle import Oracle
+    from paper_2511_21891_b200.gandalf import Gandalf
+    prm, z, gm, run = config4a()
+    assert run["shape"] == BIG and prm["M"] == 32
+    prm = dict(prm, eta=0.0, eta_g=0.0)            # Eq. 18 is grid dependent (k_perp,max); Eq. 19 stays
+    g = Gandalf(*BIG, **prm)
+    o = Oracle(*SMALL, **prm)
+    g.set_state(z, gm)
+    o.set_state(_to_small(z), _to_small(gm))
+    # one RHS evaluation (tolerance: north_star's 1e-12 relative L2 per RHS evaluation)
+    dw_g, dg_g = g.rhs()
+    dw_o, dg_o = o.rhs()
+    dw_in, dw_out = _split(dw_g)
+    dg_in, dg_out = _split(dg_g)
+    assert rel_l2(dw_in, dw_o) <= 1e-12, rel_l2(dw_in, dw_o)
+    assert rel_l2(dg_in, dg_o) <= 1e-12, rel_l2(dg_in, dg_o)
+    assert dw_out <= 1e-13 * np.abs(dw_o).max() and dg_out <= 1e-13 * np.abs(dg_o).max()
+    del dw_g, dg_g
+    # one complete step (two nested RHS evaluations): state and energy record
+    g.step(run["dt"], 1)
+    o.step(run["dt"], 1)
+    zg, gg = g.get_state()
+    zo, go = o.get_state()
+    z_in, z_out = _split(zg)
+    g_in, g_out = _split(gg)
+    assert rel_l2(z_in, zo) <= 1e-10, rel_l2(z_in, zo)
+    assert rel_l2(g_in, go) <= 1e-10, rel_l2(g_in, go)
+    assert z_out <= 1e-13 * np.abs(zo).max() and g_out <= 1e-13 * np.abs(go).max()
+    hg, ho = g.energy_history(), o.energy_history()
+    assert np.abs(hg[:, 1:] - ho[:, 1:]).max() <= 1e-9 * np.abs(ho[:, 1:]).max()
+
+
+def test_full_size_ideal_invariants_dense_state():
+    """Re sum conj(xi+-) N+- = 0 separately and Re sum_m conj(g_m) H_m = 0 (absorbing closure, no dissipation) on a
+    dense decaying spectrum at 256x256x128 with M=4 (half-plane sums with weights 1 at kx=0, 2 elsewhere)."""
+    from paper_2511_21891_b200.gandalf import Gandalf
+    nx, ny, nz = BIG
+    M = 4
+    g = Gandalf(nx, ny, nz, M=M)
+    z = synth.dense_random(nx, ny, nz, 2, seed=77, decay=4.0)
+    gm = synth.dense_random(nx, ny, nz, M, seed=78, decay=4.0)
+    g.set_state(z, gm)
+    zp, gp = g.get_state()                         # the projected state the RHS is evaluated at
+    dw, dg = g.rhs()
+    w = np.full(nx // 2 + 1, 2.0)
+    w[0] = 1.0
+    for a in range(2):
+        num = float(np.sum(w * (np.conj(zp[a]) * dw[a]).real))
+        den = float(np.sum(w * np.abs(zp[a]) * np.abs(dw[a])))
+        assert abs(num) <= 1e-12 * den, (a, num, den)
+    num = float(np.sum(w * (np.conj(gp) * dg).real))
+    den = float(np.sum(w * np.abs(gp) * np.abs(dg)))
+    assert abs(num) <= 1e-12 * den, (num, den)
