@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
     const double dt = scal[SC_DT];
     const double c = (mode == 1) ? 0.5 * dt : dt;
     const int m = f - 2;
-    const bool lo = f > 2, hi = f + 1 < d.F;
+    const bool lo = f > 2, hi = f + 1 < d.F, same = (Ws == Wn || mode == 0);
     const double dn = f >= 2 ? cdn[m] : 0.0, up = f >= 2 ? cup[m] : 0.0;
     const double cf = (mode == 2 && f >= 2) ? collfac[m] : 1.0;
     const int ncolv = min(GROUPS, plane - col0);
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
             a0[u] = ldg_cd(Ws + (size_t)f * d.PS + idx);
             if (lo) a1[u] = ldg_cd(Ws + (size_t)(f - 1) * d.PS + idx);
             if (hi) a2[u] = ldg_cd(Ws + (size_t)(f + 1) * d.PS + idx);
-            a3[u] = (Ws == Wn || mode == 0) ? a0[u] : ldg_cd(Wn + (size_t)f * d.PS + idx);
+            if (!same) a3[u] = ldg_cd(Wn + (size_t)f * d.PS + idx);   // (no copy of a0 here: it would wait on the load)
           }
         }
       }
@@ -178,7 +178,8 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
           const cd Hm = cmake(Gv.x - skz * lin.y, Gv.y + skz * lin.x);                 // + i s kz lin  (Eq. 6)
           if (mode == 0) out = Hm;
           else {
-            out = cmake(a3[u].x + c * Hm.x, a3[u].y + c * Hm.y);
+            const cd gn = same ? a0[u] : a3[u];
+            out = cmake(gn.x + c * Hm.x, gn.y + c * Hm.y);
             if (mode == 2) out = cscale(out, cf * tabp[2 * (col0 + cl) + 1] * tz[5]);
           }
         }
