@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
     const double dn = f >= 2 ? cdn[m] : 0.0, up = f >= 2 ? cup[m] : 0.0;
     const double cf = (mode == 2 && f >= 2) ? collfac[m] : 1.0;
     const int ncolv = min(GROUPS, plane - col0);
-    constexpr int NEL = KZ * GROUPS, UB = 4;
+    constexpr int NEL = KZ * GROUPS, UB = 6;
     for (int e0 = threadIdx.x; e0 < NEL; e0 += UB * GD_Z_THREADS) {
       cd a0[UB], a1[UB], a2[UB], a3[UB];
       bool ok[UB];
