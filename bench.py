@@ -273,8 +273,16 @@ def main():
             kern[name] = {"avg_ms": avg_ms, "launches": n, "share_of_step": avg_ms * n / ms,
                           "algorithmic_gb": per_launch[name] / 1e9, "achieved_gbs": per_launch[name] / 1e9 / (avg_ms * 1e-3)}
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"])
+    traffic = None          # dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)
+    try:
+        for ln in open(os.path.join(ROOT, "profiles", "r01_traffic.csv")).read().splitlines()[1:]:
+            w, k, b = ln.split(",")
+            if w == args.workload and k == dom:
+                traffic = float(b)
+    except Exception:
+        pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["achieved_gbs"], "peak": peak_gbs, "peak_source": peak_src,
-                "unit": "GB/s", "frac": kern[dom]["achieved_gbs"] / peak_gbs, "traffic": None,
+                "unit": "GB/s", "frac": kern[dom]["achieved_gbs"] / peak_gbs, "traffic": traffic,
                 "algorithmic_bytes_per_launch": per_launch[dom],
                 "step": {"algorithmic_gb_4pass_design": step_bytes / 1e9, "achieved_gbs": step_bytes / 1e9 / (ms * 1e-3 / args.steps),
                          "frac_of_measured_peak": step_bytes / 1e9 / (ms * 1e-3 / args.steps) / peak_gbs,
