@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   cd* stages = smem + FftTw<NX>::COUNT + (size_t)X::GROUPS * X::LB;   // NST x [2][KX][LD]: f~ and (df/dy)~ tiles, [kx][line]
   __shared__ unsigned s_tmem_base;
   __shared__ unsigned long long s_full[X::NST], s_empty[X::NST];
-  const int warp = threadIdx.x >> 5;
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);     // warp-uniform for the compiler (uniform registers)
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int i = 0; i < X::NST; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], X::WARPS); }
@@ -90,7 +90,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const cd* tws = smem;
   // this warp's TMEM window: lane quarter warp%4, column slot warp/4
-  const unsigned tm = s_tmem_base + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * X::TM_SLOT);
+  const unsigned tm = __shfl_sync(0xffffffffu, s_tmem_base, 0) + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * X::TM_SLOT);
   const bool active = line < nlines;
   const size_t base = (size_t)(active ? line : 0) * KX;       // (z*ny + y)*Kx  (output arrays E, kx fastest)
   const int M = d.M;
