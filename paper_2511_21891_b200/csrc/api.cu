@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <string>
 #include <vector>
@@ -158,7 +159,11 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   d.Kx = d.hx3 + 1; d.Ky = 2 * d.hy3 + 1; d.Kz = 2 * d.hz3 + 1;
   d.kx0 = 2.0 * kPi / p->Lx; d.ky0 = 2.0 * kPi / p->Ly; d.kz0 = 2.0 * kPi / p->Lz;
   d.inv_n = 1.0 / ((double)p->nx * p->ny * p->nz);
-  d.PS = (size_t)d.Kz * d.Ky * d.Kx; d.PH = (size_t)d.nz * d.Ky * d.Kx; d.PE = (size_t)d.nz * d.ny * d.Kx;
+  // Row strides.  E rows are padded to 128 B multiples (P3 then reads whole DRAM granules: 0.52 -> 0.50 ms at 4a); the same
+  // padding on the hybrid arrays was measured SLOWER (P3 0.60, P4 1.05 ms: their lane-per-row stores then camp on few L2
+  // slices), so H and Gh keep unpadded rows.
+  d.Kxp = d.Kx; d.Kxe = (d.Kx + 7) / 8 * 8;
+  d.PS = (size_t)d.Kz * d.Ky * d.Kx; d.PH = (size_t)d.nz * d.Ky * d.Kxp; d.PE = (size_t)d.nz * d.ny * d.Kxe;
   d.xl = xpass_lines_per_cta(d.nx);
   d.xlsh = 0; while ((1 << d.xlsh) < d.xl) ++d.xlsh;
   { const size_t nlb = ((size_t)d.ny * d.nz + d.xl - 1) / d.xl; d.PD = nlb * d.Kx * (size_t)d.xl; }

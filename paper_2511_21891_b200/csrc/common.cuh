@@ -3,10 +3,10 @@
 // Storage spaces (all complex fp64, kx fastest; "c" indices run over RETAINED modes only, i.e.
 // the modes Eq. 20 keeps: 3|n| <= N):
 //   compact  S[f][cz][cy][cx]   Kz*Ky*Kx per field   fully spectral state / RHS
-//   hybrid   H[f][z ][cy][cx]   nz*Ky*Kx per field   z in real space, (kx,ky) spectral
+//   hybrid   H[f][z ][cy][cx]   nz*Ky*Kxp per field  z in real space, (kx,ky) spectral; row stride Kxp (= Kx, see api.cu)
 //   xy-real  D[a][lb][cx][xl]   y,z real, kx spectral (retained kx only); line = z*ny+y = lb*xl + li, stored at slot
 //                               li ^ (cx % xl): the tile of an x-pass CTA (xl lines) is one contiguous run (P1 -> P2)
-//            E[a][z ][y ][cx]   nz*ny*Kx per array   same space, kx fastest (P2 -> P3)
+//            E[a][z ][y ][cx]   nz*ny*Kxe per array  same space, kx fastest, rows padded to Kxe = 8*ceil(Kx/8) (P2 -> P3)
 // cx = 0..Kx-1 is n_x = cx; cy = 0..Ky-1 is n_y = cy (cy <= hy3) or cy-Ky (negative modes);
 // cz likewise.  The zeroed third is never stored or transformed.
 #pragma once
@@ -17,6 +17,7 @@ struct Dims {
   int nx, ny, nz, M, F;
   int hx;                 // nx/2+1 (boundary layout)
   int Kx, Ky, Kz;         // retained counts
+  int Kxp, Kxe;           // row strides (>= Kx) of the hybrid arrays H, Gh and of E
   int hx3, hy3, hz3;      // floor(N/3)
   double kx0, ky0, kz0;   // 2 pi / L
   double inv_n;           // 1/(nx ny nz)

@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   // this warp's TMEM window: lane quarter warp%4, column slot warp/4
   const unsigned tm = __shfl_sync(0xffffffffu, s_tmem_base, 0) + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * X::TM_SLOT);
   const bool active = line < nlines;
-  const size_t base = (size_t)(active ? line : 0) * KX;       // (z*ny + y)*Kx  (output arrays E, kx fastest)
+  const size_t base = (size_t)(active ? line : 0) * d.Kxe;    // (z*ny + y)*Kxp  (output arrays E, kx fastest, padded rows)
   const int M = d.M;
   cd v[E];
   double Qp[E], Ra[E];             // Hermite sliding window; Qp doubles as the {xi+,w-} accumulator of the Elsasser part

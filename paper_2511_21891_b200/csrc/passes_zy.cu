@@ -27,6 +27,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zfft(Dims d, const cd* __restr
   const bool active = gid < ncols;
   const int plane = d.Ky * d.Kx;
   const int f = active ? gid / plane : 0, rem = active ? gid % plane : 0;
+  const int planeH = d.Ky * d.Kxp, remH = (rem / d.Kx) * d.Kxp + rem % d.Kx;       // hybrid rows are padded to Kxp
   cd v[E];
   if (DIR > 0) {   // compact -> hybrid
     const cd* src = in + (size_t)f * d.PS + rem;
@@ -37,14 +38,14 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zfft(Dims d, const cd* __restr
     }
     fft_lanes<NZ, +1>(v, t, buf, tws);
     if (active) {
-      cd* dst = out + (size_t)f * d.PH + rem;
+      cd* dst = out + (size_t)f * d.PH + remH;
 #pragma unroll
-      for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * plane, v[q]);
+      for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * planeH, v[q]);
     }
   } else {         // hybrid -> compact, masked, scaled by 1/(nx ny nz)
-    const cd* src = in + (size_t)f * d.PH + rem;
+    const cd* src = in + (size_t)f * d.PH + remH;
 #pragma unroll
-    for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * plane) : cmake(0.0, 0.0);
+    for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * planeH) : cmake(0.0, 0.0);
     fft_lanes<NZ, -1>(v, t, buf, tws);
     if (active) {
       cd* dst = out + (size_t)f * d.PS + rem;
@@ -99,12 +100,13 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
   const int col = col0 + grp;
   const bool active = col < plane;
   const int colc = active ? col : 0;
+  const int planeH = d.Ky * d.Kxp, colH = (colc / d.Kx) * d.Kxp + colc % d.Kx;   // hybrid rows are padded to Kxp
   // 1. forward z transform of the bracket term, retained kz -> tile (scaled by 1/N)
   if (Gh != nullptr) {
     cd v[E];
-    const cd* src = Gh + (size_t)f * d.PH + colc;
+    const cd* src = Gh + (size_t)f * d.PH + colH;
 #pragma unroll
-    for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * plane) : cmake(0.0, 0.0);
+    for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * planeH) : cmake(0.0, 0.0);
     fft_lanes<NZ, -1>(v, t, buf, tws);
     __syncthreads();                                           // every group is done with its exchange buffer
 #pragma unroll
@@ -200,9 +202,9 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
   __syncthreads();                                             // tile read by every group: the exchange may overwrite it
   fft_lanes<NZ, +1>(v, t, buf, tws);
   if (active) {
-    cd* dst = Hout + (size_t)f * d.PH + colc;
+    cd* dst = Hout + (size_t)f * d.PH + colH;
 #pragma unroll
-    for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * plane, v[q]);
+    for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * planeH, v[q]);
   }
 }
 
@@ -255,7 +257,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
     const int ncol = min(Y::GROUPS, d.Kx - cx0);
     if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(d.Ky * ncol * sizeof(cd)));
     for (int r = threadIdx.x; r < d.Ky; r += GD_Y_THREADS)
-      bulk_g2s(tile + (size_t)r * LD, H + (size_t)s * d.PH + ((size_t)z * d.Ky + r) * d.Kx + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
+      bulk_g2s(tile + (size_t)r * LD, H + (size_t)s * d.PH + ((size_t)z * d.Ky + r) * d.Kxp + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
   };
   constexpr int HY3 = NY / 3, KY = 2 * HY3 + 1;   // == d.hy3, d.Ky: compile-time so that the per-q mode tests fold
   int item = blockIdx.x;
@@ -356,7 +358,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd_pair(Dims d, const cd*
   fft_load_table<NY>(smem, tw);                  // ends with __syncthreads()
   if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(NY * ncol * 2 * sizeof(cd)));
   for (int r = threadIdx.x; r < NY; r += GD_Y_THREADS) {
-    const cd* src = Ein + ((size_t)z * NY + r) * d.Kx + cx0;
+    const cd* src = Ein + ((size_t)z * NY + r) * d.Kxe + cx0;
     bulk_g2s(tile + (size_t)r * LD, src, (unsigned)(ncol * sizeof(cd)), &bar);
     bulk_g2s(tile + (size_t)r * LD + HG, src + d.PE, (unsigned)(ncol * sizeof(cd)), &bar);
   }
@@ -375,7 +377,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd_pair(Dims d, const cd*
   const cd* sib = tile + (size_t)(grp ^ HG) * Y::YBUF;
   const double kx = d.kx0 * cx;
   if (active) {
-    cd* dst = Gh + (size_t)which * d.PH + (size_t)z * d.Ky * d.Kx + cx;
+    cd* dst = Gh + (size_t)which * d.PH + (size_t)z * d.Ky * d.Kxp + cx;
 #pragma unroll
     for (int q = 0; q < E; ++q) {
       const int cy = fft2c(t + T * q, NY, d.hy3, d.Ky);
@@ -384,7 +386,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd_pair(Dims d, const cd*
         const cd A = which ? o : v[q], B = which ? v[q] : o;
         const double ky = d.ky0 * fft2n(t + T * q, NY);
         const double hk2 = (which ? 0.5 : -0.5) * (kx * kx + ky * ky);
-        st_cd(dst + (size_t)cy * d.Kx, cmake(-0.5 * A.x + hk2 * B.x, -0.5 * A.y + hk2 * B.y));
+        st_cd(dst + (size_t)cy * d.Kxp, cmake(-0.5 * A.x + hk2 * B.x, -0.5 * A.y + hk2 * B.y));
       }
     }
   }
@@ -421,7 +423,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd(Dims d, const cd* __re
     const int ncol = min(Y::GROUPS, d.Kx - cx0);
     if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(NY * ncol * sizeof(cd)));
     for (int r = threadIdx.x; r < NY; r += GD_Y_THREADS)
-      bulk_g2s(tile + (size_t)r * LD, Ein + (size_t)a * d.PE + ((size_t)z * NY + r) * d.Kx + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
+      bulk_g2s(tile + (size_t)r * LD, Ein + (size_t)a * d.PE + ((size_t)z * NY + r) * d.Kxe + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
   };
   int item = blockIdx.x;
   if (item < nitems) issue(item);
@@ -441,11 +443,11 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd(Dims d, const cd* __re
     if (item < nitems) issue(item);              // prefetch: overlaps the transform and the stores below
     fft_lanes_split<NY, -1>(v, t, xbuf, tws);
     if (active) {
-      cd* dst = Gh + (size_t)a * d.PH + (size_t)z * KY * d.Kx + cx;
+      cd* dst = Gh + (size_t)a * d.PH + (size_t)z * KY * d.Kxp + cx;
 #pragma unroll
       for (int q = 0; q < E; ++q) {
         const int cy = fft2c(t + T * q, NY, HY3, KY);
-        if (cy >= 0) st_cd(dst + cy * d.Kx, v[q]);
+        if (cy >= 0) st_cd(dst + cy * d.Kxp, v[q]);
       }
     }
   }
