@@ -208,14 +208,15 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
   }
 }
 
-// Geometry of the y passes: GD_Y_THREADS lanes per CTA = GROUPS lane groups = GROUPS adjacent columns of ONE array,
+// Geometry of the y passes: THREADS lanes per CTA = GROUPS lane groups = GROUPS adjacent columns of ONE array,
 // so a CTA covers GROUPS*16 B contiguous per row (256 B at ny = 256: strided row segments narrower than that lose
 // HBM efficiency, profiles/r01_stride_microbench.md) and two CTAs fit on an SM (<= 128 registers per lane).
-#define GD_Y_THREADS 256
 template <int NY> struct YGeom {
   using G = FftGeom<NY>;
   static constexpr int T = G::T, E = G::E;
-  static constexpr int GROUPS = GD_Y_THREADS / T;            // columns per CTA
+  static constexpr int THREADS = (T >= 32) ? 512 : 256;      // ny = 512 (one warp per transform): 16 warps so that a tile is still 16 columns wide
+  static constexpr int CTAS = (THREADS == 512) ? 1 : 2;      // resident CTAs per SM
+  static constexpr int GROUPS = THREADS / T;                 // columns per CTA
   static constexpr int YBUF = (G::S > 1 ? G::BUF : NY) + 1;  // per-group buffer (FFT exchange; A/B hand-over in P3)
   static constexpr int REGION = (GROUPS * YBUF > NY * (GROUPS + 1)) ? GROUPS * YBUF : NY * (GROUPS + 1);   // also holds a padded [NY][GROUPS] tile
   static constexpr size_t SMEM = ((size_t)REGION + FftTw<NY>::COUNT) * sizeof(cd);
@@ -236,7 +237,7 @@ template <int NY> struct YInvGeom {
   static constexpr size_t SMEM = ((size_t)FftTw<NY>::COUNT + (size_t)KYMAX * LD) * sizeof(cd) + (size_t)Y::GROUPS * XB * sizeof(double);
 };
 template <int NY>
-__global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __restrict__ H, cd* __restrict__ D,
+__global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Dims d, const cd* __restrict__ H, cd* __restrict__ D,
                                                         const cd* __restrict__ tw, int ncb, int nitems) {
   using Y = YGeom<NY>;
   using G = FftGeom<NY>;
@@ -256,7 +257,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
     const int cx0 = cb * Y::GROUPS;
     const int ncol = min(Y::GROUPS, d.Kx - cx0);
     if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(d.Ky * ncol * sizeof(cd)));
-    for (int r = threadIdx.x; r < d.Ky; r += GD_Y_THREADS)
+    for (int r = threadIdx.x; r < d.Ky; r += Y::THREADS)
       bulk_g2s(tile + (size_t)r * LD, H + (size_t)s * d.PH + ((size_t)z * d.Ky + r) * d.Kxp + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
   };
   constexpr int HY3 = NY / 3, KY = 2 * HY3 + 1;   // == d.hy3, d.Ky: compile-time so that the per-q mode tests fold
@@ -336,7 +337,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yinv(Dims d, const cd* __re
 // columns, hand the results over through shared memory and form N+- = -1/2 A -+ 1/2 kperp^2 B  (Eq. 1 with
 // Eq. 11).  The FFT exchange buffers alias the tile once every lane holds its column.
 template <int NY>
-__global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
+__global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
                                                              const cd* __restrict__ tw, int ncb) {
   using Y = YGeom<NY>;
   using G = FftGeom<NY>;
@@ -357,7 +358,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd_pair(Dims d, const cd*
   if (threadIdx.x == 0) mbar_init(&bar, 1);
   fft_load_table<NY>(smem, tw);                  // ends with __syncthreads()
   if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(NY * ncol * 2 * sizeof(cd)));
-  for (int r = threadIdx.x; r < NY; r += GD_Y_THREADS) {
+  for (int r = threadIdx.x; r < NY; r += Y::THREADS) {
     const cd* src = Ein + ((size_t)z * NY + r) * d.Kxe + cx0;
     bulk_g2s(tile + (size_t)r * LD, src, (unsigned)(ncol * sizeof(cd)), &bar);
     bulk_g2s(tile + (size_t)r * LD + HG, src + d.PE, (unsigned)(ncol * sizeof(cd)), &bar);
@@ -401,7 +402,7 @@ template <int NY> struct YFwdGeom {
   static constexpr size_t SMEM = ((size_t)FftTw<NY>::COUNT + (size_t)NY * LD) * sizeof(cd) + (size_t)Y::GROUPS * XB * sizeof(double);
 };
 template <int NY>
-__global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
+__global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yfwd(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
                                                         const cd* __restrict__ tw, int ncb, int nitems) {
   using Y = YGeom<NY>;
   using G = FftGeom<NY>;
@@ -422,7 +423,7 @@ __global__ void __launch_bounds__(GD_Y_THREADS, 2) k_yfwd(Dims d, const cd* __re
     const int cx0 = cb * Y::GROUPS;
     const int ncol = min(Y::GROUPS, d.Kx - cx0);
     if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(NY * ncol * sizeof(cd)));
-    for (int r = threadIdx.x; r < NY; r += GD_Y_THREADS)
+    for (int r = threadIdx.x; r < NY; r += Y::THREADS)
       bulk_g2s(tile + (size_t)r * LD, Ein + (size_t)a * d.PE + ((size_t)z * NY + r) * d.Kxe + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
   };
   int item = blockIdx.x;
@@ -490,7 +491,7 @@ cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStr
   {                                                                                                        \
     const int ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;                                    \
     const int nitems = d.F * d.nz * ncb;                                                                   \
-    k_yinv<NN><<<nitems < 2 * g_num_sms ? nitems : 2 * g_num_sms, GD_Y_THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, nitems); \
+    k_yinv<NN><<<nitems < YGeom<NN>::CTAS * g_num_sms ? nitems : YGeom<NN>::CTAS * g_num_sms, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, nitems); \
   }
   GD_DISPATCH(d.ny, YICASE)
   return cudaGetLastError();
@@ -500,9 +501,9 @@ cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, cudaSt
   {                                                                                                        \
     constexpr int HG = YGeom<NN>::GROUPS / 2;                                                              \
     const int ncb2 = (d.Kx + HG - 1) / HG, ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;       \
-    k_yfwd_pair<NN><<<d.nz * ncb2, GD_Y_THREADS, YGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb2);               \
+    k_yfwd_pair<NN><<<d.nz * ncb2, YGeom<NN>::THREADS, YGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb2);               \
     const int nitems = d.M * d.nz * ncb;                                                                   \
-    if (d.M > 0) k_yfwd<NN><<<nitems < 2 * g_num_sms ? nitems : 2 * g_num_sms, GD_Y_THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, nitems); \
+    if (d.M > 0) k_yfwd<NN><<<nitems < YGeom<NN>::CTAS * g_num_sms ? nitems : YGeom<NN>::CTAS * g_num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, nitems); \
   }
   GD_DISPATCH(d.ny, YFCASE)
   return cudaGetLastError();

@@ -185,14 +185,16 @@ __global__ void __launch_bounds__(256) k_energy_partial(Dims d, const cd* __rest
     partial[(size_t)blockIdx.x * 5 + threadIdx.x] = v;
   }
 }
-// Final sum in fixed order.  advance != 0: t += dt, and the record {t, E_A, E+, E-, Ekin, Emag, Wg} goes to rec.
-__global__ void k_energy_final(const double* __restrict__ partial, int nblocks, double* __restrict__ rec, double* scal, int advance) {
+// Final sum in a fixed order (deterministic): warp k sums quantity k, lane l takes blocks l, l+32, ... then a shuffle tree.
+// advance != 0: t += dt, and the record {t, E_A, E+, E-, Ekin, Emag, Wg} goes to rec.
+__global__ void __launch_bounds__(160) k_energy_final(const double* __restrict__ partial, int nblocks, double* __restrict__ rec, double* scal, int advance) {
   __shared__ double sh[5];
-  if (threadIdx.x < 5) {
-    double v = 0.0;
-    for (int b = 0; b < nblocks; ++b) v += partial[(size_t)b * 5 + threadIdx.x];
-    sh[threadIdx.x] = v;
-  }
+  const int k = threadIdx.x >> 5, l = threadIdx.x & 31;
+  double v = 0.0;
+  for (int b = l; b < nblocks; b += 32) v += partial[(size_t)b * 5 + k];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  if (l == 0) sh[k] = v;
   __syncthreads();
   if (threadIdx.x == 0) {
     if (advance) { scal[SC_T] += scal[SC_DT]; scal[SC_LASTDT] = scal[SC_DT]; }
@@ -274,7 +276,7 @@ cudaError_t launch_forcing(const Dims& d, cd* S, const int* pairs, int npairs, d
 cudaError_t launch_energy(const Dims& d, const cd* S, double* partial, int nblocks, double* rec, double* scal, int advance,
                           cudaStream_t st) {
   k_energy_partial<<<nblocks, 256, 0, st>>>(d, S, partial);
-  k_energy_final<<<1, 32, 0, st>>>(partial, nblocks, rec, scal, advance);
+  k_energy_final<<<1, 160, 0, st>>>(partial, nblocks, rec, scal, advance);
   return cudaGetLastError();
 }
 cudaError_t launch_spectrum(const Dims& d, const cd* S, double* col, int nbins, int literal, double dk, double* out, cudaStream_t st) {
