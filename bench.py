@@ -63,6 +63,23 @@ def algorithmic_bytes(shape, M):
     return per_launch, step_4pass
 
 
+def max_over_ranks(x, world, device="cuda"):
+    """Replicas only (DESIGN.md "Multi-GPU"): the job's time is the slowest replica's.  No data-path collective exists;
+    this all-reduce(MAX) of one scalar is the only communication of the bench."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_steps_per_s(ms_max, steps, world):
+    """Every rank advances its own replica by `steps` steps in `ms_max` (max over ranks): weak scaling."""
+    return world * steps / (ms_max * 1e-3)
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -222,13 +239,10 @@ def main():
     launches = sim.launch_count() - n0
     ktimes = sim.kernel_times()
     sim.kernel_timing(False)
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world)
     hist = sim.energy_history()
     assert hist.shape[0] == args.warmup + args.steps and np.isfinite(hist).all()
-    steps_per_s = world * args.steps / (ms * 1e-3)
+    steps_per_s = whole_job_steps_per_s(ms, args.steps, world)
 
     # ---- end to end through the C ABI with HOST (pinned) buffers: H2D state, one step, D2H energies
     e2e = None
@@ -250,10 +264,7 @@ def main():
             en = sim.energy_history()       # device -> host read of the step's result (energy record)
         torch.cuda.synchronize()
         el = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([el], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            el = float(t.item())
+        el = max_over_ranks(el, world)
         e2e = {"value": 2 * world * args.e2e_steps / el, "unit": "RHS evals/s", "steps": args.e2e_steps,
                "h2d_bytes_per_step": int(z.nbytes + (g.nbytes if M else 0)), "d2h_bytes_per_step": int(en.nbytes),
                "what": "gandalf_set_state(host pinned) + gandalf_step(dt,1) + gandalf_energy_history(host) per step"}
