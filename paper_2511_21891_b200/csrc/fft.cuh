@@ -207,6 +207,35 @@ template <int N> GD_HD void fft_gather(cd (&v)[FftPlan<N>::E], int t, const cd* 
   for (int q = 0; q < G::E; ++q) v[q] = buf[G::pad(t + G::T * q)];
 }
 
+// Stage-1 compute with the first NREG stage twiddles of this lane held in registers (twr[i-1] = table entry of
+// input i; only for plans whose stage 1 has ONE butterfly per lane, so the twiddles depend on the lane alone):
+// fewer shared-memory reads per transform for kernels that run many transforms per lane.  DIR = -1 only.
+template <int N, int NREG> GD_HD void fft_stage1_compute_rt(cd (&v)[FftPlan<N>::E], int t, const cd* __restrict__ tws,
+                                                            const cd (&twr)[NREG]) {
+  using G = FftGeom<N>;
+  constexpr int R = G::template radix<1>();
+  constexpr int NS = G::template ns<1>();
+  static_assert(G::E / R == 1 && G::S == 2, "one stage-1 butterfly per lane");
+  cd x[R];
+#pragma unroll
+  for (int i = 0; i < R; ++i) x[i] = v[i];
+  const cd* tb = tws + FftTw<N>::template off<1>() + (t % NS);
+#pragma unroll
+  for (int i = 1; i < R; ++i) {
+    const cd w = (i - 1 < NREG) ? twr[(i - 1 < NREG) ? i - 1 : 0] : tb[(i - 1) * NS];
+    x[i] = cmul(x[i], w);
+  }
+  butterfly<R, -1>(x);
+#pragma unroll
+  for (int i = 0; i < R; ++i) v[i] = x[i];
+}
+template <int N, int NREG> GD_HD void fft_load_stage1_twiddles(cd (&twr)[NREG], int t, const cd* __restrict__ tws) {
+  using G = FftGeom<N>;
+  constexpr int NS = G::template ns<1>();
+#pragma unroll
+  for (int i = 0; i < NREG; ++i) twr[i] = tws[FftTw<N>::template off<1>() + i * NS + (t % NS)];
+}
+
 // Split exchange: the real parts cross the lanes first, then the imaginary parts, through a buffer of doubles
 // (FftGeom<N>::BUF entries of 8 bytes -- half the shared memory of the complex exchange; in place, because a lane's
 // .x registers can be overwritten by the gather while its .y registers still wait to be scattered).
@@ -258,6 +287,16 @@ template <int N, int DIR> __device__ __forceinline__ void fft_lanes(cd (&v)[FftP
     __syncwarp();
     fft_stage_compute<N, DIR, 2>(v, t, tws);
   }
+}
+// Forward transform with register-held stage-1 twiddles (see fft_stage1_compute_rt).
+template <int N, int NREG> __device__ __forceinline__ void fft_lanes_fwd_rt(cd (&v)[FftPlan<N>::E], int t, cd* buf,
+                                                                            const cd* __restrict__ tws, const cd (&twr)[NREG]) {
+  fft_stage_compute<N, -1, 0>(v, t, tws);
+  fft_stage_scatter<N, 0>(v, t, buf);
+  __syncwarp();
+  fft_gather<N>(v, t, buf);
+  __syncwarp();
+  fft_stage1_compute_rt<N, NREG>(v, t, tws, twr);
 }
 template <int N, int s> __device__ __forceinline__ void fft_exchange_split(cd (&v)[FftPlan<N>::E], int t, double* buf) {
   fft_stage_scatter_c<N, s, 0>(v, t, buf);

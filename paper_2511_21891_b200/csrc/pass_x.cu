@@ -15,6 +15,9 @@
 // (Eq. 16) rides on the Elsasser part.
 #include "common.cuh"
 
+#ifndef GD_X_NTWR
+#define GD_X_NTWR 8
+#endif
 template <int NX>
 struct XGeom {
   using G = FftGeom<NX>;
@@ -27,6 +30,8 @@ struct XGeom {
   static constexpr int LD = GROUPS;                         // row of a staged tile [kx][line]; line slot XOR-swizzled with kx
   static constexpr int STAGE = 2 * KXP * LD;                // one stage: the tiles of f~ and (df/dy)~ for all lines of the CTA
   static constexpr int NST = 3;                             // stages in flight (full/empty mbarrier ring)
+  // stage-1 twiddles held in registers (plans with one stage-1 butterfly per lane): fewer shared-memory reads per transform
+  static constexpr int NTWR = (G::S == 2 && E / FftPlan<NX>::R1 == 1) ? GD_X_NTWR : 0;
   static constexpr size_t SMEM = ((size_t)GROUPS * LB + (size_t)NST * STAGE + FftTw<NX>::COUNT) * sizeof(cd);
   // Tensor memory as a thread-private scratchpad (tcgen05.ld/st, shape 32x32b: lane i of a warp owns TMEM lane
   // 32*(warp%4)+i).  Per thread: 8 words per x-point for (Phi_x,Phi_y,Psi_x,Psi_y) and 2 words per x-point for the
@@ -123,6 +128,8 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   bool tail_done = (M == 0);
   int e0 = 0, e1 = 1;
   double gmax = 0.0;
+  cd twr[X::NTWR > 0 ? X::NTWR : 1];
+  if constexpr (X::NTWR > 0) fft_load_stage1_twiddles<NX, X::NTWR>(twr, t, tws);
   if (warp == 0) {
     for (int kn = 0; kn < X::NST - 1 && kn < nkinds; ++kn) produce(kn, src_array(kn));
   }
@@ -177,7 +184,8 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
       }
     }
 
-    fft_lanes<NX, -1>(v, t, buf, tws);
+    if constexpr (X::NTWR > 0) fft_lanes_fwd_rt<NX, X::NTWR>(v, t, buf, tws, twr);
+    else fft_lanes<NX, -1>(v, t, buf, tws);
 
     if (fwd) {
       // separate the two real lines' spectra by Hermitian symmetry, keep kx <= nx/3, store.  The partner X[nx - c] of
