@@ -178,6 +178,99 @@ def cpu_baseline_sample(name, full_shape):
                       f"workload, all moments; rate scaled by {nz_s}/{full_shape[2]} to the full grid"}
 
 
+def cufft_comparison(sim, stream, shape, prm, reps=3):
+    """Timed comparison ONLY (north_star: "cuFFT may appear only as a timed comparison"; BASELINE config 4): the same RHS
+    evaluation written the way the paper describes its own code -- vendor FFT (torch.fft = cuFFT
+    3-D D2Z/Z2D on the full grid, boolean-mask dealiasing) plus un-fused elementwise tensor ops -- with the SAME transform
+    count as the product path (derivatives of xi+-, w+- once; two inverse transforms and one forward transform per moment).
+    It is not on the product path and not the oracle; its result is compared with gandalf_rhs for the record."""
+    import torch
+    nx, ny, nz = shape
+    M = prm.get("M", 0)
+    dev = torch.device("cuda", sim.params.device)
+    two_pi = 2.0 * np.pi
+    Lx, Ly, Lz = (prm.get(k, two_pi) for k in ("Lx", "Ly", "Lz"))
+    nxs = torch.arange(nx // 2 + 1, device=dev, dtype=torch.float64)
+    nys = torch.fft.fftfreq(ny, 1.0 / ny, device=dev, dtype=torch.float64)
+    nzs = torch.fft.fftfreq(nz, 1.0 / nz, device=dev, dtype=torch.float64)
+    kx = (two_pi / Lx * nxs)[None, None, :]
+    ky = (two_pi / Ly * nys)[None, :, None]
+    kz = (two_pi / Lz * nzs)[:, None, None]
+    mask = ((3 * nxs.abs() <= nx)[None, None, :] & (3 * nys.abs() <= ny)[None, :, None] & (3 * nzs.abs() <= nz)[:, None, None])
+    k2 = kx * kx + ky * ky
+    ik2 = torch.where(k2 > 0, 1.0 / k2, torch.zeros_like(k2))
+    dn = [np.sqrt(m / 2.0) for m in range(M)]
+    up = [np.sqrt((m + 1) / 2.0) for m in range(M)]
+    if M:
+        if prm.get("closure", 0) == 1 and M >= 2:
+            dn[M - 1] += up[M - 1]
+        up[M - 1] = 0.0
+    sgn = float(prm.get("g_sign", 1))
+    sz = (nz, ny, nx)
+
+    def grad(fh):
+        return (torch.fft.irfftn(1j * kx * fh, s=sz, norm="forward"), torch.fft.irfftn(1j * ky * fh, s=sz, norm="forward"))
+
+    def fwd(f):
+        return torch.fft.rfftn(f, s=sz, norm="forward") * mask
+
+    def rhs(zeta, g):
+        w = -k2 * zeta                                             # vorticities
+        xpx, xpy = grad(zeta[0]); xmx, xmy = grad(zeta[1])
+        wpx, wpy = grad(w[0]); wmx, wmy = grad(w[1])
+        A = fwd(xpx * wmy - xpy * wmx + xmx * wpy - xmy * wpx)
+        B = fwd(xpx * xmy - xpy * xmx)
+        dw = torch.stack((-0.5 * A - 0.5 * k2 * B, -0.5 * A + 0.5 * k2 * B))
+        del wpx, wpy, wmx, wmy, A, B
+        phx, phy, psx, psy = 0.5 * (xpx + xmx), 0.5 * (xpy + xmy), 0.5 * (xpx - xmx), 0.5 * (xpy - xmy)
+        dg = torch.empty_like(g)
+        Qp = None; Ra = None
+        for m in range(M):
+            gx, gy = grad(g[m])
+            P = phx * gy - phy * gx
+            Q = psx * gy - psy * gx
+            if m >= 1:
+                dg[m - 1] = fwd(Ra + up[m - 1] * Q)
+            Ra = (dn[m] * Qp - P) if m >= 1 else -P
+            Qp = Q
+        if M:
+            dg[M - 1] = fwd(Ra)
+            zero = torch.zeros_like(g[0])
+            for m in range(M):
+                lin = g[m] - dn[m] * (g[m - 1] if m >= 1 else zero) - up[m] * (g[m + 1] if m + 1 < M else zero)
+                dg[m] = dg[m] + sgn * 1j * kz * lin
+        return dw, dg
+
+    with torch.cuda.stream(stream):                                # the context's stream: device-pointer calls are stream-ordered
+        zeta, g = sim.get_state(device=True)
+        dw_o, dg_o = sim.rhs(device=True)
+    torch.cuda.synchronize()
+    dw_c, dg_c = rhs(zeta, g)                                      # also warms cuFFT's plans
+    err_w = float((dw_c - dw_o).norm() / dw_o.norm())
+    err_g = float((dg_c - dg_o).norm() / dg_o.norm()) if M else 0.0
+    del dw_c, dg_c, dw_o, dg_o
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        rhs(zeta, g)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_c = e0.elapsed_time(e1) / reps
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        f0.record(stream)
+        for _ in range(reps):
+            sim.rhs(device=True)
+        f1.record(stream)
+    torch.cuda.synchronize()
+    ms_o = f0.elapsed_time(f1) / reps
+    return {"what": "one RHS evaluation: torch.fft (cuFFT) 3-D transforms on the full grid + un-fused elementwise ops, same transform count",
+            "cufft_path_ms_per_rhs": ms_c, "cufft_path_rhs_per_s": 1e3 / ms_c,
+            "gandalf_rhs_call_ms": ms_o, "note": "gandalf_rhs_call_ms includes exporting the RHS to the boundary layout",
+            "rel_l2_vs_gandalf_rhs": {"dw": err_w, "dg": err_g}, "reps": reps}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -187,6 +280,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cufft-compare", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -300,6 +394,12 @@ def main():
                          "frac_of_8TBs_nominal": step_bytes / 1e9 / (ms * 1e-3 / args.steps) / 8000.0},
                 "kernels": kern}
 
+    cufft = None
+    if rank == 0 and world == 1 and not args.no_cufft_compare:
+        try:
+            cufft = cufft_comparison(sim, stream, shape, prm)
+        except Exception as exc:                      # the comparison must never take the bench line down
+            cufft = {"error": repr(exc)[:200]}
     if rank == 0:
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
@@ -312,7 +412,7 @@ def main():
             "config": {"workload": wl, "grid": list(shape), "M": M, "dt": dt, "fields": F, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "no flush needed: every kernel streams inputs far larger than the 126 MB L2 (working set per step > 9 GB at 4a)"},
             "steps_per_s": steps_per_s, "grid_point_moments_per_s": steps_per_s * shape[0] * shape[1] * shape[2] * F,
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cufft_comparison": cufft,
             "final_energy": {"E_A": float(hist[-1, 1]), "W_g": float(hist[-1, 6])},
         }
         print(json.dumps(line), flush=True)
