@@ -114,6 +114,16 @@ int gandalf_energy(gandalf_ctx* ctx, double out[6]);
  * |xi-|^2) (bins sum to E_A); 1: |xi+|^2 + |xi-|^2 as printed.  out: nbins doubles on the HOST. */
 int gandalf_kperp_spectrum(gandalf_ctx* ctx, int nbins, int literal_eq26, double* out);
 
+/* Hermite spectrum [Eq. 27: C_m = <|g_m|^2>], instantaneous and volume averaged:
+ * C_m = sum_k |g_m(k)|^2 over the full spectrum (so that sum_m C_m = 2 W_g).  out: M doubles on the HOST
+ * (nothing is written when M = 0).  SURVEY.md 8(f) rank 1. */
+int gandalf_hermite_spectrum(gandalf_ctx* ctx, double* out);
+
+/* Parallel spectrum E(k_par) [PAPER.md:385; Q25]: bin j = |n_z|, j = 0..nbins-1, of the Alfvenic mode
+ * energy 1/4 kperp^2 (|xi+|^2 + |xi-|^2) summed over (kx, ky) (bins sum to E_A; bins above nz/3 are zero).
+ * out: nbins doubles on the HOST. */
+int gandalf_kpar_spectrum(gandalf_ctx* ctx, int nbins, double* out);
+
 /* Copy up to max_records of the per-step records {t, E_A, E_plus, E_minus, E_kin, E_mag, W_g}
  * (7 doubles each, oldest first, host output) and the count.  Returns GANDALF_ERR_NONFINITE
  * if any recorded energy is NaN/Inf (records are still copied). */

@@ -65,6 +65,8 @@ def _load():
         lib.oracle_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
         lib.oracle_energy.argtypes = [C.c_void_p, P]
         lib.oracle_kperp_spectrum.argtypes = [C.c_void_p, C.c_int, C.c_int, P]
+        lib.oracle_hermite_spectrum.argtypes = [C.c_void_p, P]
+        lib.oracle_kpar_spectrum.argtypes = [C.c_void_p, C.c_int, P]
         lib.oracle_energy_history.argtypes = [C.c_void_p, C.c_int, P, C.POINTER(C.c_int)]
         lib.oracle_get_time.argtypes = [C.c_void_p, P, C.POINTER(C.c_longlong), P]
         lib.oracle_last_error.argtypes = [C.c_void_p]
@@ -181,6 +183,16 @@ class Oracle:
     def kperp_spectrum(self, nbins, literal_eq26=False):
         out = np.zeros(nbins)
         self._check(self._lib.oracle_kperp_spectrum(self._h, nbins, int(literal_eq26), _dp(out)), "spectrum")
+        return out
+
+    def hermite_spectrum(self):
+        out = np.zeros(max(self.M, 1))
+        self._check(self._lib.oracle_hermite_spectrum(self._h, _dp(out)), "hermite spectrum")
+        return out[: self.M]
+
+    def kpar_spectrum(self, nbins):
+        out = np.zeros(nbins)
+        self._check(self._lib.oracle_kpar_spectrum(self._h, nbins, _dp(out)), "kpar spectrum")
         return out
 
     def energy_history(self, max_records=1 << 20):

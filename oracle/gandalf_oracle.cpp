@@ -690,6 +690,35 @@ int oracle_kperp_spectrum(oracle_ctx* c, int nbins, int literal_eq26, double* ou
   return 0;
 }
 
+// Hermite spectrum (Eq. 27): C_m = <|g_m|^2> = sum over the FULL spectrum of |g_m(k)|^2 (Parseval with
+// the physical normalisation of Eq. 9).  out: M doubles.
+int oracle_hermite_spectrum(oracle_ctx* c, double* out) {
+  if (!c || (c->M > 0 && !out)) return -1;
+  for (int m = 0; m < c->M; ++m) {
+    double s = 0.0;
+    for (size_t i = 0; i < c->N; ++i) s += std::norm(c->g[m][i]);
+    out[m] = s;
+  }
+  return 0;
+}
+
+// Parallel spectrum (Q25): bin j = |n_z| of the Alfvenic mode energy 1/4 kperp^2 (|xi+|^2+|xi-|^2).
+int oracle_kpar_spectrum(oracle_ctx* c, int nbins, double* out) {
+  if (!c || !out || nbins <= 0) return -1;
+  for (int j = 0; j < nbins; ++j) out[j] = 0.0;
+  for (int iz = 0; iz < c->nz; ++iz)
+    for (int iy = 0; iy < c->ny; ++iy)
+      for (int ix = 0; ix < c->nx; ++ix) {
+        double k2 = kperp2(c, iy, ix);
+        if (!(k2 > 0.0)) continue;
+        size_t i = IDX(c, iz, iy, ix);
+        cplx xp = -c->w[0][i] / k2, xm = -c->w[1][i] / k2;
+        int j = std::abs(c->mz[iz]);
+        if (j < nbins) out[j] += 0.25 * k2 * (std::norm(xp) + std::norm(xm));
+      }
+  return 0;
+}
+
 int oracle_energy_history(oracle_ctx* c, int max_records, double* out, int* n) {
   if (!c || !n) return -1;
   int have = (int)(c->hist.size() / 7);

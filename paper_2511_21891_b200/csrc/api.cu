@@ -35,6 +35,8 @@ cudaError_t launch_forcing(const Dims& d, cd* S, const int* pairs, int npairs, d
 cudaError_t launch_energy(const Dims& d, const cd* S, double* partial, int nblocks, double* rec, double* scal, int advance,
                           cudaStream_t st);
 cudaError_t launch_spectrum(const Dims& d, const cd* S, double* col, int nbins, int literal, double dk, double* out, cudaStream_t st);
+cudaError_t launch_hermite_spectrum(const Dims& d, const cd* S, double* out, cudaStream_t st);
+cudaError_t launch_kpar_spectrum(const Dims& d, const cd* S, double* rows, int nbins, double* out, cudaStream_t st);
 
 static const double kPi = 3.14159265358979323846264338327950288;
 enum { KC_ZINV = 0, KC_YINV = 1, KC_XPASS = 2, KC_YFWD = 3, KC_ZSTEP = 4, KC_N = 5 };
@@ -441,6 +443,39 @@ int gandalf_kperp_spectrum(gandalf_ctx* c, int nbins, int literal_eq26, double* 
   }
   const double dk = 2.0 * kPi / std::fmax(c->p.Lx, c->p.Ly);
   GD_CUDA(c, timed(c, -1, 2, [&] { return launch_spectrum(c->d, c->S0, c->spec_col, nbins, literal_eq26, dk, c->spec_out, c->st); }));
+  GD_CUDA(c, cudaMemcpyAsync(out, c->spec_out, (size_t)nbins * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+  GD_CUDA(c, cudaStreamSynchronize(c->st));
+  return GANDALF_OK;
+}
+
+static int ensure_spec(gandalf_ctx* c, int n) {
+  if (n <= c->spec_cap) return GANDALF_OK;
+  if (c->spec_out) { GD_CUDA(c, cudaStreamSynchronize(c->st)); cudaFree(c->spec_out); c->spec_out = nullptr; c->spec_cap = 0; }
+  GD_CUDA(c, cudaMalloc((void**)&c->spec_out, (size_t)n * sizeof(double)));
+  c->spec_cap = n;
+  return GANDALF_OK;
+}
+
+int gandalf_hermite_spectrum(gandalf_ctx* c, double* out) {
+  if (!c || (c->d.M > 0 && !out)) return GANDALF_ERR_INVALID;
+  if (c->d.M == 0) return GANDALF_OK;
+  GD_CUDA(c, cudaSetDevice(c->p.device));
+  int rc = ensure_spec(c, c->d.M);
+  if (rc) return rc;
+  GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_spectrum(c->d, c->S0, c->spec_out, c->st); }));
+  GD_CUDA(c, cudaMemcpyAsync(out, c->spec_out, (size_t)c->d.M * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+  GD_CUDA(c, cudaStreamSynchronize(c->st));
+  return GANDALF_OK;
+}
+
+int gandalf_kpar_spectrum(gandalf_ctx* c, int nbins, double* out) {
+  if (!c || !out || nbins <= 0 || nbins > 65535) return GANDALF_ERR_INVALID;
+  GD_CUDA(c, cudaSetDevice(c->p.device));
+  int rc = ensure_spec(c, nbins);
+  if (rc) return rc;
+  // spec_col (Ky*Kx doubles) has room for the Kz per-plane sums: Kz <= Ky*Kx because nx, ny >= 8 ... checked here
+  if ((size_t)c->d.Kz > (size_t)c->d.Ky * c->d.Kx) GD_FAIL(c, GANDALF_ERR_UNSUPPORTED, "gandalf_kpar_spectrum: nz too large for this grid");
+  GD_CUDA(c, timed(c, -1, 2, [&] { return launch_kpar_spectrum(c->d, c->S0, c->spec_col, nbins, c->spec_out, c->st); }));
   GD_CUDA(c, cudaMemcpyAsync(out, c->spec_out, (size_t)nbins * sizeof(double), cudaMemcpyDeviceToHost, c->st));
   GD_CUDA(c, cudaStreamSynchronize(c->st));
   return GANDALF_OK;

@@ -245,6 +245,52 @@ __global__ void __launch_bounds__(256) k_spec_bins(Dims d, const double* __restr
   if (threadIdx.x == 0) out[j] = sh[0];
 }
 
+// ---- Hermite spectrum C_m = <|g_m|^2> (Eq. 27) and parallel spectrum E(|n_z|) (Q25) ----
+// One block per row r: a fixed-order strided sum and a tree reduction (deterministic).
+//   kind 0: r = m,  C_m = sum_k |g_m(k)|^2 over the full spectrum (half-plane weight 1 at kx = 0, else 2)
+//   kind 1: r = cz, the Alfvenic mode energy 1/4 |w+-|^2 / kperp^2 summed over the (kx,ky) plane of that kz
+__global__ void __launch_bounds__(256) k_row_sums(Dims d, const cd* __restrict__ S, int kind, double* __restrict__ out) {
+  const int r = blockIdx.x;
+  const int plane = d.Ky * d.Kx;
+  double acc = 0.0;
+  if (kind == 0) {
+    const cd* g = S + (size_t)(2 + r) * d.PS;
+    for (size_t i = threadIdx.x; i < d.PS; i += blockDim.x) {
+      const cd v = g[i];
+      acc += ((int)(i % d.Kx) == 0 ? 1.0 : 2.0) * (v.x * v.x + v.y * v.y);
+    }
+  } else {
+    for (int i = threadIdx.x; i < plane; i += blockDim.x) {
+      const int cx = i % d.Kx, cy = i / d.Kx;
+      const double kx = d.kx0 * cx, ky = d.ky0 * c2n(cy, d.hy3, d.Ky);
+      const double k2 = kx * kx + ky * ky;
+      if (k2 > 0.0) {
+        const cd wp = S[(size_t)r * plane + i], wm = S[d.PS + (size_t)r * plane + i];
+        acc += (cx == 0 ? 1.0 : 2.0) * 0.25 * ((wp.x * wp.x + wp.y * wp.y) + (wm.x * wm.x + wm.y * wm.y)) / k2;
+      }
+    }
+  }
+  __shared__ double sh[256];
+  sh[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[r] = sh[0];
+}
+// bins j = |n_z|: out[j] = row(+j) + row(-j)
+__global__ void k_kpar_bins(Dims d, const double* __restrict__ rows, int nbins, double* __restrict__ out) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nbins) return;
+  double v = 0.0;
+  if (j <= d.hz3) {
+    v = rows[j];
+    if (j > 0) v += rows[d.Kz - j];
+  }
+  out[j] = v;
+}
+
 // ---- launchers ---------------------------------------------------------------------------------------------
 static inline int nblk(size_t n, int b) { return (int)((n + b - 1) / b); }
 
@@ -282,5 +328,14 @@ cudaError_t launch_energy(const Dims& d, const cd* S, double* partial, int nbloc
 cudaError_t launch_spectrum(const Dims& d, const cd* S, double* col, int nbins, int literal, double dk, double* out, cudaStream_t st) {
   k_spec_columns<<<nblk((size_t)d.Ky * d.Kx, 256), 256, 0, st>>>(d, S, col, literal);
   k_spec_bins<<<nbins, 256, 0, st>>>(d, col, dk, out);
+  return cudaGetLastError();
+}
+cudaError_t launch_hermite_spectrum(const Dims& d, const cd* S, double* out, cudaStream_t st) {
+  k_row_sums<<<d.M, 256, 0, st>>>(d, S, 0, out);
+  return cudaGetLastError();
+}
+cudaError_t launch_kpar_spectrum(const Dims& d, const cd* S, double* rows, int nbins, double* out, cudaStream_t st) {
+  k_row_sums<<<d.Kz, 256, 0, st>>>(d, S, 1, rows);
+  k_kpar_bins<<<nblk((size_t)nbins, 128), 128, 0, st>>>(d, rows, nbins, out);
   return cudaGetLastError();
 }

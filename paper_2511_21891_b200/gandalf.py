@@ -66,6 +66,8 @@ def load_library():
     lib.gandalf_step.argtypes = [V, D, I]
     lib.gandalf_energy.argtypes = [V, PD]
     lib.gandalf_kperp_spectrum.argtypes = [V, I, I, PD]
+    lib.gandalf_hermite_spectrum.argtypes = [V, PD]
+    lib.gandalf_kpar_spectrum.argtypes = [V, I, PD]
     lib.gandalf_energy_history.argtypes = [V, I, PD, C.POINTER(I)]
     lib.gandalf_get_time.argtypes = [V, PD, C.POINTER(C.c_longlong), PD]
     lib.gandalf_launch_count.argtypes = [V]
@@ -177,6 +179,16 @@ class Gandalf:
     def kperp_spectrum(self, nbins, literal_eq26=False):
         out = np.zeros(nbins)
         self._ck(self._lib.gandalf_kperp_spectrum(self._h, nbins, int(literal_eq26), out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def hermite_spectrum(self):
+        out = np.zeros(max(self.M, 1))
+        self._ck(self._lib.gandalf_hermite_spectrum(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out[: self.M]
+
+    def kpar_spectrum(self, nbins):
+        out = np.zeros(nbins)
+        self._ck(self._lib.gandalf_kpar_spectrum(self._h, nbins, out.ctypes.data_as(C.POINTER(C.c_double))))
         return out
 
     def energy_history(self, max_records=None):

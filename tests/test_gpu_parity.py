@@ -235,3 +235,15 @@ def test_launch_count_and_kernel_timing():
     assert g.launch_count() - n0 == 2 * 14
     assert kt["x_pass_P2"][1] == 4 and kt["x_pass_P2"][0] > 0
     assert kt["z_step_P4"][1] == 4 and kt["z_step_P4"][0] > 0
+
+
+def test_hermite_and_parallel_spectra_match_oracle():
+    prm, z, gm, run = config2(32, 32, 16, 6)
+    o, g = _pair(run["shape"], prm)
+    o.set_state(z, gm); g.set_state(z, gm)
+    o.step(run["dt"], 5); g.step(run["dt"], 5)
+    co, cg = o.hermite_spectrum(), g.hermite_spectrum()
+    assert np.abs(cg - co).max() <= 1e-10 * co.max()
+    ko, kg = o.kpar_spectrum(9), g.kpar_spectrum(9)
+    assert np.abs(kg - ko).max() <= 1e-10 * ko.max()
+    assert abs(kg.sum() - g.energy()[0]) <= 1e-12 * kg.sum() and abs(cg.sum() - 2 * g.energy()[5]) <= 1e-12 * cg.sum()

@@ -223,6 +223,28 @@ def test_p10_spectrum_sums_to_energy():
     assert s[2] > 0 and np.count_nonzero(s) == 1
 
 
+# ---- P12: Hermite and parallel spectra (Eq. 27; Q25) -----------------------------
+def test_p12_hermite_and_parallel_spectra():
+    nx, ny, nz, M = 16, 16, 8, 5
+    o = Oracle(nx, ny, nz, M=M)
+    o.set_state(synth.dense_random(nx, ny, nz, 2, seed=31), synth.dense_random(nx, ny, nz, M, seed=32))
+    e = o.energy()
+    cm = o.hermite_spectrum()
+    assert cm.shape == (M,) and abs(cm.sum() - 2.0 * e[5]) <= 1e-13 * cm.sum()          # sum_m C_m = 2 W_g
+    _, g = o.get_state()
+    w = np.full(nx // 2 + 1, 2.0); w[0] = 1.0
+    for m in range(M):                                                                  # Parseval on the half-plane
+        assert abs(cm[m] - float((np.abs(g[m]) ** 2 * w).sum())) <= 1e-13 * cm[m]
+    kp = o.kpar_spectrum(nz // 2 + 1)
+    assert abs(kp.sum() - e[0]) <= 1e-13 * e[0]                                         # bins sum to E_A
+    assert np.all(kp[nz // 3 + 1:] == 0.0)                                              # removed k_z carry nothing
+    # a single mode (1, 0, -2) lands in the bin |n_z| = 2 with its whole energy
+    o2 = Oracle(nx, ny, nz)
+    o2.set_state(synth.single_mode(nx, ny, nz, (1, 0, -2), 0.7))
+    s = o2.kpar_spectrum(5)
+    assert np.count_nonzero(s) == 1 and abs(s[2] - o2.energy()[0]) <= 1e-14 * s[2]
+
+
 # ---- P11: forcing (Eq. 25, Q17) ----------------------------------------------------------------
 def test_p11_forcing_power_and_hermitian_consistency():
     nx, ny, nz = 16, 16, 8
