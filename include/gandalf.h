@@ -59,6 +59,9 @@ typedef struct gandalf_params {
   int    force_nperp_min, force_nperp_max, force_nz_max;  /* forced shell in mode numbers          */
   unsigned long long seed;/* forcing RNG key (counter-based, Q17)                       */
   double cfl;             /* C of Eq. 16, used when gandalf_step gets dt <= 0      */
+  double force_g_amp;     /* white-noise forcing of g_0 at k = (0,0,+-force_g_nz): amplitude a_g, mean injected
+                             power a_g^2 into W_g; 0 = off  [velocity-space benchmark; Q26] */
+  int    force_g_nz;      /* forced parallel mode number (>= 1, retained); paper: 1               */
   int    device;          /* CUDA device ordinal                                                  */
   void*  stream;          /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
 } gandalf_params;

@@ -41,13 +41,14 @@ class OracleParams(C.Structure):
         ("force_nz_max", C.c_int),
         ("seed", C.c_ulonglong),
         ("cfl", C.c_double),
+        ("force_g_amp", C.c_double), ("force_g_nz", C.c_int),
     ]
 
 
 _DEFAULTS = dict(M=0, Lx=2 * np.pi, Ly=2 * np.pi, Lz=2 * np.pi, vA=1.0, eta=0.0, r=1, eta_normalized=0,
                  eta_z=0.0, r_z=1, eta_g=0.0, nu_coll=0.0, p=1.0, closure=0, if_variant=0, g_sign=1,
                  nonlinear=1, hermite_coeff=0, force_eps=0.0, force_nperp_min=1, force_nperp_max=2,
-                 force_nz_max=1, seed=0, cfl=0.3)
+                 force_nz_max=1, seed=0, cfl=0.3, force_g_amp=0.0, force_g_nz=1)
 
 _lib = None
 

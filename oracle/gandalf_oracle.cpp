@@ -68,6 +68,7 @@ struct oracle_params {
   double force_eps; int force_nperp_min, force_nperp_max, force_nz_max;
   unsigned long long seed;
   double cfl;
+  double force_g_amp; int force_g_nz;   // g_0 forcing at k = (0,0,+-nz) (Q26)
 };
 
 }  // extern "C"
@@ -450,6 +451,20 @@ static void apply_forcing(oracle_ctx* c, State& s, double dt) {
     }
 }
 
+// Velocity-space benchmark forcing ("single forced mode k=(0,0,1) in g_0"; reading Q26): after the
+// dissipation step, delta g_0(0,0,n) = a_g sqrt(dt) (eta_r + i eta_i)/sqrt(2), the conjugate at (0,0,-n).
+// RNG key seed ^ 0xA5A5A5A5A5A5A5A5, counters 2*step and 2*step+1; Box-Muller as in apply_forcing.
+static void apply_forcing_g(oracle_ctx* c, State& s, double dt) {
+  const oracle_params& p = c->p;
+  if (!(p.force_g_amp > 0.0) || c->M < 1) return;
+  unsigned long long key = p.seed ^ 0xA5A5A5A5A5A5A5A5ULL;
+  double u1 = rng_uniform(key, 2ULL * (unsigned long long)c->step), u2 = rng_uniform(key, 2ULL * (unsigned long long)c->step + 1ULL);
+  double rad = std::sqrt(-2.0 * std::log(1.0 - u1));
+  cplx dg = p.force_g_amp * std::sqrt(dt) * cplx(rad * std::cos(2.0 * PI * u2), rad * std::sin(2.0 * PI * u2)) / std::sqrt(2.0);
+  s.g[0][IDX(c, wrap(p.force_g_nz, c->nz), 0, 0)] += dg;
+  s.g[0][IDX(c, wrap(-p.force_g_nz, c->nz), 0, 0)] += std::conj(dg);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Diagnostics (Q14, Q15): sums over the full spectrum.
 // ---------------------------------------------------------------------------------------------
@@ -532,6 +547,7 @@ static int step_once(oracle_ctx* c, double dt_in) {
   apply_dissipation(c, s1, dt);
   // forcing increment (Q17), then time and diagnostics
   apply_forcing(c, s1, dt);
+  apply_forcing_g(c, s1, dt);
   c->w[0].swap(s1.w[0]); c->w[1].swap(s1.w[1]); c->g.swap(s1.g);
   c->t += dt; c->step += 1; c->last_dt = dt;
   State cur; cur.w[0] = c->w[0]; cur.w[1] = c->w[1]; cur.g = c->g;

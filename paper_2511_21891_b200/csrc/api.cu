@@ -32,6 +32,8 @@ cudaError_t launch_pack(const Dims& d, const cd* in, cd* S, int nfields, int nze
 cudaError_t launch_unpack(const Dims& d, const cd* S, cd* out, int nfields, int nzeta, cudaStream_t st);
 cudaError_t launch_forcing(const Dims& d, cd* S, const int* pairs, int npairs, double amp, unsigned long long seed,
                            long long step, const double* scal, cudaStream_t st);
+cudaError_t launch_forcing_g(const Dims& d, cd* S, int nzf, double amp, unsigned long long seed, long long step,
+                             const double* scal, cudaStream_t st);
 cudaError_t launch_energy(const Dims& d, const cd* S, double* partial, int nblocks, double* rec, double* scal, int advance,
                           cudaStream_t st);
 cudaError_t launch_spectrum(const Dims& d, const cd* S, double* col, int nbins, int literal, double dk, double* out, cudaStream_t st);
@@ -135,6 +137,7 @@ int gandalf_default_params(gandalf_params* p) {
   p->g_sign = 1; p->nonlinear = 1;
   p->force_nperp_min = 1; p->force_nperp_max = 2; p->force_nz_max = 1;
   p->cfl = 0.3;
+  p->force_g_nz = 1;
   return GANDALF_OK;
 }
 
@@ -147,6 +150,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (p->r < 1 || p->r_z < 1 || !(p->p > 0) || (p->g_sign != 1 && p->g_sign != -1)) return GANDALF_ERR_INVALID;
   if (p->eta < 0 || p->eta_z < 0 || p->eta_g < 0 || p->nu_coll < 0 || p->force_eps < 0) return GANDALF_ERR_INVALID;
   if (p->closure != 0 && p->closure != 1) return GANDALF_ERR_INVALID;
+  if (p->force_g_amp < 0 || (p->force_g_amp > 0 && (p->M < 1 || p->force_g_nz < 1 || p->force_g_nz > p->nz / 3))) return GANDALF_ERR_INVALID;
   if (p->M > 0 && p->vA != 1.0) return GANDALF_ERR_UNSUPPORTED;
   if (cudaSetDevice(p->device) != cudaSuccess) { cudaGetLastError(); return GANDALF_ERR_CUDA; }
 
@@ -410,6 +414,13 @@ int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
       }));
       // the forcing touches w+- only: refresh the hybrid copy of those two fields
       if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, +1, c->S0, c->H, c->twz, 2, c->st); }));
+    }
+    if (c->p.force_g_amp > 0.0) {
+      GD_CUDA(c, timed(c, -1, 1, [&] {
+        return launch_forcing_g(d, c->S0, c->p.force_g_nz, c->p.force_g_amp, c->p.seed, c->step, c->scal, c->st);
+      }));
+      // the forcing touches g_0 only: refresh the hybrid copy of that field
+      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, +1, c->S0 + 2 * d.PS, c->H + 2 * d.PH, c->twz, 1, c->st); }));
     }
     GD_CUDA(c, timed(c, -1, 2, [&] {
       return launch_energy(d, c->S0, c->partial, kEnergyBlocks, c->hist + (size_t)c->step * 7, c->scal, 1, c->st);

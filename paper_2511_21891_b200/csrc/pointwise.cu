@@ -143,6 +143,23 @@ __global__ void k_forcing(Dims d, cd* __restrict__ S, const int* __restrict__ pa
   }
 }
 
+// g_0 forcing of the velocity-space benchmark (Q26): one thread.
+__global__ void k_forcing_g(Dims d, cd* __restrict__ S, int nzf, double amp, unsigned long long seed, long long step,
+                            const double* __restrict__ scal) {
+  const unsigned long long key = seed ^ 0xA5A5A5A5A5A5A5A5ULL;
+  const double u1 = rng_u01(key, 2ULL * (unsigned long long)step), u2 = rng_u01(key, 2ULL * (unsigned long long)step + 1ULL);
+  const double rad = sqrt(-2.0 * log(1.0 - u1));
+  double sn, cs;
+  sincos(2.0 * 3.14159265358979323846 * u2, &sn, &cs);
+  const double sc = amp * sqrt(scal[SC_DT]) * 0.70710678118654752440;
+  const cd dg = cmake(sc * rad * cs, sc * rad * sn);
+  cd* g0 = S + (size_t)2 * d.PS;
+  const size_t plane = (size_t)d.Ky * d.Kx;
+  const size_t i1 = (size_t)nzf * plane, i2 = (size_t)(d.Kz - nzf) * plane;      // (kx, ky) = (0, 0); kz = +nzf, -nzf
+  g0[i1] = cmake(g0[i1].x + dg.x, g0[i1].y + dg.y);
+  g0[i2] = cmake(g0[i2].x + dg.x, g0[i2].y - dg.y);
+}
+
 // ---- energies (Q14): deterministic two-level reduction ---------------------------------------
 // partial[b][5] = { E+, E-, E_kin, E_mag, W_g } of block b; half-plane weight 1 at kx = 0, else 2.
 __global__ void __launch_bounds__(256) k_energy_partial(Dims d, const cd* __restrict__ S, double* __restrict__ partial) {
@@ -337,5 +354,10 @@ cudaError_t launch_hermite_spectrum(const Dims& d, const cd* S, double* out, cud
 cudaError_t launch_kpar_spectrum(const Dims& d, const cd* S, double* rows, int nbins, double* out, cudaStream_t st) {
   k_row_sums<<<d.Kz, 256, 0, st>>>(d, S, 1, rows);
   k_kpar_bins<<<nblk((size_t)nbins, 128), 128, 0, st>>>(d, rows, nbins, out);
+  return cudaGetLastError();
+}
+cudaError_t launch_forcing_g(const Dims& d, cd* S, int nzf, double amp, unsigned long long seed, long long step,
+                             const double* scal, cudaStream_t st) {
+  k_forcing_g<<<1, 1, 0, st>>>(d, S, nzf, amp, seed, step, scal);
   return cudaGetLastError();
 }

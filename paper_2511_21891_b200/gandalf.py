@@ -32,6 +32,7 @@ class GandalfParams(C.Structure):
         ("force_nz_max", C.c_int),
         ("seed", C.c_ulonglong),
         ("cfl", C.c_double),
+        ("force_g_amp", C.c_double), ("force_g_nz", C.c_int),
         ("device", C.c_int),
         ("stream", C.c_void_p),
     ]

@@ -268,3 +268,37 @@ def test_p11_forcing_power_and_hermitian_consistency():
     o2.set_state(np.zeros((2, nz, ny, nx // 2 + 1)))
     o2.step(dt, 3)
     assert np.array_equal(o2.energy_history(), h[:3])
+
+
+# ---- P13: g_0 forcing of the velocity-space benchmark (Q26) ------------------------------------
+def test_p13_g0_forcing_power_support_and_restart():
+    nx, ny, nz, M, a, dt = 8, 8, 8, 3, 0.3, 1e-2
+    zero_z = np.zeros((2, nz, ny, nx // 2 + 1))
+    zero_g = np.zeros((M, nz, ny, nx // 2 + 1))
+    # mean injected power: one step from rest, many keys; W_g = |delta|^2 has mean a^2 dt (exponentially distributed)
+    K, acc = 400, 0.0
+    for k in range(K):
+        o = Oracle(nx, ny, nz, M=M, nonlinear=0, force_g_amp=a, force_g_nz=2, seed=1000 + k)
+        o.set_state(zero_z, zero_g)
+        o.step(dt, 1)
+        acc += o.energy()[5]
+    mean = acc / K
+    assert abs(mean - a * a * dt) <= 3.0 * a * a * dt / np.sqrt(K), (mean, a * a * dt)
+    # support and Hermitian consistency: only g_0 at (0,0,+-2), conjugate partners
+    _, g = o.get_state()
+    nzv = np.argwhere(np.abs(g) > 0)
+    assert {tuple(r) for r in nzv} == {(0, 2, 0, 0), (0, nz - 2, 0, 0)}
+    assert g[0, 2, 0, 0] == np.conj(g[0, nz - 2, 0, 0])
+    # restart: 6 steps == 3 + (state, time, step restored by the same sequence of calls) 3 more steps with the same key
+    o1 = Oracle(nx, ny, nz, M=M, nonlinear=0, force_g_amp=a, force_g_nz=1, seed=7, nu_coll=0.2, p=2.0)
+    o1.set_state(zero_z, zero_g); o1.step(dt, 6)
+    o2 = Oracle(nx, ny, nz, M=M, nonlinear=0, force_g_amp=a, force_g_nz=1, seed=7, nu_coll=0.2, p=2.0)
+    o2.set_state(zero_z, zero_g); o2.step(dt, 3); o2.step(dt, 3)
+    assert np.array_equal(o1.get_state()[1], o2.get_state()[1])
+    # streaming conserves W_g: with the forcing off after a kick, W_g stays put (nu = 0)
+    o3 = Oracle(nx, ny, nz, M=8, nonlinear=0)
+    g0 = np.zeros((8, nz, ny, nx // 2 + 1), dtype=np.complex128); g0[0, 1, 0, 0] = 0.5; g0[0, nz - 1, 0, 0] = 0.5
+    o3.set_state(zero_z, g0)
+    w0 = o3.energy()[5]
+    o3.step(1e-3, 50)
+    assert abs(o3.energy()[5] - w0) <= 1e-6 * w0          # RK2 is second order: drift ~ (kz dt)^3 per step
