@@ -290,3 +290,21 @@ def test_velocity_space_benchmark_linear_cascade_slope_reported():
     slope = np.polyfit(np.log(ms), np.log(cm[2:21]), 1)[0]
     print(f"velocity-space benchmark: time-averaged C_m slope over m in [2,20] = {slope:.3f} (paper: -0.50 +- 0.02)")
     assert np.isfinite(cm).all() and cm[2] > cm[20] > cm[100] and slope < 0
+
+
+def test_repeated_runs_are_bit_identical():
+    """No result depends on CTA scheduling: fixed-order reductions, no floating-point atomics (the CFL maximum is an
+    order-independent atomicMax), persistent kernels that assign work by index.  Two runs of config 3 (forcing + CFL dt)
+    must agree bit for bit -- also a race check for the TMA / mbarrier pipelines."""
+    from paper_2511_21891_b200.gandalf import Gandalf
+    prm, z, gm, run = config3(32, 32, 16, 6)
+    outs = []
+    for _ in range(2):
+        g = Gandalf(*run["shape"], **prm)
+        g.set_state(z, gm)
+        g.step(0.0, 12)
+        zz, gg = g.get_state()
+        outs.append((zz.copy(), gg.copy(), g.energy_history().copy()))
+        g.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert np.array_equal(outs[0][2], outs[1][2])
