@@ -92,7 +92,6 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   cd* tile = smem + FftTw<NZ>::COUNT;                          // [KZ][LD], aliases the exchange buffers
   cd* buf = tile + (size_t)grp * (G::BUF + 1);
-  fft_load_table<NZ>(smem, tw);
   const cd* tws = smem;
   const int plane = d.Ky * d.Kx;
   const int f = blockIdx.x % d.F, cb = blockIdx.x / d.F;
@@ -101,12 +100,19 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
   const bool active = col < plane;
   const int colc = active ? col : 0;
   const int planeH = d.Ky * d.Kxp, colH = (colc / d.Kx) * d.Kxp + colc % d.Kx;   // hybrid rows are padded to Kxp
+  // per-item scalars and the column of Gh are requested BEFORE the twiddle table is staged, so that all three
+  // round trips overlap
+  const double dt = scal[SC_DT];
+  const int m = f - 2;
+  const double dn = f >= 2 ? cdn[m] : 0.0, up = f >= 2 ? cup[m] : 0.0;
+  const double cf = (mode == 2 && f >= 2) ? collfac[m] : 1.0;
   // 1. forward z transform of the bracket term, retained kz -> tile (scaled by 1/N)
   if (Gh != nullptr) {
     cd v[E];
     const cd* src = Gh + (size_t)f * d.PH + colH;
 #pragma unroll
     for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * planeH) : cmake(0.0, 0.0);
+    fft_load_table<NZ>(smem, tw);                              // ends with __syncthreads()
     fft_lanes<NZ, -1>(v, t, buf, tws);
     __syncthreads();                                           // every group is done with its exchange buffer
 #pragma unroll
@@ -115,18 +121,15 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
       if (cz >= 0) tile[cz * LD + grp] = cscale(v[q], d.inv_n);
     }
   } else {
+    fft_load_table<NZ>(smem, tw);                              // ends with __syncthreads()
     for (int e = threadIdx.x; e < KZ * LD; e += GD_Z_THREADS) tile[e] = cmake(0.0, 0.0);
   }
   __syncthreads();
   // 2. pointwise stage update on the tile: thread <-> (kz, column), columns fastest (row-contiguous global accesses);
   //    the loads of UB modes are issued together
   {
-    const double dt = scal[SC_DT];
     const double c = (mode == 1) ? 0.5 * dt : dt;
-    const int m = f - 2;
     const bool lo = f > 2, hi = f + 1 < d.F, same = (Ws == Wn || mode == 0);
-    const double dn = f >= 2 ? cdn[m] : 0.0, up = f >= 2 ? cup[m] : 0.0;
-    const double cf = (mode == 2 && f >= 2) ? collfac[m] : 1.0;
     const int ncolv = min(GROUPS, plane - col0);
     constexpr int NEL = KZ * GROUPS, UB = 6;
     for (int e0 = threadIdx.x; e0 < NEL; e0 += UB * GD_Z_THREADS) {
