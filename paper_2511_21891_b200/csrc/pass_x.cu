@@ -29,7 +29,7 @@ struct XGeom {
   static constexpr int GROUPS = THREADS / T;                // lines per CTA: consecutive (z,y), y fastest
   static constexpr int LD = GROUPS;                         // row of a staged tile [kx][line]; line slot XOR-swizzled with kx
   static constexpr int STAGE = 2 * KXP * LD;                // one stage: the tiles of f~ and (df/dy)~ for all lines of the CTA
-  static constexpr int NST = 3;                             // stages in flight (full/empty mbarrier ring)
+  static constexpr int NST = 3;                             // stages in flight (full/empty mbarrier ring), <= 5 (the first NST-1 are Elsasser arrays)
   // stage-1 twiddles held in registers (plans with one stage-1 butterfly per lane): fewer shared-memory reads per transform
   static constexpr int NTWR = (G::S == 2 && E / FftPlan<NX>::R1 == 1) ? GD_X_NTWR : 0;
   static constexpr size_t SMEM = ((size_t)GROUPS * LB + (size_t)NST * STAGE + FftTw<NX>::COUNT) * sizeof(cd);
@@ -85,6 +85,18 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int i = 0; i < X::NST; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], X::WARPS); }
+    // the first NST-1 stages (xi+, xi-: arrays 0/1 and 2/3) are requested right away, by the thread that initialised
+    // the barriers, so that they travel while tensor memory is allocated and the twiddle table is staged
+    constexpr unsigned TILE_BYTES0 = (unsigned)(X::KXP * X::LD * sizeof(cd));
+#pragma unroll
+    for (int kn = 0; kn < X::NST - 1; ++kn) {
+      const int a = kn == 0 ? 0 : kn == 1 ? 2 : kn == 2 ? 6 : 4;
+      mbar_arrive_expect_tx(&s_full[kn], 2u * TILE_BYTES0);
+      cd* st = stages + (size_t)kn * X::STAGE;
+      const cd* src = D + (size_t)a * d.PD + (size_t)blockIdx.x * (X::KXP * X::LD);
+      bulk_g2s(st, src, TILE_BYTES0, &s_full[kn]);
+      bulk_g2s(st + X::KXP * X::LD, src + d.PD, TILE_BYTES0, &s_full[kn]);
+    }
   }
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&s_tmem_base)), "r"(512) : "memory");
@@ -130,9 +142,6 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   double gmax = 0.0;
   cd twr[X::NTWR > 0 ? X::NTWR : 1];
   if constexpr (X::NTWR > 0) fft_load_stage1_twiddles<NX, X::NTWR>(twr, t, tws);
-  if (warp == 0) {
-    for (int kn = 0; kn < X::NST - 1 && kn < nkinds; ++kn) produce(kn, src_array(kn));
-  }
   for (;;) {
     if (!fwd) {
       if (kind == nkinds) {
