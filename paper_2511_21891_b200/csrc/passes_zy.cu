@@ -1,15 +1,16 @@
-// passes_zy.cu -- z transforms (compact <-> hybrid) and the y passes P1 / P3 of the RHS pipeline.
+// passes_zy.cu -- the z transforms and the y passes of the RHS pipeline.
 //
-//   k_zinv : S[f][cz][cy][cx] -> H[f][z][cy][cx]      inverse c2c along z, zero-padded
-//   k_zfwd : H -> S                                   forward c2c along z, kz part of Eq. 20, 1/N scale
-//   k_yinv : P1.  H -> D: for w+- also xi = -w/kperp^2; for every source field f the
-//            pair ( f , d f/dy = IFFT_y(i ky f) )  (Eq. 10), inverse c2c along y;
-//            the two arrays of a pair are transformed by sibling warps (no second copy of the input in registers)
-//   k_yfwd : P3.  E -> H: forward c2c along y, ky part of Eq. 20; the Elsasser pair is assembled as
-//            N+- = -1/2 A -+ 1/2 kperp^2 B  (Eq. 1 with Eq. 11)
-// Every FFT is fft_lanes<N> (fft.cuh): T lanes of one warp per column, data in registers, one
-// shared-memory exchange per stage boundary.  Adjacent lane groups take adjacent cx so that global
-// accesses of a warp cover contiguous kx runs.
+//   k_zfft<+1>  : S[f][cz][cy][cx] -> H[f][z][cy][cx]  inverse c2c along z, zero-padded; only after
+//                 set_state and after a forcing increment (k_zfft<-1>, the stand-alone forward transform, is kept for tests
+//                 of the building block but is not on the step path any more)
+//   k_zstep     : P4.  Gh -> S', H': forward z transform + stage update + inverse z transform in one kernel
+//   k_yinv      : P1.  H -> D: for every source field the two arrays U = kx f + df/dy, V = df/dy - kx f (Eq. 10,
+//                 PAPER.md:134; for w+- also of xi = -w/kperp^2), inverse c2c along y
+//   k_yfwd(_pair): P3.  E -> Gh: forward c2c along y, ky part of Eq. 20; the Elsasser pair is assembled as
+//                 N+- = -1/2 A -+ 1/2 kperp^2 B  (Eq. 1 with Eq. 11)
+// Every FFT is the lane-group transform of fft.cuh: T lanes of one warp per column, data in registers, one
+// shared-memory exchange per stage boundary.  The y passes stage their input tiles with bulk async copies (TMA engine,
+// mbarrier completion) so that global memory sees whole row segments; see DESIGN.md section 5.
 #include <vector>
 #include "common.cuh"
 
