@@ -28,6 +28,7 @@ import numpy as np  # noqa: E402
 
 WORKLOADS = {
     "4a": ("config4a", dict(nx=256, ny=256, nz=128, M=32)),
+    "4a2": ("config4a", dict(nx=256, ny=256, nz=128, M=32, nspecies=2)),     # both species: 2 + 64 fields
     "4b": ("config4b", dict(nx=512, ny=512, nz=256)),
     "2": ("config2", dict(nx=64, ny=64, nz=32, M=16)),
     "0": ("config0", dict(nx=32, ny=32, nz=16)),
@@ -145,7 +146,7 @@ def run_reference(args, rank, world):
     el = time.perf_counter() - t0
     frac = nz_s / full[2]
     steps_per_s = args.steps / el * frac
-    M = prm.get("M", 0)
+    M = prm.get("M", 0) * prm.get("nspecies", 1)
     line = {
         "impl": "reference", "metric": "RHS evals/s", "value": 2 * steps_per_s, "unit": "RHS evals/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / steps_per_s, "higher_is_better": True,
@@ -301,7 +302,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     prm, z, g, run = make_workload(args.workload)
-    shape, dt, M = run["shape"], run["dt"], prm.get("M", 0)
+    shape, dt, M = run["shape"], run["dt"], prm.get("M", 0) * prm.get("nspecies", 1)      # M = moment fields
     F = 2 + M
     stream = torch.cuda.Stream()
     sim = Gandalf(*shape, device=local, stream=stream.cuda_stream, **prm)
@@ -395,7 +396,7 @@ def main():
                 "kernels": kern}
 
     cufft = None
-    if rank == 0 and world == 1 and not args.no_cufft_compare:
+    if rank == 0 and world == 1 and not args.no_cufft_compare and prm.get("nspecies", 1) == 1:
         try:
             cufft = cufft_comparison(sim, stream, shape, prm)
         except Exception as exc:                      # the comparison must never take the bench line down
@@ -404,7 +405,8 @@ def main():
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             cpu = cpu_baseline_sample(args.workload, shape)
-        wl = {"4a": "BASELINE config 4(a)", "4b": "BASELINE config 4(b)"}.get(args.workload, f"BASELINE config {args.workload}")
+        wl = {"4a": "BASELINE config 4(a)", "4b": "BASELINE config 4(b)",
+              "4a2": "BASELINE config 4(a) with both slow-mode species (2+64 fields)"}.get(args.workload, f"BASELINE config {args.workload}")
         line = {
             "metric": "RHS evals/s", "value": 2 * steps_per_s, "unit": "RHS evals/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",

@@ -62,6 +62,9 @@ typedef struct gandalf_params {
   double force_g_amp;     /* white-noise forcing of g_0 at k = (0,0,+-force_g_nz): amplitude a_g, mean injected
                              power a_g^2 into W_g; 0 = off  [velocity-space benchmark; Q26] */
   int    force_g_nz;      /* forced parallel mode number (>= 1, retained); paper: 1               */
+  int    nspecies;        /* 1: one set g_0..g_{M-1} with sign g_sign.  2: both slow-mode species [Eq. 2-4, PAPER.md:57-66;
+                             memory layout of PAPER.md:357]: g_hat holds 2M fields, g^+ (sign g_sign) then g^- (sign
+                             -g_sign); they share Phi, Psi and do not couple in Eq. 6 as printed (Q11, Q27) */
   int    device;          /* CUDA device ordinal                                                  */
   void*  stream;          /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
 } gandalf_params;

@@ -42,13 +42,14 @@ class OracleParams(C.Structure):
         ("seed", C.c_ulonglong),
         ("cfl", C.c_double),
         ("force_g_amp", C.c_double), ("force_g_nz", C.c_int),
+        ("nspecies", C.c_int),
     ]
 
 
 _DEFAULTS = dict(M=0, Lx=2 * np.pi, Ly=2 * np.pi, Lz=2 * np.pi, vA=1.0, eta=0.0, r=1, eta_normalized=0,
                  eta_z=0.0, r_z=1, eta_g=0.0, nu_coll=0.0, p=1.0, closure=0, if_variant=0, g_sign=1,
                  nonlinear=1, hermite_coeff=0, force_eps=0.0, force_nperp_min=1, force_nperp_max=2,
-                 force_nz_max=1, seed=0, cfl=0.3, force_g_amp=0.0, force_g_nz=1)
+                 force_nz_max=1, seed=0, cfl=0.3, force_g_amp=0.0, force_g_nz=1, nspecies=1)
 
 _lib = None
 
@@ -124,7 +125,7 @@ class Oracle:
                 raise TypeError(f"unknown oracle parameter {k!r}")
         vals.update(kw)
         self.params = OracleParams(nx=nx, ny=ny, nz=nz, **vals)
-        self.nx, self.ny, self.nz, self.M = nx, ny, nz, int(vals["M"])
+        self.nx, self.ny, self.nz, self.M = nx, ny, nz, int(vals["M"]) * int(vals["nspecies"])   # M = moment FIELDS
         self.hx = nx // 2 + 1
         h = C.c_void_p()
         rc = lib.oracle_create(C.byref(self.params), C.byref(h))

@@ -69,6 +69,7 @@ struct oracle_params {
   unsigned long long seed;
   double cfl;
   double force_g_amp; int force_g_nz;   // g_0 forcing at k = (0,0,+-nz) (Q26)
+  int nspecies;       // 1: g (sign g_sign);  2: g^+ (g_sign) then g^- (-g_sign), M moments each (Q27)
 };
 
 }  // extern "C"
@@ -124,7 +125,8 @@ struct Field {               // one full complex spectrum or real-space complex 
 
 struct oracle_ctx {
   oracle_params p;
-  int nx, ny, nz, M;
+  int nx, ny, nz, M;                        // M = number of moment FIELDS = nspecies * Msp
+  int Msp, nsp;                             // moments per species, species
   size_t N;                                 // nx*ny*nz
   std::vector<double> kx, ky, kz;           // physical wavenumbers per FFT index (Eq. 9 text)
   std::vector<int> mx, my, mz;              // signed integer mode numbers per FFT index
@@ -257,10 +259,11 @@ static void potentials(const oracle_ctx* c, const std::vector<cplx>& w, std::vec
 
 // The neighbour g_{m} with the closure applied for m == M: absorbing -> none,
 // reflecting -> g_{M-2}.  Returns -1 when the neighbour is identically zero.
-static int neighbour_index(const oracle_ctx* c, int m) {
+static int neighbour_index(const oracle_ctx* c, int sp, int m) {   // field index of moment m of species sp, or -1
+  const int M = c->Msp;
   if (m < 0) return -1;
-  if (m < c->M) return m;
-  if (m == c->M && c->p.closure == 1 && c->M >= 2) return c->M - 2;
+  if (m < M) return sp * M + m;
+  if (m == M && c->p.closure == 1 && M >= 2) return sp * M + M - 2;
   return -1;
 }
 
@@ -316,34 +319,37 @@ static void rhs_eval(const oracle_ctx* c, const State& s, State& out, double* ma
       std::vector<Grad> gg(M);
       for (int m = 0; m < M; ++m) gradient(c, s.g[m], gg[m]);
       std::vector<cplx> br;
-      for (int m = 0; m < M; ++m) {
-        bracket_from_grads(c, gPhi, gg[m], br);                       // {Phi, g_m}
-        for (size_t i = 0; i < c->N; ++i) out.g[m][i] -= br[i];
-        int lo = neighbour_index(c, m - 1), hi = neighbour_index(c, m + 1);
-        if (lo >= 0 && c->coef_dn[m] != 0.0) {
-          bracket_from_grads(c, gPsi, gg[lo], br);                    // {Psi, g_{m-1}}
-          for (size_t i = 0; i < c->N; ++i) out.g[m][i] += c->coef_dn[m] * br[i];
+      for (int sp = 0; sp < c->nsp; ++sp)                               // the bracket terms of Eq. 6 are the same for g^+ and g^-
+        for (int m = 0; m < c->Msp; ++m) {
+          const int fi = sp * c->Msp + m;
+          bracket_from_grads(c, gPhi, gg[fi], br);                    // {Phi, g_m}
+          for (size_t i = 0; i < c->N; ++i) out.g[fi][i] -= br[i];
+          int lo = neighbour_index(c, sp, m - 1), hi = neighbour_index(c, sp, m + 1);
+          if (lo >= 0 && c->coef_dn[m] != 0.0) {
+            bracket_from_grads(c, gPsi, gg[lo], br);                  // {Psi, g_{m-1}}
+            for (size_t i = 0; i < c->N; ++i) out.g[fi][i] += c->coef_dn[m] * br[i];
+          }
+          if (hi >= 0) {
+            bracket_from_grads(c, gPsi, gg[hi], br);                  // {Psi, g_{m+1}}
+            for (size_t i = 0; i < c->N; ++i) out.g[fi][i] += c->coef_up[m] * br[i];
+          }
         }
-        if (hi >= 0) {
-          bracket_from_grads(c, gPsi, gg[hi], br);                    // {Psi, g_{m+1}}
-          for (size_t i = 0; i < c->N; ++i) out.g[m][i] += c->coef_up[m] * br[i];
-        }
-      }
     }
   }
   // linear streaming / phase-mixing terms of Eq. 6 (d/dz -> i kz), sign s = +1 for g^+ (upper signs)
-  const double sgn = (double)c->p.g_sign;
-  for (int m = 0; m < M; ++m) {
-    int lo = neighbour_index(c, m - 1), hi = neighbour_index(c, m + 1);
+  for (int fi = 0; fi < M; ++fi) {
+    const int sp = fi / c->Msp, m = fi % c->Msp;
+    const double sgn = (sp == 0) ? (double)c->p.g_sign : -(double)c->p.g_sign;   // upper / lower signs of Eq. 6
+    int lo = neighbour_index(c, sp, m - 1), hi = neighbour_index(c, sp, m + 1);
 #pragma omp parallel for collapse(2) schedule(static)
     for (int iz = 0; iz < c->nz; ++iz)
       for (int iy = 0; iy < c->ny; ++iy)
         for (int ix = 0; ix < c->nx; ++ix) {
           size_t i = IDX(c, iz, iy, ix);
-          cplx lin = s.g[m][i];
+          cplx lin = s.g[fi][i];
           if (lo >= 0) lin -= c->coef_dn[m] * s.g[lo][i];
           if (hi >= 0) lin -= c->coef_up[m] * s.g[hi][i];
-          out.g[m][i] += cplx(0.0, sgn * c->kz[iz]) * lin;
+          out.g[fi][i] += cplx(0.0, sgn * c->kz[iz]) * lin;
         }
   }
 }
@@ -384,9 +390,10 @@ static void apply_dissipation(const oracle_ctx* c, State& s, double dt) {
           rate_gk = p.eta_g * perp_rate_shape(c, iy, ix);
           if (p.eta_z > 0.0) rate_gk += p.eta_z * par_rate_shape(c, iz);
         }
-        for (int m = 0; m < c->M; ++m) {
-          double rate = rate_gk + p.nu_coll * std::pow((double)m / (double)c->M, 2.0 * p.p);   // Eq. 19
-          s.g[m][i] *= std::exp(-rate * dt);
+        for (int fi = 0; fi < c->M; ++fi) {
+          const int m = fi % c->Msp;
+          double rate = rate_gk + p.nu_coll * std::pow((double)m / (double)c->Msp, 2.0 * p.p);   // Eq. 19
+          s.g[fi][i] *= std::exp(-rate * dt);
         }
       }
 }
@@ -607,8 +614,10 @@ int oracle_create(const oracle_params* p, oracle_ctx** out) {
   if (!is_pow2(p->nx) || !is_pow2(p->ny) || !is_pow2(p->nz) || p->nx < 4 || p->ny < 4 || p->nz < 2) return -1;
   if (p->M < 0 || !(p->Lx > 0) || !(p->Ly > 0) || !(p->Lz > 0)) return -1;
   if (p->M > 0 && p->vA != 1.0) return -4;                 // Q12
+  if (p->nspecies != 1 && p->nspecies != 2) return -1;
   oracle_ctx* c = new oracle_ctx();
-  c->p = *p; c->nx = p->nx; c->ny = p->ny; c->nz = p->nz; c->M = p->M;
+  c->p = *p; c->nx = p->nx; c->ny = p->ny; c->nz = p->nz;
+  c->Msp = p->M; c->nsp = p->nspecies; c->M = p->M * p->nspecies;
   c->N = (size_t)p->nx * p->ny * p->nz;
   c->kx.resize(c->nx); c->ky.resize(c->ny); c->kz.resize(c->nz);
   c->mx.resize(c->nx); c->my.resize(c->ny); c->mz.resize(c->nz);
@@ -617,14 +626,14 @@ int oracle_create(const oracle_params* p, oracle_ctx** out) {
   for (int i = 0; i < c->nz; ++i) { c->mz[i] = signed_mode(i, c->nz); c->kz[i] = 2 * PI * c->mz[i] / p->Lz; }
   c->w[0].assign(c->N, cplx(0, 0)); c->w[1].assign(c->N, cplx(0, 0));
   c->g.assign(c->M, std::vector<cplx>(c->N, cplx(0, 0)));
-  c->coef_dn.resize(c->M + 1); c->coef_up.resize(c->M + 1);
-  for (int m = 0; m <= c->M; ++m) {
+  c->coef_dn.resize(c->Msp + 1); c->coef_up.resize(c->Msp + 1);
+  for (int m = 0; m <= c->Msp; ++m) {
     c->coef_dn[m] = std::sqrt(m / 2.0);                    // Eq. 6c
     c->coef_up[m] = std::sqrt((m + 1) / 2.0);
   }
   if (p->hermite_coeff == 1) {                             // literal Eq. 6a / 6b (Q24)
-    if (c->M > 0) c->coef_up[0] = std::sqrt(2.0);
-    if (c->M > 1) c->coef_up[1] = std::sqrt(1.5);
+    if (c->Msp > 0) c->coef_up[0] = std::sqrt(2.0);
+    if (c->Msp > 1) c->coef_up[1] = std::sqrt(1.5);
   }
   c->t = 0.0; c->step = 0; c->last_dt = 0.0;
   *out = c;

@@ -138,6 +138,7 @@ int gandalf_default_params(gandalf_params* p) {
   p->force_nperp_min = 1; p->force_nperp_max = 2; p->force_nz_max = 1;
   p->cfl = 0.3;
   p->force_g_nz = 1;
+  p->nspecies = 1;
   return GANDALF_OK;
 }
 
@@ -151,6 +152,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (p->eta < 0 || p->eta_z < 0 || p->eta_g < 0 || p->nu_coll < 0 || p->force_eps < 0) return GANDALF_ERR_INVALID;
   if (p->closure != 0 && p->closure != 1) return GANDALF_ERR_INVALID;
   if (p->force_g_amp < 0 || (p->force_g_amp > 0 && (p->M < 1 || p->force_g_nz < 1 || p->force_g_nz > p->nz / 3))) return GANDALF_ERR_INVALID;
+  if (p->nspecies != 1 && p->nspecies != 2) return GANDALF_ERR_INVALID;
   if (p->M > 0 && p->vA != 1.0) return GANDALF_ERR_UNSUPPORTED;
   if (cudaSetDevice(p->device) != cudaSuccess) { cudaGetLastError(); return GANDALF_ERR_CUDA; }
 
@@ -159,7 +161,8 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   c->p = *p;
   c->st = (cudaStream_t)p->stream;
   Dims& d = c->d;
-  d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.M = p->M; d.F = 2 + p->M;
+  d.nx = p->nx; d.ny = p->ny; d.nz = p->nz;
+  d.Msp = p->M; d.M = p->M * p->nspecies; d.F = 2 + d.M;     // d.M = number of moment FIELDS (species-major)
   d.hx = p->nx / 2 + 1;
   d.hx3 = p->nx / 3; d.hy3 = p->ny / 3; d.hz3 = p->nz / 3;
   d.Kx = d.hx3 + 1; d.Ky = 2 * d.hy3 + 1; d.Kz = 2 * d.hz3 + 1;
@@ -200,14 +203,20 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (e == cudaSuccess) e = prepare_passes_zy(d.ny, d.nz);
 
   // Hermite coupling coefficients with the closure folded in (Q10, Q23, Q24)
+  // The tables run over the moment FIELDS, species after species: dn = 0 at the first and up = 0 at the last moment of a
+  // species, so neither the sliding window of the x-pass nor the streaming stencil of P4 couples the species (Q27).
   std::vector<double> dn(M + 1, 0.0), up(M + 1, 0.0), cr(M + 1, 0.0);
-  for (int m = 0; m < M; ++m) { dn[m] = std::sqrt(m / 2.0); up[m] = std::sqrt((m + 1) / 2.0); }
-  if (p->hermite_coeff == 1) { if (M > 0) up[0] = std::sqrt(2.0); if (M > 1) up[1] = std::sqrt(1.5); }
-  if (M > 0) {
-    if (p->closure == 1 && M >= 2) dn[M - 1] += up[M - 1];   // g_M := g_{M-2}
-    up[M - 1] = 0.0;                                          // g_M := 0 otherwise
+  const int Ms = d.Msp;
+  for (int sp = 0; sp < p->nspecies; ++sp) {
+    double* dns = dn.data() + sp * Ms; double* ups = up.data() + sp * Ms; double* crs = cr.data() + sp * Ms;
+    for (int m = 0; m < Ms; ++m) { dns[m] = std::sqrt(m / 2.0); ups[m] = std::sqrt((m + 1) / 2.0); }
+    if (p->hermite_coeff == 1) { if (Ms > 0) ups[0] = std::sqrt(2.0); if (Ms > 1) ups[1] = std::sqrt(1.5); }
+    if (Ms > 0) {
+      if (p->closure == 1 && Ms >= 2) dns[Ms - 1] += ups[Ms - 1];   // g_M := g_{M-2}
+      ups[Ms - 1] = 0.0;                                            // g_M := 0 otherwise
+    }
+    for (int m = 0; m < Ms; ++m) crs[m] = p->nu_coll * std::pow((double)m / (double)Ms, 2.0 * p->p);   // Eq. 19
   }
-  for (int m = 0; m < M; ++m) cr[m] = p->nu_coll * std::pow((double)m / (double)M, 2.0 * p->p);   // Eq. 19
   // forcing pairs (Eq. 25; Q17): canonical members of each +-k pair in a fixed enumeration order
   std::vector<int> pr;
   double sumk2 = 0.0;

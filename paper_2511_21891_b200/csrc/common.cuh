@@ -14,7 +14,8 @@
 #include "fft.cuh"
 
 struct Dims {
-  int nx, ny, nz, M, F;
+  int nx, ny, nz, M, F;   // M = number of moment FIELDS (nspecies * Msp), F = 2 + M
+  int Msp;                // moments per species
   int hx;                 // nx/2+1 (boundary layout)
   int Kx, Ky, Kz;         // retained counts
   int Kxp, Kxe;           // row strides (>= Kx) of the hybrid arrays H, Gh and of E

@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
             }
           }
         } else {
-          const double skz = skz_sign * d.kz0 * c2n(cz, NZ / 3, KZ);
+          const double skz = (m < d.Msp ? skz_sign : -skz_sign) * d.kz0 * c2n(cz, NZ / 3, KZ);   // g^+ : upper, g^- : lower signs of Eq. 6
           const cd lin = cmake(a0[u].x - dn * a1[u].x - up * a2[u].x, a0[u].y - dn * a1[u].y - up * a2[u].y);
           const cd Hm = cmake(Gv.x - skz * lin.y, Gv.y + skz * lin.x);                 // + i s kz lin  (Eq. 6)
           if (mode == 0) out = Hm;

@@ -33,6 +33,7 @@ class GandalfParams(C.Structure):
         ("seed", C.c_ulonglong),
         ("cfl", C.c_double),
         ("force_g_amp", C.c_double), ("force_g_nz", C.c_int),
+        ("nspecies", C.c_int),
         ("device", C.c_int),
         ("stream", C.c_void_p),
     ]
@@ -104,7 +105,8 @@ class Gandalf:
         if stream is not None:
             p.stream = int(stream)
         self.params = p
-        self.nx, self.ny, self.nz, self.M, self.hx = nx, ny, nz, M, nx // 2 + 1
+        # self.M = number of moment FIELDS at the boundary (2M with both species: g^+ then g^-)
+        self.nx, self.ny, self.nz, self.M, self.hx = nx, ny, nz, M * max(int(p.nspecies), 1), nx // 2 + 1
         h = C.c_void_p()
         rc = lib.gandalf_create(C.byref(p), C.byref(h))
         if rc != OK:

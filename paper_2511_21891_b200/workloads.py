@@ -31,10 +31,13 @@ def config3(nx=128, ny=128, nz=64, M=32, seed=3000, eta=3e3):
     return prm, z, g, dict(dt=0.0, steps=2000, shape=(nx, ny, nz))
 
 
-def config4a(nx=256, ny=256, nz=128, M=32, seed=4000):
+def config4a(nx=256, ny=256, nz=128, M=32, seed=4000, nspecies=1):
     prm, _, _, _ = config2(8, 8, 2, M)
     z = synth.random_zeta(nx, ny, nz, seed)
     g = synth.random_g(nx, ny, nz, M, seed + 1, total=0.01)
+    if nspecies == 2:       # both slow-mode species (PAPER.md:357 layout): g^+ then g^-, 2M fields
+        prm = dict(prm, nspecies=2)
+        g = np.concatenate([g, synth.random_g(nx, ny, nz, M, seed + 2, total=0.01)])
     return prm, z, g, dict(dt=5e-4, steps=50, shape=(nx, ny, nz))
 
 

@@ -308,3 +308,21 @@ def test_repeated_runs_are_bit_identical():
         g.close()
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
     assert np.array_equal(outs[0][2], outs[1][2])
+
+
+@pytest.mark.parametrize("M,closure", [(3, 0), (4, 1), (1, 0)])
+def test_two_species_match_oracle(M, closure):
+    """nspecies = 2: g^+ and g^- share the Phi, Psi lines of the fused row pass; the species must not
+    couple through the Hermite sliding window (x-pass) or the streaming stencil (P4)."""
+    shape = (32, 32, 16)
+    prm = dict(M=M, nspecies=2, closure=closure, nu_coll=0.5, p=2.0, eta=0.5, r=2, eta_normalized=1, eta_g=0.5)
+    o, g = _pair(shape, prm)
+    z = synth.random_zeta(*shape, 6000)
+    gm = np.concatenate([synth.random_g(*shape, M, 6001, total=0.01, filled=min(2, M)),
+                         synth.random_g(*shape, M, 6002, total=0.02, filled=min(2, M))])
+    o.set_state(z, gm); g.set_state(z, gm)
+    _check_rhs(o, g)
+    o.step(5e-4, 10); g.step(5e-4, 10)
+    _check_state(o, g, TOL_10STEPS)
+    _check_history(o, g)
+    assert np.abs(g.hermite_spectrum() - o.hermite_spectrum()).max() <= 1e-10 * o.hermite_spectrum().max()

@@ -302,3 +302,31 @@ def test_p13_g0_forcing_power_support_and_restart():
     w0 = o3.energy()[5]
     o3.step(1e-3, 50)
     assert abs(o3.energy()[5] - w0) <= 1e-6 * w0          # RK2 is second order: drift ~ (kz dt)^3 per step
+
+
+# ---- P14: both slow-mode species (Q27) ------------------------------------------------
+def test_p14_two_species_equal_two_single_species_runs():
+    """Eq. 6 as printed has no g^+ / g^- coupling (Q11): a two-species run must equal two single-species runs with the
+    signs +1 and -1 that share the same Alfvenic fields -- exactly, for the RHS and after steps with every option on."""
+    nx, ny, nz, M = 16, 16, 8, 4
+    z = synth.dense_random(nx, ny, nz, 2, seed=41, decay=3.0)
+    gp = synth.dense_random(nx, ny, nz, M, seed=42, decay=3.0)
+    gm = synth.dense_random(nx, ny, nz, M, seed=43, decay=3.0)
+    kw = dict(M=M, nu_coll=0.4, p=2.0, eta=0.3, r=2, eta_normalized=1, eta_g=0.2)
+    both = Oracle(nx, ny, nz, nspecies=2, **kw)
+    both.set_state(z, np.concatenate([gp, gm]))
+    op = Oracle(nx, ny, nz, g_sign=+1, **kw); op.set_state(z, gp)
+    om = Oracle(nx, ny, nz, g_sign=-1, **kw); om.set_state(z, gm)
+    dw, dg = both.rhs()
+    dwp, dgp = op.rhs(); dwm, dgm = om.rhs()
+    assert np.array_equal(dw, dwp) and np.array_equal(dw, dwm)
+    assert np.array_equal(dg[:M], dgp) and np.array_equal(dg[M:], dgm)
+    assert not np.allclose(dgp, dgm)
+    for o in (both, op, om):
+        o.step(1e-3, 5)
+    zb, gb = both.get_state()
+    assert np.array_equal(zb, op.get_state()[0])
+    assert np.array_equal(gb[:M], op.get_state()[1]) and np.array_equal(gb[M:], om.get_state()[1])
+    # W_g is the sum over both species; the Hermite spectrum lists 2M values
+    assert abs(both.energy()[5] - (op.energy()[5] + om.energy()[5])) <= 1e-14 * both.energy()[5]
+    assert both.hermite_spectrum().shape == (2 * M,)
