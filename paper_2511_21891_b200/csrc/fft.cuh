@@ -308,6 +308,13 @@ template <int N, int s> __device__ __forceinline__ void fft_exchange_split(cd (&
   fft_gather_c<N, 1>(v, t, buf);
   __syncwarp();
 }
+// Forward transform with the split exchange and register-held stage-1 twiddles.
+template <int N, int NREG> __device__ __forceinline__ void fft_lanes_fwd_rt_split(cd (&v)[FftPlan<N>::E], int t, double* buf,
+                                                                                  const cd* __restrict__ tws, const cd (&twr)[NREG]) {
+  fft_stage_compute<N, -1, 0>(v, t, tws);
+  fft_exchange_split<N, 0>(v, t, buf);
+  fft_stage1_compute_rt<N, NREG>(v, t, tws, twr);
+}
 // Same transform with the split exchange; buf: FftGeom<N>::BUF doubles per lane group.
 template <int N, int DIR> __device__ __forceinline__ void fft_lanes_split(cd (&v)[FftPlan<N>::E], int t, double* buf,
                                                                            const cd* __restrict__ tws) {

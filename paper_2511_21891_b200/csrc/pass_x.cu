@@ -15,6 +15,9 @@
 // (Eq. 16) rides on the Elsasser part.
 #include "common.cuh"
 
+#ifndef GD_X_SPLIT
+#define GD_X_SPLIT 1
+#endif
 #ifndef GD_X_NTWR
 #define GD_X_NTWR 8
 #endif
@@ -22,14 +25,17 @@ template <int NX>
 struct XGeom {
   using G = FftGeom<NX>;
   static constexpr int T = G::T, E = G::E;
-  static constexpr int LB = NX + NX / G::PADDIV + 1;        // line buffer (FFT exchange + unpack), complex entries
+  static constexpr int SPLITX = GD_X_SPLIT;                 // 1: split (8-byte) FFT exchange: half the buffer, more stages in flight
+  static constexpr int LB = SPLITX ? (NX + NX / G::PADDIV + 2) / 2 : NX + NX / G::PADDIV + 1;   // per-group FFT exchange buffer, complex entries
   static constexpr int KXP = NX / 3 + 1;                    // retained kx count (== Dims::Kx)
   static constexpr int THREADS = 256;                       // 8 warps, one CTA per SM (it owns all 512 TMEM columns)
   static constexpr int WARPS = THREADS / 32;
   static constexpr int GROUPS = THREADS / T;                // lines per CTA: consecutive (z,y), y fastest
   static constexpr int LD = GROUPS;                         // row of a staged tile [kx][line]; line slot XOR-swizzled with kx
   static constexpr int STAGE = 2 * KXP * LD;                // one stage: the tiles of f~ and (df/dy)~ for all lines of the CTA
-  static constexpr int NST = 3;                             // stages in flight (full/empty mbarrier ring), <= 5 (the first NST-1 are Elsasser arrays)
+  static constexpr size_t SMEM_CAP = 227 * 1024;
+  static constexpr size_t smem_for(int nst) { return ((size_t)GROUPS * LB + (size_t)nst * STAGE + FftTw<NX>::COUNT) * sizeof(cd); }
+  static constexpr int NST = (SPLITX && smem_for(4) <= SMEM_CAP) ? 4 : (smem_for(3) <= SMEM_CAP ? 3 : 2);                             // stages in flight (full/empty mbarrier ring), <= 5 (the first NST-1 are Elsasser arrays)
   // stage-1 twiddles held in registers (plans with one stage-1 butterfly per lane): fewer shared-memory reads per transform
   static constexpr int NTWR = (G::S == 2 && E / FftPlan<NX>::R1 == 1) ? GD_X_NTWR : 0;
   static constexpr size_t SMEM = ((size_t)GROUPS * LB + (size_t)NST * STAGE + FftTw<NX>::COUNT) * sizeof(cd);
@@ -193,7 +199,9 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
       }
     }
 
-    if constexpr (X::NTWR > 0) fft_lanes_fwd_rt<NX, X::NTWR>(v, t, buf, tws, twr);
+    if constexpr (X::SPLITX && X::NTWR > 0) fft_lanes_fwd_rt_split<NX, X::NTWR>(v, t, reinterpret_cast<double*>(buf), tws, twr);
+    else if constexpr (X::SPLITX) fft_lanes_split<NX, -1>(v, t, reinterpret_cast<double*>(buf), tws);
+    else if constexpr (X::NTWR > 0) fft_lanes_fwd_rt<NX, X::NTWR>(v, t, buf, tws, twr);
     else fft_lanes<NX, -1>(v, t, buf, tws);
 
     if (fwd) {
