@@ -291,7 +291,7 @@ static int rhs_pipeline(gandalf_ctx* c, bool want_cfl) {
   if (!c->p.nonlinear && !want_cfl) return GANDALF_OK;
   // nonlinear == 0 with the CFL dt: Eq. 16 still needs max|grad Phi|, so P1/P2 run and the brackets are discarded
   if (want_cfl) GD_CUDA(c, timed(c, -1, 1, [&] { return launch_zero_u64(c->maxbits, c->st); }));
-  GD_CUDA(c, timed(c, KC_YINV, 1, [&] { return launch_yinv(d, c->H, c->D, c->twy, c->st); }));
+  GD_CUDA(c, timed(c, KC_YINV, d.M > 0 ? 2 : 1, [&] { return launch_yinv(d, c->H, c->D, c->twy, c->st); }));
   GD_CUDA(c, timed(c, KC_XPASS, 1, [&] {
     return launch_xpass(d, c->D, c->E, c->twx, c->cdn, c->cup, want_cfl ? c->maxbits : nullptr, c->st, false);
   }));

@@ -240,7 +240,7 @@ template <int NY> struct YInvGeom {
   static constexpr int XB = (FftGeom<NY>::S > 1 ? FftGeom<NY>::BUF : 0) + 2;            // doubles per group
   static constexpr size_t SMEM = ((size_t)FftTw<NY>::COUNT + (size_t)KYMAX * LD) * sizeof(cd) + (size_t)Y::GROUPS * XB * sizeof(double);
 };
-template <int NY>
+template <int NY, bool ELS>   // ELS: the Elsasser sources s = 0, 1 (four outputs each, potentials first); else s = 2 + m
 __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Dims d, const cd* __restrict__ H, cd* __restrict__ D,
                                                         const cd* __restrict__ tw, int ncb, int nitems) {
   using Y = YGeom<NY>;
@@ -257,7 +257,7 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Di
   const cd* tws = smem;
   auto issue = [&](int item) {                   // all threads: one bulk copy per tile row (row = retained ky)
     const int cb = item % ncb, sz = item / ncb;
-    const int z = sz % d.nz, s = sz / d.nz;
+    const int z = sz % d.nz, s = sz / d.nz + (ELS ? 0 : 2);
     const int cx0 = cb * Y::GROUPS;
     const int ncol = min(Y::GROUPS, d.Kx - cx0);
     if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(d.Ky * ncol * sizeof(cd)));
@@ -271,12 +271,12 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Di
   const double kyt = d.ky0 * t, kyT = d.ky0 * T;
   while (item < nitems) {
     const int cb = item % ncb, sz = item / ncb;
-    const int z = sz % d.nz, s = sz / d.nz;
+    const int z = sz % d.nz, s = sz / d.nz + (ELS ? 0 : 2);
     const int cx = cb * Y::GROUPS + grp;
     const bool active = cx < d.Kx;
     const double kx = d.kx0 * cx;
     const int cxa = active ? cx : 0;
-    const int rounds = (s < 2) ? 4 : 2;
+    constexpr int rounds = ELS ? 4 : 2;
     // D[a][line block][kx][xl], line = z*ny + y, slot (line % xl) ^ (kx % xl): the lanes of a group fill whole aligned
     // runs of one block row.  Offsets of element q: off0 + q*ostr when a block row holds at most T lines.
     const int lineb = z * NY + t;
@@ -288,9 +288,9 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Di
     phase ^= 1u;
     item += gridDim.x;
     for (int r = 0; r < rounds; ++r) {
-      const bool pot = (s < 2) && (r < 2);       // rounds 0,1 of an Elsasser source: the potential xi = -w/kperp^2
+      const bool pot = ELS && (r < 2);           // rounds 0,1 of an Elsasser source: the potential xi = -w/kperp^2
       const int which = r & 1;                   // 0: U, 1: V
-      const int a = (s < 2 ? (pot ? 2 * s : 4 + 2 * s) : 8 + 2 * (s - 2)) + which;
+      const int a = (ELS ? (pot ? 2 * s : 4 + 2 * s) : 8 + 2 * (s - 2)) + which;
       cd v[E];
 #pragma unroll
       for (int q = 0; q < E; ++q) {
@@ -494,8 +494,10 @@ cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStr
 #define YICASE(NN)                                                                                         \
   {                                                                                                        \
     const int ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;                                    \
-    const int nitems = d.F * d.nz * ncb;                                                                   \
-    k_yinv<NN><<<nitems < YGeom<NN>::CTAS * g_num_sms ? nitems : YGeom<NN>::CTAS * g_num_sms, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, nitems); \
+    const int cap = YGeom<NN>::CTAS * g_num_sms;                                                           \
+    const int ne = 2 * d.nz * ncb, nm = d.M * d.nz * ncb;                                                  \
+    k_yinv<NN, true><<<ne < cap ? ne : cap, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, ne);                 \
+    if (nm > 0) k_yinv<NN, false><<<nm < cap ? nm : cap, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, nm);    \
   }
   GD_DISPATCH(d.ny, YICASE)
   return cudaGetLastError();
@@ -529,7 +531,9 @@ cudaError_t prepare_passes_zy(int ny, int nz) {
   GD_DISPATCH(nz, ZPCASE)
 #define YPCASE(NN)                                                                                                         \
   {                                                                                                                        \
-    cudaError_t e = cudaFuncSetAttribute(k_yinv<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YInvGeom<NN>::SMEM); \
+    cudaError_t e = cudaFuncSetAttribute(k_yinv<NN, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YInvGeom<NN>::SMEM); \
+    if (e != cudaSuccess) return e;                                                                                        \
+    e = cudaFuncSetAttribute(k_yinv<NN, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YInvGeom<NN>::SMEM);      \
     if (e != cudaSuccess) return e;                                                                                        \
     e = cudaFuncSetAttribute(k_yfwd_pair<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YGeom<NN>::SMEM);          \
     if (e != cudaSuccess) return e;                                                                                        \

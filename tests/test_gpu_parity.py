@@ -231,8 +231,8 @@ def test_launch_count_and_kernel_timing():
     g.kernel_timing(True)
     g.step(run["dt"], 2)
     kt = g.kernel_times()
-    # per step: 2 x (P1, P2, P3 pair + P3 moments, P4) + dt + factor tables + 2 energy kernels
-    assert g.launch_count() - n0 == 2 * 14
+    # per step: 2 x (P1 Elsasser + P1 moments, P2, P3 pair + P3 moments, P4) + dt + factor tables + 2 energy kernels
+    assert g.launch_count() - n0 == 2 * 16
     assert kt["x_pass_P2"][1] == 4 and kt["x_pass_P2"][0] > 0
     assert kt["z_step_P4"][1] == 4 and kt["z_step_P4"][0] > 0
 
