@@ -78,8 +78,8 @@ template <int NZ> struct ZStepGeom {
   static constexpr int REGION = XCH > KZ * LD ? XCH : KZ * LD;
   static constexpr size_t SMEM = ((size_t)REGION + FftTw<NZ>::COUNT) * sizeof(cd);
 };
-template <int NZ>
-__global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if_variant, double skz_sign, const cd* __restrict__ Gh,
+template <int NZ, int MODE>   // MODE 0 / 1 / 2 = RHS only / predictor / corrector + dissipation (compile time: fewer registers)
+__global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, double skz_sign, const cd* __restrict__ Gh,
                                                       const cd* __restrict__ Wn, const cd* __restrict__ Ws, cd* __restrict__ Wout,
                                                       cd* __restrict__ Hout, const double* __restrict__ scal,
                                                       const double* __restrict__ cdn, const double* __restrict__ cup,
@@ -87,6 +87,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int mode, int if
                                                       const double* __restrict__ tabp, const cd* __restrict__ tw) {
   using G = FftGeom<NZ>;
   using Z = ZStepGeom<NZ>;
+  constexpr int mode = MODE;
   constexpr int T = G::T, E = G::E;
   constexpr int GROUPS = Z::GROUPS, KZ = Z::KZ, LD = Z::LD;
   extern __shared__ cd smem[];
@@ -485,8 +486,12 @@ cudaError_t launch_zstep(const Dims& d, int mode, int if_variant, int g_sign, co
                          const double* tabp, const cd* tw, cudaStream_t st) {
   const long long ncols = (long long)d.Ky * d.Kx;
 #define ZSCASE(NN)                                                                                               \
-  k_zstep<NN><<<fft_blocks<NN>(ncols) * d.F, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, mode, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, \
-                                                                             Hout, scal, cdn, cup, collfac, tabz, tabp, tw);
+  {                                                                                                              \
+    const int nb = fft_blocks<NN>(ncols) * d.F;                                                                  \
+    if (mode == 0) k_zstep<NN, 0><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
+    else if (mode == 1) k_zstep<NN, 1><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
+    else k_zstep<NN, 2><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
+  }
   GD_DISPATCH(d.nz, ZSCASE)
   return cudaGetLastError();
 }
@@ -525,7 +530,11 @@ cudaError_t prepare_passes_zy(int ny, int nz) {
     if (e != cudaSuccess) return e;                                                                                        \
     e = cudaFuncSetAttribute(k_zfft<NN, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<NN>());             \
     if (e != cudaSuccess) return e;                                                                                        \
-    e = cudaFuncSetAttribute(k_zstep<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);           \
+    e = cudaFuncSetAttribute(k_zstep<NN, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);        \
+    if (e != cudaSuccess) return e;                                                                                        \
+    e = cudaFuncSetAttribute(k_zstep<NN, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);        \
+    if (e != cudaSuccess) return e;                                                                                        \
+    e = cudaFuncSetAttribute(k_zstep<NN, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);        \
     if (e != cudaSuccess) return e;                                                                                        \
   }
   GD_DISPATCH(nz, ZPCASE)
