@@ -25,7 +25,8 @@ template <int NX>
 struct XGeom {
   using G = FftGeom<NX>;
   static constexpr int T = G::T, E = G::E;
-  static constexpr int SPLITX = GD_X_SPLIT;                 // 1: split (8-byte) FFT exchange: half the buffer, more stages in flight
+  static constexpr int SPLITX = (GD_X_SPLIT && G::S == 2) ? 1 : 0;   // split (8-byte) FFT exchange for the two-stage plans: half the buffer,
+                                                                     // one more stage in flight (three-stage plans would pay two split exchanges)
   static constexpr int LB = SPLITX ? (NX + NX / G::PADDIV + 2) / 2 : NX + NX / G::PADDIV + 1;   // per-group FFT exchange buffer, complex entries
   static constexpr int KXP = NX / 3 + 1;                    // retained kx count (== Dims::Kx)
   static constexpr int THREADS = 256;                       // 8 warps, one CTA per SM (it owns all 512 TMEM columns)

@@ -216,11 +216,13 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
 // Geometry of the y passes: THREADS lanes per CTA = GROUPS lane groups = GROUPS adjacent columns of ONE array,
 // so a CTA covers GROUPS*16 B contiguous per row (256 B at ny = 256: strided row segments narrower than that lose
 // HBM efficiency, profiles/r01_stride_microbench.md) and two CTAs fit on an SM (<= 128 registers per lane).
-template <int NY> struct YGeom {
+template <int NY, bool PAIR = false> struct YGeom {
   using G = FftGeom<NY>;
   static constexpr int T = G::T, E = G::E;
-  static constexpr int THREADS = (T >= 32) ? 512 : 256;      // ny = 512 (one warp per transform): 16 warps so that a tile is still 16 columns wide
-  static constexpr int CTAS = (THREADS == 512) ? 1 : 2;      // resident CTAs per SM
+  // ny = 512 (one warp per transform): 12 warps = 12 columns with 170 registers per lane (no spills); the pair kernel keeps
+  // 16 warps = 2 x 8 columns
+  static constexpr int THREADS = (T >= 32) ? (PAIR ? 512 : 384) : 256;
+  static constexpr int CTAS = (THREADS > 256) ? 1 : 2;       // resident CTAs per SM
   static constexpr int GROUPS = THREADS / T;                 // columns per CTA
   static constexpr int YBUF = (G::S > 1 ? G::BUF : NY) + 1;  // per-group buffer (FFT exchange; A/B hand-over in P3)
   static constexpr int REGION = (GROUPS * YBUF > NY * (GROUPS + 1)) ? GROUPS * YBUF : NY * (GROUPS + 1);   // also holds a padded [NY][GROUPS] tile
@@ -310,7 +312,7 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Di
           if (T * q <= HY3 || T * q + T - 1 >= NY - HY3) {      // compile-time: some lane of this q holds a retained ky
             const double ky = fma(kyT, (double)(q < E / 2 ? q : q - E), kyt);     // ky0 * signed mode number of t + T q
             double ar = skx, ai = ky;
-            if (pot) { const double k2 = kx * kx + ky * ky; const double f = k2 > 0.0 ? -1.0 / k2 : 0.0; ar *= f; ai *= f; }   // xi = -w/kperp^2
+            if (pot) { const double k2 = kx * kx + ky * ky; const double f = k2 > 0.0 ? -__drcp_rn(k2) : 0.0; ar *= f; ai *= f; }   // xi = -w/kperp^2 (correctly rounded reciprocal == -1.0/k2)
             v[q] = cmake(ar * v[q].x - ai * v[q].y, ar * v[q].y + ai * v[q].x);
           }
         }
@@ -342,9 +344,9 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Di
 // columns, hand the results over through shared memory and form N+- = -1/2 A -+ 1/2 kperp^2 B  (Eq. 1 with
 // Eq. 11).  The FFT exchange buffers alias the tile once every lane holds its column.
 template <int NY>
-__global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
+__global__ void __launch_bounds__(YGeom<NY, true>::THREADS, YGeom<NY, true>::CTAS) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
                                                              const cd* __restrict__ tw, int ncb) {
-  using Y = YGeom<NY>;
+  using Y = YGeom<NY, true>;
   using G = FftGeom<NY>;
   constexpr int T = G::T, E = G::E;
   constexpr int HG = Y::GROUPS / 2;
@@ -380,7 +382,7 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yfwd_pa
 #pragma unroll
   for (int q = 0; q < E; ++q) buf[t + T * q] = v[q];
   __syncthreads();
-  const cd* sib = tile + (size_t)(grp ^ HG) * Y::YBUF;
+  const cd* sib = tile + (size_t)(grp < HG ? grp + HG : grp - HG) * Y::YBUF;
   const double kx = d.kx0 * cx;
   if (active) {
     cd* dst = Gh + (size_t)which * d.PH + (size_t)z * d.Ky * d.Kxp + cx;
@@ -510,9 +512,9 @@ cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStr
 cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, cudaStream_t st) {
 #define YFCASE(NN)                                                                                         \
   {                                                                                                        \
-    constexpr int HG = YGeom<NN>::GROUPS / 2;                                                              \
+    constexpr int HG = YGeom<NN, true>::GROUPS / 2;                                                              \
     const int ncb2 = (d.Kx + HG - 1) / HG, ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;       \
-    k_yfwd_pair<NN><<<d.nz * ncb2, YGeom<NN>::THREADS, YGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb2);               \
+    k_yfwd_pair<NN><<<d.nz * ncb2, YGeom<NN, true>::THREADS, YGeom<NN, true>::SMEM, st>>>(d, E, Gh, tw, ncb2);               \
     const int nitems = d.M * d.nz * ncb;                                                                   \
     if (d.M > 0) k_yfwd<NN><<<nitems < YGeom<NN>::CTAS * g_num_sms ? nitems : YGeom<NN>::CTAS * g_num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, nitems); \
   }
@@ -544,7 +546,7 @@ cudaError_t prepare_passes_zy(int ny, int nz) {
     if (e != cudaSuccess) return e;                                                                                        \
     e = cudaFuncSetAttribute(k_yinv<NN, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YInvGeom<NN>::SMEM);      \
     if (e != cudaSuccess) return e;                                                                                        \
-    e = cudaFuncSetAttribute(k_yfwd_pair<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YGeom<NN>::SMEM);          \
+    e = cudaFuncSetAttribute(k_yfwd_pair<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YGeom<NN, true>::SMEM);          \
     if (e != cudaSuccess) return e;                                                                                        \
     e = cudaFuncSetAttribute(k_yfwd<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YFwdGeom<NN>::SMEM);            \
     if (e != cudaSuccess) return e;                                                                                        \
