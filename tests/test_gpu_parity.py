@@ -326,3 +326,17 @@ def test_two_species_match_oracle(M, closure):
     _check_state(o, g, TOL_10STEPS)
     _check_history(o, g)
     assert np.abs(g.hermite_spectrum() - o.hermite_spectrum()).max() <= 1e-10 * o.hermite_spectrum().max()
+
+
+def test_config3_full_size_first_steps():
+    """BASELINE config 3 at its full size (128x128x64, M=32, forcing, CFL dt, k_perp^8 and k_z^8 hyperdissipation): the first
+    two steps against the oracle on the same grid (the oracle needs ~15-30 s per step there; Q20)."""
+    prm, z, gm, run = config3()
+    assert run["shape"] == (128, 128, 64) and prm["M"] == 32
+    o, g = _pair(run["shape"], prm)
+    o.set_state(z, gm); g.set_state(z, gm)
+    o.step(0.0, 2); g.step(0.0, 2)
+    to, tg = o.time(), g.time()
+    assert abs(tg[0] - to[0]) <= 1e-12 * to[0] and abs(tg[2] - to[2]) <= 1e-12 * to[2]
+    _check_state(o, g, TOL_10STEPS)
+    _check_history(o, g)
