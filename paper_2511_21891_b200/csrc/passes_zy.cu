@@ -216,17 +216,13 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
 // Geometry of the y passes: THREADS lanes per CTA = GROUPS lane groups = GROUPS adjacent columns of ONE array,
 // so a CTA covers GROUPS*16 B contiguous per row (256 B at ny = 256: strided row segments narrower than that lose
 // HBM efficiency, profiles/r01_stride_microbench.md) and two CTAs fit on an SM (<= 128 registers per lane).
-template <int NY, bool PAIR = false> struct YGeom {
+template <int NY> struct YGeom {
   using G = FftGeom<NY>;
   static constexpr int T = G::T, E = G::E;
-  // ny = 512 (one warp per transform): 12 warps = 12 columns with 170 registers per lane (no spills); the pair kernel keeps
-  // 16 warps = 2 x 8 columns
-  static constexpr int THREADS = (T >= 32) ? (PAIR ? 512 : 384) : 256;
+  // ny = 512 (one warp per transform): 12 warps = 12 columns with 170 registers per lane (no spills)
+  static constexpr int THREADS = (T >= 32) ? 384 : 256;
   static constexpr int CTAS = (THREADS > 256) ? 1 : 2;       // resident CTAs per SM
   static constexpr int GROUPS = THREADS / T;                 // columns per CTA
-  static constexpr int YBUF = (G::S > 1 ? G::BUF : NY) + 1;  // per-group buffer (FFT exchange; A/B hand-over in P3)
-  static constexpr int REGION = (GROUPS * YBUF > NY * (GROUPS + 1)) ? GROUPS * YBUF : NY * (GROUPS + 1);   // also holds a padded [NY][GROUPS] tile
-  static constexpr size_t SMEM = ((size_t)REGION + FftTw<NY>::COUNT) * sizeof(cd);
 };
 
 // P1.  Persistent CTAs over the work items (source field s, z, block of GROUPS columns).  Sources: s = 0,1 -> w+, w-;
@@ -340,65 +336,14 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Di
 // completion) into a padded shared-memory tile, so the global side moves whole row segments and the lanes then read
 // their own column conflict-free.
 //
-// k_yfwd_pair: work item (z, block of GROUPS/2 columns): the two halves of the CTA transform A and B of the same
-// columns, hand the results over through shared memory and form N+- = -1/2 A -+ 1/2 kperp^2 B  (Eq. 1 with
-// Eq. 11).  The FFT exchange buffers alias the tile once every lane holds its column.
+// k_yfwd_pair: persistent CTAs over the work items (z, block of GROUPS columns).  Every lane group transforms column A,
+// keeps it in registers, transforms column B of the same kx and forms N+- = -1/2 A -+ 1/2 kperp^2 B  (Eq. 1 with
+// Eq. 11).  One tile buffer: B's tile is in flight during A's transform, the next item's A tile
+// during B's transform.  (Geometry and shared-memory layout of k_yfwd below.)
+template <int NY> struct YFwdGeom;
 template <int NY>
-__global__ void __launch_bounds__(YGeom<NY, true>::THREADS, YGeom<NY, true>::CTAS) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
-                                                             const cd* __restrict__ tw, int ncb) {
-  using Y = YGeom<NY, true>;
-  using G = FftGeom<NY>;
-  constexpr int T = G::T, E = G::E;
-  constexpr int HG = Y::GROUPS / 2;
-  constexpr int LD = Y::GROUPS + 1;              // padded tile row (complex entries)
-  extern __shared__ cd smem[];
-  __shared__ unsigned long long bar;
-  const int grp = threadIdx.x / T, t = threadIdx.x % T;
-  cd* tile = smem + FftTw<NY>::COUNT;
-  cd* buf = tile + (size_t)grp * Y::YBUF;
-  const int cb = blockIdx.x % ncb, z = blockIdx.x / ncb;
-  const int which = grp / HG;
-  const int cx0 = cb * HG;
-  const int cx = cx0 + grp % HG;
-  const bool active = cx < d.Kx;
-  const int ncol = min(HG, d.Kx - cx0);          // columns of this block that exist
-  if (threadIdx.x == 0) mbar_init(&bar, 1);
-  fft_load_table<NY>(smem, tw);                  // ends with __syncthreads()
-  if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(NY * ncol * 2 * sizeof(cd)));
-  for (int r = threadIdx.x; r < NY; r += Y::THREADS) {
-    const cd* src = Ein + ((size_t)z * NY + r) * d.Kxe + cx0;
-    bulk_g2s(tile + (size_t)r * LD, src, (unsigned)(ncol * sizeof(cd)), &bar);
-    bulk_g2s(tile + (size_t)r * LD + HG, src + d.PE, (unsigned)(ncol * sizeof(cd)), &bar);
-  }
-  const cd* tws = smem;
-  mbar_wait(&bar, 0);
-  cd v[E];
-#pragma unroll
-  for (int q = 0; q < E; ++q) v[q] = active ? tile[(size_t)(t + T * q) * LD + grp] : cmake(0.0, 0.0);
-  __syncthreads();                               // tile consumed: the exchange buffers may overwrite it
-  fft_lanes<NY, -1>(v, t, buf, tws);
-  // hand-over: every group publishes its transform, the sibling (other array, same column) reads it
-  __syncwarp();
-#pragma unroll
-  for (int q = 0; q < E; ++q) buf[t + T * q] = v[q];
-  __syncthreads();
-  const cd* sib = tile + (size_t)(grp < HG ? grp + HG : grp - HG) * Y::YBUF;
-  const double kx = d.kx0 * cx;
-  if (active) {
-    cd* dst = Gh + (size_t)which * d.PH + (size_t)z * d.Ky * d.Kxp + cx;
-#pragma unroll
-    for (int q = 0; q < E; ++q) {
-      const int cy = fft2c(t + T * q, NY, d.hy3, d.Ky);
-      if (cy >= 0) {
-        const cd o = sib[t + T * q];
-        const cd A = which ? o : v[q], B = which ? v[q] : o;
-        const double ky = d.ky0 * fft2n(t + T * q, NY);
-        const double hk2 = (which ? 0.5 : -0.5) * (kx * kx + ky * ky);
-        st_cd(dst + (size_t)cy * d.Kxp, cmake(-0.5 * A.x + hk2 * B.x, -0.5 * A.y + hk2 * B.y));
-      }
-    }
-  }
-}
+__global__ void __launch_bounds__(YGeom<NY>::THREADS, 1) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
+                                                                     const cd* __restrict__ tw, int ncb, int nitems);
 
 // k_yfwd: persistent CTAs over the work items (array a >= 2, z, block of GROUPS columns).  The exchange uses its
 // own (split, 8-byte) buffers, so the NEXT item's tile is in flight while the current one is transformed and stored.
@@ -461,6 +406,71 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yfwd(Di
   }
 }
 
+template <int NY>
+__global__ void __launch_bounds__(YGeom<NY>::THREADS, 1) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
+                                                                     const cd* __restrict__ tw, int ncb, int nitems) {
+  using Y = YGeom<NY>;
+  using G = FftGeom<NY>;
+  using YF = YFwdGeom<NY>;
+  constexpr int T = G::T, E = G::E, LD = YF::LD;
+  constexpr int HY3 = NY / 3, KY = 2 * HY3 + 1;   // == d.hy3, d.Ky
+  extern __shared__ cd smem[];
+  __shared__ unsigned long long bar;
+  const int grp = threadIdx.x / T, t = threadIdx.x % T;
+  cd* tile = smem + FftTw<NY>::COUNT;
+  double* xbuf = reinterpret_cast<double*>(tile + (size_t)NY * LD) + (size_t)grp * YF::XB;
+  if (threadIdx.x == 0) mbar_init(&bar, 1);
+  fft_load_table<NY>(smem, tw);                  // ends with __syncthreads()
+  const cd* tws = smem;
+  auto issue = [&](int item, int arr) {          // all threads: one bulk copy per tile row of E array `arr` (0: A, 1: B)
+    const int cb = item % ncb, z = item / ncb;
+    const int cx0 = cb * Y::GROUPS;
+    const int ncol = min(Y::GROUPS, d.Kx - cx0);
+    if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(NY * ncol * sizeof(cd)));
+    for (int r = threadIdx.x; r < NY; r += Y::THREADS)
+      bulk_g2s(tile + (size_t)r * LD, Ein + (size_t)arr * d.PE + ((size_t)z * NY + r) * d.Kxe + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
+  };
+  int item = blockIdx.x;
+  if (item < nitems) issue(item, 0);
+  unsigned phase = 0;
+  while (item < nitems) {
+    const int cb = item % ncb, z = item / ncb;
+    const int cx = cb * Y::GROUPS + grp;
+    const bool active = cx < d.Kx;
+    cd va[E], v[E];
+    mbar_wait(&bar, phase);
+    phase ^= 1u;
+#pragma unroll
+    for (int q = 0; q < E; ++q) va[q] = active ? tile[(t + T * q) * LD + grp] : cmake(0.0, 0.0);
+    __syncthreads();                             // A tile consumed by every lane
+    issue(item, 1);                              // B's tile travels during A's transform
+    fft_lanes_split<NY, -1>(va, t, xbuf, tws);
+    mbar_wait(&bar, phase);
+    phase ^= 1u;
+#pragma unroll
+    for (int q = 0; q < E; ++q) v[q] = active ? tile[(t + T * q) * LD + grp] : cmake(0.0, 0.0);
+    __syncthreads();                             // B tile consumed
+    item += gridDim.x;
+    if (item < nitems) issue(item, 0);           // the next item's A tile travels during B's transform and the stores
+    fft_lanes_split<NY, -1>(v, t, xbuf, tws);
+    if (active) {
+      const double kx = d.kx0 * cx;
+      cd* dp = Gh + (size_t)z * KY * d.Kxp + cx;
+      cd* dm = dp + d.PH;
+#pragma unroll
+      for (int q = 0; q < E; ++q) {
+        const int cy = fft2c(t + T * q, NY, HY3, KY);
+        if (cy >= 0) {
+          const double ky = d.ky0 * fft2n(t + T * q, NY);
+          const double hk2 = 0.5 * (kx * kx + ky * ky);
+          st_cd(dp + cy * d.Kxp, cmake(-0.5 * va[q].x - hk2 * v[q].x, -0.5 * va[q].y - hk2 * v[q].y));
+          st_cd(dm + cy * d.Kxp, cmake(-0.5 * va[q].x + hk2 * v[q].x, -0.5 * va[q].y + hk2 * v[q].y));
+        }
+      }
+    }
+  }
+}
+
 static int g_num_sms = 148;   // persistent kernels launch 2 CTAs per SM
 
 // ---- launchers ------------------------------------------------------------------------------------
@@ -512,9 +522,9 @@ cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStr
 cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, cudaStream_t st) {
 #define YFCASE(NN)                                                                                         \
   {                                                                                                        \
-    constexpr int HG = YGeom<NN, true>::GROUPS / 2;                                                              \
-    const int ncb2 = (d.Kx + HG - 1) / HG, ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;       \
-    k_yfwd_pair<NN><<<d.nz * ncb2, YGeom<NN, true>::THREADS, YGeom<NN, true>::SMEM, st>>>(d, E, Gh, tw, ncb2);               \
+    const int ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;                                    \
+    const int np = d.nz * ncb;                                                                             \
+    k_yfwd_pair<NN><<<np < g_num_sms ? np : g_num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, np);   \
     const int nitems = d.M * d.nz * ncb;                                                                   \
     if (d.M > 0) k_yfwd<NN><<<nitems < YGeom<NN>::CTAS * g_num_sms ? nitems : YGeom<NN>::CTAS * g_num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, nitems); \
   }
@@ -546,7 +556,7 @@ cudaError_t prepare_passes_zy(int ny, int nz) {
     if (e != cudaSuccess) return e;                                                                                        \
     e = cudaFuncSetAttribute(k_yinv<NN, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YInvGeom<NN>::SMEM);      \
     if (e != cudaSuccess) return e;                                                                                        \
-    e = cudaFuncSetAttribute(k_yfwd_pair<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YGeom<NN, true>::SMEM);          \
+    e = cudaFuncSetAttribute(k_yfwd_pair<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YFwdGeom<NN>::SMEM);             \
     if (e != cudaSuccess) return e;                                                                                        \
     e = cudaFuncSetAttribute(k_yfwd<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)YFwdGeom<NN>::SMEM);            \
     if (e != cudaSuccess) return e;                                                                                        \
