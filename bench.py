@@ -31,6 +31,10 @@ WORKLOADS = {
     "4a2": ("config4a", dict(nx=256, ny=256, nz=128, M=32, nspecies=2)),     # both species: 2 + 64 fields
     "4b": ("config4b", dict(nx=512, ny=512, nz=256)),
     "2": ("config2", dict(nx=64, ny=64, nz=32, M=16)),
+    # driven turbulence; e.g. --steps 79990 --warmup 10 reaches the statistically steady state (t ~ 17).  cfl = 0.03, not
+    # BASELINE's 0.3: with C = 0.3 on max|grad Phi| alone (Eq. 16) the explicit RK2 of the Hermite couplings
+    # sqrt(m/2){Psi, g_m+-1} is unstable at M = 32 -- oracle and GPU blow up identically (Q28)
+    "3": ("config3", dict(nx=128, ny=128, nz=64, M=32)),
     "0": ("config0", dict(nx=32, ny=32, nz=16)),
 }
 
@@ -41,6 +45,8 @@ def make_workload(name, **override):
     kw = dict(kw)
     kw.update(override)
     prm, z, g, run = getattr(cases, fn)(**kw)
+    if name == "3":
+        prm = dict(prm, cfl=0.03)
     return prm, z, g, run
 
 
@@ -337,6 +343,14 @@ def main():
     ms = max_over_ranks(ms, world)
     hist = sim.energy_history()
     assert hist.shape[0] == args.warmup + args.steps and np.isfinite(hist).all()
+    spectrum = None
+    if args.workload == "3":      # BASELINE config 3 "reports the k_perp energy spectrum" (Eq. 26; unpinned statistics)
+        sp = sim.kperp_spectrum(44)
+        ks = np.arange(44)
+        sel = (ks >= 2) & (ks <= 12) & (sp > 0)
+        slope = float(np.polyfit(np.log(ks[sel]), np.log(sp[sel]), 1)[0]) if sel.sum() >= 3 else None
+        spectrum = {"E_kperp": [float(x) for x in sp], "fit_range": [2, 12], "slope": slope, "paper_slope": -5.0 / 3.0,
+                    "t_end": float(hist[-1, 0]), "mean_dt": float(hist[-1, 0] / hist.shape[0])}
     steps_per_s = whole_job_steps_per_s(ms, args.steps, world)
 
     # ---- end to end through the C ABI with HOST (pinned) buffers: H2D state, one step, D2H energies
@@ -414,7 +428,7 @@ def main():
             "config": {"workload": wl, "grid": list(shape), "M": M, "dt": dt, "fields": F, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "no flush needed: every kernel streams inputs far larger than the 126 MB L2 (working set per step > 9 GB at 4a)"},
             "steps_per_s": steps_per_s, "grid_point_moments_per_s": steps_per_s * shape[0] * shape[1] * shape[2] * F,
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cufft_comparison": cufft,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cufft_comparison": cufft, "kperp_spectrum": spectrum,
             "final_energy": {"E_A": float(hist[-1, 1]), "W_g": float(hist[-1, 6])},
         }
         print(json.dumps(line), flush=True)
