@@ -340,3 +340,20 @@ def test_config3_full_size_first_steps():
     assert abs(tg[0] - to[0]) <= 1e-12 * to[0] and abs(tg[2] - to[2]) <= 1e-12 * to[2]
     _check_state(o, g, TOL_10STEPS)
     _check_history(o, g)
+
+
+def test_finding_q28_advective_cfl_is_not_sufficient_with_moments():
+    """DESIGN.md Q28: with C = 0.3 on max|grad Phi| alone (Eq. 16) the explicit RK2 of the Hermite couplings
+    sqrt(m/2){Psi, g_m+-1} is unstable once enough moments are kept (the oracle blows up with the same digits); C = 0.03
+    ~ 0.3/(1+sqrt(2M)) is stable.  64x64x32, M = 16, config 3's forcing and dissipation."""
+    from paper_2511_21891_b200.gandalf import Gandalf
+    prm, z, gm, run = config3(64, 64, 32, 16)
+    g = Gandalf(*run["shape"], **prm)
+    g.set_state(z, gm)
+    g.step(0.0, 40)
+    assert g.energy_history()[-1, 6] > 1e10            # W_g (2.4720e+24 in the oracle and on the GPU)
+    g2 = Gandalf(*run["shape"], **dict(prm, cfl=0.03))
+    g2.set_state(z, gm)
+    g2.step(0.0, 400)
+    h = g2.energy_history()
+    assert np.isfinite(h).all() and h[-1, 6] < 0.05 and 1.0 < h[-1, 1] < 3.0
