@@ -33,7 +33,7 @@ struct XGeom {
   static constexpr int WARPS = THREADS / 32;
   static constexpr int GROUPS = THREADS / T;                // lines per CTA: consecutive (z,y), y fastest
   static constexpr int LD = GROUPS;                         // row of a staged tile [kx][line]; line slot XOR-swizzled with kx
-  static constexpr int STAGE = 2 * KXP * LD;                // one stage: the tiles of f~ and (df/dy)~ for all lines of the CTA
+  static constexpr int STAGE = 2 * KXP * LD;                // one stage: the tiles of U and V (P1) for all lines of the CTA
   static constexpr size_t SMEM_CAP = 227 * 1024;
   static constexpr size_t smem_for(int nst) { return ((size_t)GROUPS * LB + (size_t)nst * STAGE + FftTw<NX>::COUNT) * sizeof(cd); }
   static constexpr int NST = (SPLITX && smem_for(4) <= SMEM_CAP) ? 4 : (smem_for(3) <= SMEM_CAP ? 3 : 2);                             // stages in flight (full/empty mbarrier ring), <= 5 (the first NST-1 are Elsasser arrays)
@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   const int line = blockIdx.x * X::GROUPS + grp;
   cd* buf = smem + FftTw<NX>::COUNT + (size_t)grp * X::LB;
-  cd* stages = smem + FftTw<NX>::COUNT + (size_t)X::GROUPS * X::LB;   // NST x [2][KX][LD]: f~ and (df/dy)~ tiles, [kx][line]
+  cd* stages = smem + FftTw<NX>::COUNT + (size_t)X::GROUPS * X::LB;   // NST x [2][KX][LD]: U and V tiles, [kx][line]
   __shared__ unsigned s_tmem_base;
   __shared__ unsigned long long s_full[X::NST], s_empty[X::NST];
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);     // warp-uniform for the compiler (uniform registers)
