@@ -76,6 +76,7 @@ template <int NZ> struct ZStepGeom {
   static constexpr int LD = GROUPS + 1;                      // padded row of the [kz][column] tile
   static constexpr int XCH = GROUPS * (G::BUF + 1);          // FFT exchange buffers (alias the tile)
   static constexpr int REGION = XCH > KZ * LD ? XCH : KZ * LD;
+  static constexpr bool TMA_IN = (NZ * LD <= REGION);        // the staged [nz][GROUPS] tile of Gh fits in the region
   static constexpr size_t SMEM = ((size_t)REGION + FftTw<NZ>::COUNT) * sizeof(cd);
 };
 template <int NZ, int MODE>   // MODE 0 / 1 / 2 = RHS only / predictor / corrector + dissipation (compile time: fewer registers)
@@ -91,6 +92,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
   constexpr int T = G::T, E = G::E;
   constexpr int GROUPS = Z::GROUPS, KZ = Z::KZ, LD = Z::LD;
   extern __shared__ cd smem[];
+  __shared__ unsigned long long bar;
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   cd* tile = smem + FftTw<NZ>::COUNT;                          // [KZ][LD], aliases the exchange buffers
   cd* buf = tile + (size_t)grp * (G::BUF + 1);
@@ -111,10 +113,25 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
   // 1. forward z transform of the bracket term, retained kz -> tile (scaled by 1/N)
   if (Gh != nullptr) {
     cd v[E];
-    const cd* src = Gh + (size_t)f * d.PH + colH;
+    if (Z::TMA_IN && d.Kxp == d.Kx) {
+      // (unpadded hybrid rows: the block's columns are contiguous in memory even across a ky row end)  The [nz][GROUPS]
+      // tile comes by one bulk async copy per z row (TMA engine) into the region the exchange buffers will reuse.
+      const int ncolv = min(GROUPS, plane - col0);
+      if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_arrive_expect_tx(&bar, (unsigned)(NZ * ncolv * sizeof(cd))); }
+      __syncthreads();
+      const cd* src0 = Gh + (size_t)f * d.PH + col0;
+      for (int r = threadIdx.x; r < NZ; r += GD_Z_THREADS) bulk_g2s(tile + (size_t)r * LD, src0 + (size_t)r * planeH, (unsigned)(ncolv * sizeof(cd)), &bar);
+      fft_load_table<NZ>(smem, tw);                            // ends with __syncthreads()
+      mbar_wait(&bar, 0);
 #pragma unroll
-    for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * planeH) : cmake(0.0, 0.0);
-    fft_load_table<NZ>(smem, tw);                              // ends with __syncthreads()
+      for (int q = 0; q < E; ++q) v[q] = active ? tile[(t + T * q) * LD + grp] : cmake(0.0, 0.0);
+      __syncthreads();                                         // tile consumed: the exchange buffers may overwrite it
+    } else {
+      const cd* src = Gh + (size_t)f * d.PH + colH;
+#pragma unroll
+      for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * planeH) : cmake(0.0, 0.0);
+      fft_load_table<NZ>(smem, tw);                            // ends with __syncthreads()
+    }
     fft_lanes<NZ, -1>(v, t, buf, tws);
     __syncthreads();                                           // every group is done with its exchange buffer
 #pragma unroll
