@@ -223,7 +223,19 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
   }
   __syncthreads();                                             // tile read by every group: the exchange may overwrite it
   fft_lanes<NZ, +1>(v, t, buf, tws);
-  if (active) {
+  if (Z::TMA_IN && d.Kxp == d.Kx) {
+    // the [nz][GROUPS] result tile goes through the (now free) exchange region and leaves by one bulk async store per z row
+    const int ncolv = min(GROUPS, plane - col0);
+    __syncthreads();                                           // every group is done with its exchange buffer
+#pragma unroll
+    for (int q = 0; q < E; ++q) tile[(t + T * q) * LD + grp] = v[q];
+    fence_proxy_async();                                       // generic-proxy writes -> visible to the async proxy
+    __syncthreads();
+    cd* dst0 = Hout + (size_t)f * d.PH + col0;
+    for (int r = threadIdx.x; r < NZ; r += GD_Z_THREADS) bulk_s2g(dst0 + (size_t)r * planeH, tile + (size_t)r * LD, (unsigned)(ncolv * sizeof(cd)));
+    bulk_commit();
+    bulk_wait_read0();                                         // shared memory must stay valid until the engine has read it
+  } else if (active) {
     cd* dst = Hout + (size_t)f * d.PH + colH;
 #pragma unroll
     for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * planeH, v[q]);
