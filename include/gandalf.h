@@ -34,6 +34,7 @@ extern "C" {
 #define GANDALF_ERR_CUDA        -2   /* a CUDA runtime call or kernel launch failed             */
 #define GANDALF_ERR_NONFINITE   -3   /* NaN/Inf seen in the energy reduction of the last step   */
 #define GANDALF_ERR_UNSUPPORTED -4   /* e.g. M > 0 with vA != 1 (Eq. 6 is written for v_A = 1)  */
+#define GANDALF_ERR_CFL         -5   /* dt <= 0 asked for the CFL step of Eq. 16 but max|grad Phi| = 0 and no dt_max */
 
 typedef struct gandalf_ctx gandalf_ctx;   /* opaque */
 
@@ -55,16 +56,24 @@ typedef struct gandalf_params {
   int    g_sign;          /* +1: upper signs of Eq. 6 (g^+), -1: lower signs (g^-)                */
   int    nonlinear;       /* 1: brackets on; 0: brackets replaced by zero (linear tests)          */
   int    hermite_coeff;   /* 0: sqrt(m/2), sqrt((m+1)/2) for every m [Eq. 6c]; 1: literal sqrt(2), sqrt(3/2) of Eq. 6a/6b (Q24) */
-  double force_eps;       /* energy injection rate of the white-noise forcing; 0 = off [Eq. 25]   */
+  double force_eps;       /* energy injection rate of the white-noise forcing; 0 = off [Eq. 25]; > 0 with an
+                             empty forced shell is GANDALF_ERR_INVALID                              */
   int    force_nperp_min, force_nperp_max, force_nz_max;  /* forced shell in mode numbers          */
   unsigned long long seed;/* forcing RNG key (counter-based, Q17)                       */
   double cfl;             /* C of Eq. 16, used when gandalf_step gets dt <= 0      */
   double force_g_amp;     /* white-noise forcing of g_0 at k = (0,0,+-force_g_nz): amplitude a_g, mean injected
-                             power a_g^2 into W_g; 0 = off  [velocity-space benchmark; Q26] */
+                             power a_g^2 into W_g; 0 = off  [velocity-space benchmark; Q26].  With
+                             nspecies = 2 only g^+_0 (the first species) is forced                        */
   int    force_g_nz;      /* forced parallel mode number (>= 1, retained); paper: 1               */
   int    nspecies;        /* 1: one set g_0..g_{M-1} with sign g_sign.  2: both slow-mode species [Eq. 2-4, PAPER.md:57-66;
                              memory layout of PAPER.md:357]: g_hat holds 2M fields, g^+ (sign g_sign) then g^- (sign
                              -g_sign); they share Phi, Psi and do not couple in Eq. 6 as printed (Q11, Q27) */
+  double dt_max;          /* > 0: upper bound of the CFL step of Eq. 16, and the step taken when max|grad Phi| = 0;
+                             0 = no bound (paper-literal Eq. 16; a vanishing flow is then GANDALF_ERR_CFL)  (Q29) */
+  int    hermite_exact;   /* 0: Hermite moments by plain RK2 [Alg. 1 l.4, l.9] (default).  1: the streaming / phase-mixing
+                             operator s i kz (I - T) of Eq. 6 is integrated exactly (matrix exponential in m per kz,
+                             integrating-factor midpoint for the brackets) [future work of PAPER.md:657, 829; lifts the
+                             dt < dz/v_th constraint of PAPER.md:214; Q30] */
   int    device;          /* CUDA device ordinal                                                  */
   void*  stream;          /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
 } gandalf_params;
@@ -89,6 +98,20 @@ int gandalf_destroy(gandalf_ctx* ctx);
 int gandalf_set_state(gandalf_ctx* ctx, const double* zeta_hat, const double* g_hat, int on_device);
 int gandalf_get_state(gandalf_ctx* ctx, double* zeta_hat, double* g_hat, int on_device);
 
+/* Exact checkpoint / restart of the evolved variables (SURVEY.md section 5 "Checkpoint / resume"; PAPER.md:389-391
+ * "bit-exact restarts").  The raw state is what the library time-steps: the vorticities w^+, w^- = -kperp^2 xi^+-
+ * [PAPER.md:156] and g_m, complex fp64, RETAINED modes only, a[field][cz][cy][cx] with cx = 0..nx/3 (n_x = cx),
+ * cy = 0..2(ny/3) (n_y = cy for cy <= ny/3, else cy - (2(ny/3)+1)), cz likewise: gandalf_state_raw_doubles() doubles.
+ * (gandalf_get_state / gandalf_set_state convert to potentials and back, which is not bit exact.)
+ * gandalf_set_state_raw copies the array in without projection and keeps time, step counter and history;
+ * gandalf_set_time sets the simulation time and the step counter -- the forcing RNG counters derive from the step
+ * number (Q17, Q26), so a run resumed with {get_state_raw, get_time} -> new context -> {set_state_raw,
+ * set_time} continues bit for bit.  The energy history restarts at the resumed step. */
+int gandalf_state_raw_doubles(const gandalf_ctx* ctx, long long* n);
+int gandalf_get_state_raw(gandalf_ctx* ctx, double* out, int on_device);
+int gandalf_set_state_raw(gandalf_ctx* ctx, const double* in, int on_device);
+int gandalf_set_time(gandalf_ctx* ctx, double t, long long step);
+
 /* Right-hand side at the current state, boundary layout, without advancing it:
  *   dw_hat[2] = N^+, N^-  : -1/2 [ {xi+,w-} + {xi-,w+} -+ lap_perp {xi+,xi-} ]  (Eq. 1 / Eq. 12 RHS,
  *               vorticity units, the linear -+ i kz vA w term is NOT included -- the integrating
@@ -102,8 +125,10 @@ int gandalf_rhs(gandalf_ctx* ctx, double* dw_hat, double* dg_hat, int on_device)
 /* Advance nsteps complete steps of Algorithm 2 [PAPER.md:297-315]: (CFL dt) -> RHS -> half-step
  * predictor with integrating factors (Eq. 15) and plain RK2 for g_m -> midpoint RHS -> full-step
  * corrector (Alg. 1 l.8-9) -> exponential dissipation (Eq. 17-19) -> forcing increment (Eq. 25).
- * dt > 0: fixed step.  dt <= 0: dt = cfl * min(Lx/nx, Ly/ny) / max|grad_perp Phi| recomputed every
- * step ON THE DEVICE from the state at t_n (Eq. 16), no host synchronisation.
+ * dt > 0: fixed step.  dt <= 0: dt = min(dt_max, cfl * min(Lx/nx, Ly/ny) / max|grad_perp Phi|) recomputed every
+ * step ON THE DEVICE from the state at t_n (Eq. 16), no host synchronisation.  If the flow vanishes (max = 0) and
+ * dt_max = 0 the step and all later ones are no-ops (dt = 0: the state survives, as in the oracle) and every
+ * synchronising call returns GANDALF_ERR_CFL until gandalf_set_state.
  * One energy record is appended per step to the device-resident history.  The call is
  * asynchronous on the ctx's stream; errors detected on the device (non-finite energy) are
  * reported by gandalf_energy_history / gandalf_energy / gandalf_get_time, which synchronise. */

@@ -43,13 +43,14 @@ class OracleParams(C.Structure):
         ("cfl", C.c_double),
         ("force_g_amp", C.c_double), ("force_g_nz", C.c_int),
         ("nspecies", C.c_int),
+        ("dt_max", C.c_double),
     ]
 
 
 _DEFAULTS = dict(M=0, Lx=2 * np.pi, Ly=2 * np.pi, Lz=2 * np.pi, vA=1.0, eta=0.0, r=1, eta_normalized=0,
                  eta_z=0.0, r_z=1, eta_g=0.0, nu_coll=0.0, p=1.0, closure=0, if_variant=0, g_sign=1,
                  nonlinear=1, hermite_coeff=0, force_eps=0.0, force_nperp_min=1, force_nperp_max=2,
-                 force_nz_max=1, seed=0, cfl=0.3, force_g_amp=0.0, force_g_nz=1, nspecies=1)
+                 force_nz_max=1, seed=0, cfl=0.3, force_g_amp=0.0, force_g_nz=1, nspecies=1, dt_max=0.0)
 
 _lib = None
 
@@ -71,6 +72,7 @@ def _load():
         lib.oracle_kpar_spectrum.argtypes = [C.c_void_p, C.c_int, P]
         lib.oracle_energy_history.argtypes = [C.c_void_p, C.c_int, P, C.POINTER(C.c_int)]
         lib.oracle_get_time.argtypes = [C.c_void_p, P, C.POINTER(C.c_longlong), P]
+        lib.oracle_set_time.argtypes = [C.c_void_p, C.c_double, C.c_longlong]
         lib.oracle_last_error.argtypes = [C.c_void_p]
         lib.oracle_last_error.restype = C.c_char_p
         lib.oracle_fft1d.argtypes = [C.c_int, C.c_int, P, P]
@@ -211,6 +213,9 @@ class Oracle:
         d = C.c_double(0)
         self._lib.oracle_get_time(self._h, C.byref(t), C.byref(s), C.byref(d))
         return t.value, s.value, d.value
+
+    def set_time(self, t, step):
+        self._check(self._lib.oracle_set_time(self._h, float(t), int(step)), "set_time")
 
     # full-spectrum helpers used by the pins
     def bracket_full(self, f_hat, g_hat):

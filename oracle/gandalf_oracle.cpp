@@ -70,6 +70,7 @@ struct oracle_params {
   double cfl;
   double force_g_amp; int force_g_nz;   // g_0 forcing at k = (0,0,+-nz) (Q26)
   int nspecies;       // 1: g (sign g_sign);  2: g^+ (g_sign) then g^- (-g_sign), M moments each (Q27)
+  double dt_max;      // > 0: upper bound of the CFL step of Eq. 16 (and the step taken when the flow vanishes); 0 = none (Q29)
 };
 
 }  // extern "C"
@@ -508,8 +509,12 @@ static int step_once(oracle_ctx* c, double dt_in) {
   rhs_eval(c, sn, k1, (dt_in > 0.0) ? nullptr : &maxg2);
   if (!(dt_in > 0.0)) {
     double dxy = std::fmin(c->p.Lx / c->nx, c->p.Ly / c->ny);
-    if (!(maxg2 > 0.0)) { c->err = "CFL: max|grad Phi| is zero"; return -1; }
-    dt = c->p.cfl * dxy / std::sqrt(maxg2);                           // Eq. 16
+    if (maxg2 > 0.0) {
+      dt = c->p.cfl * dxy / std::sqrt(maxg2);                         // Eq. 16
+      if (c->p.dt_max > 0.0 && dt > c->p.dt_max) dt = c->p.dt_max;    // Q29
+    } else if (c->p.dt_max > 0.0) {
+      dt = c->p.dt_max;                                               // no flow: Eq. 16 gives no bound (Q29)
+    } else { c->err = "CFL: max|grad Phi| is zero"; return -1; }
   }
   // Alg. 1 l.3-4: half-step predictor (Eq. 15)
   sh.w[0].resize(c->N); sh.w[1].resize(c->N); sh.g.assign(M, std::vector<cplx>(c->N));
@@ -758,6 +763,13 @@ int oracle_get_time(const oracle_ctx* c, double* t, long long* step, double* las
   if (t) *t = c->t;
   if (step) *step = c->step;
   if (last_dt) *last_dt = c->last_dt;
+  return 0;
+}
+
+// Restart support: time and step counter (the forcing RNG counters derive from the step number, Q17/Q26).
+int oracle_set_time(oracle_ctx* c, double t, long long step) {
+  if (!c || step < 0) return -1;
+  c->t = t; c->step = step;
   return 0;
 }
 

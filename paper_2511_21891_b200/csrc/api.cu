@@ -14,9 +14,9 @@
 #include "common.cuh"
 
 // ---- kernels' launchers (defined in passes_zy.cu, pass_x.cu, pointwise.cu) --------------------------------
-cudaError_t launch_zfft(const Dims& d, int dir, const cd* in, cd* out, const cd* tw, int nfields, cudaStream_t st);
-cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStream_t st);
-cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, cudaStream_t st);
+cudaError_t launch_zfft(const Dims& d, const cd* in, cd* out, const cd* tw, int nfields, cudaStream_t st);
+cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, int num_sms, cudaStream_t st);
+cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, int num_sms, cudaStream_t st);
 cudaError_t prepare_passes_zy(int ny, int nz);
 int xpass_lines_per_cta(int nx);
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
@@ -25,7 +25,7 @@ cudaError_t launch_zstep(const Dims& d, int mode, int if_variant, int g_sign, co
                          const double* scal, const double* cdn, const double* cup, const double* collfac, const double* tabz,
                          const double* tabp, const cd* tw, cudaStream_t st);
 cudaError_t launch_tables(const Dims& d, const PhysParams& p, const double* scal, double* tabz, double* tabp, cudaStream_t st);
-cudaError_t launch_prepare_dt(double fixed_dt, double cfl_dxy, const unsigned long long* maxbits, double* scal,
+cudaError_t launch_prepare_dt(double fixed_dt, double cfl_dxy, double dt_max, const unsigned long long* maxbits, double* scal,
                               const double* crate, double* collfac, int M, cudaStream_t st);
 cudaError_t launch_zero_u64(unsigned long long* p, cudaStream_t st);
 cudaError_t launch_pack(const Dims& d, const cd* in, cd* S, int nfields, int nzeta, cudaStream_t st);
@@ -59,7 +59,8 @@ struct gandalf_ctx {
   int spec_cap;
   long long hist_cap;
   // host bookkeeping
-  long long step; bool H_valid;
+  long long step, hist_base; bool H_valid;   // history record i belongs to step hist_base + i
+  int num_sms;
   long long launches;
   bool timing;
   struct Ev { cudaEvent_t a, b; int cls; };
@@ -79,6 +80,20 @@ struct gandalf_ctx {
   } while (0)
 
 static bool pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// canonical members (nx > 0, or nx = 0 and ny > 0) of the +-k pairs of the forced shell (Eq. 25; Q17)
+static int count_forced_pairs(const gandalf_params* p) {
+  const int lo2 = p->force_nperp_min * p->force_nperp_min, hi2 = p->force_nperp_max * p->force_nperp_max;
+  int n = 0;
+  for (int nz = -p->force_nz_max; nz <= p->force_nz_max; ++nz)
+    for (int ny = -p->force_nperp_max; ny <= p->force_nperp_max; ++ny)
+      for (int nx = 0; nx <= p->force_nperp_max; ++nx) {
+        const int n2 = nx * nx + ny * ny;
+        if (n2 < lo2 || n2 > hi2 || n2 == 0) continue;
+        if ((nx > 0) || (nx == 0 && ny > 0)) ++n;
+      }
+  return n;
+}
 
 template <class T> static cudaError_t dalloc(T** p, size_t count) { return cudaMalloc((void**)p, count * sizeof(T)); }
 
@@ -139,6 +154,7 @@ int gandalf_default_params(gandalf_params* p) {
   p->cfl = 0.3;
   p->force_g_nz = 1;
   p->nspecies = 1;
+  p->dt_max = 0.0; p->hermite_exact = 0;
   return GANDALF_OK;
 }
 
@@ -153,6 +169,10 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (p->closure != 0 && p->closure != 1) return GANDALF_ERR_INVALID;
   if (p->force_g_amp < 0 || (p->force_g_amp > 0 && (p->M < 1 || p->force_g_nz < 1 || p->force_g_nz > p->nz / 3))) return GANDALF_ERR_INVALID;
   if (p->nspecies != 1 && p->nspecies != 2) return GANDALF_ERR_INVALID;
+  if (!(p->dt_max >= 0.0) || !(p->cfl > 0.0)) return GANDALF_ERR_INVALID;
+  if (p->hermite_exact != 0 && p->hermite_exact != 1) return GANDALF_ERR_INVALID;
+  if (p->force_eps > 0.0 && (p->force_nperp_min < 0 || p->force_nperp_max > p->nx / 3 || p->force_nperp_max > p->ny / 3 ||
+                             p->force_nz_max > p->nz / 3 || count_forced_pairs(p) == 0)) return GANDALF_ERR_INVALID;   // empty / unresolved shell
   if (p->M > 0 && p->vA != 1.0) return GANDALF_ERR_UNSUPPORTED;
   if (cudaSetDevice(p->device) != cudaSuccess) { cudaGetLastError(); return GANDALF_ERR_CUDA; }
 
@@ -201,6 +221,9 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (e == cudaSuccess) e = upload_twiddles(&c->twz, d.nz, c->st);
   if (e == cudaSuccess) e = launch_xpass(d, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, c->st, true);
   if (e == cudaSuccess) e = prepare_passes_zy(d.ny, d.nz);
+  c->num_sms = 0;
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, p->device);
+  if (c->num_sms <= 0) c->num_sms = 148;
 
   // Hermite coupling coefficients with the closure folded in (Q10, Q23, Q24)
   // The tables run over the moment FIELDS, species after species: dn = 0 at the first and up = 0 at the last moment of a
@@ -250,7 +273,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
     A(cudaStreamSynchronize(c->st));
   }
   if (e != cudaSuccess) { cudaGetLastError(); free_all(c); delete c; return GANDALF_ERR_CUDA; }
-  c->step = 0; c->H_valid = true; c->launches = 0; c->timing = false;
+  c->step = 0; c->hist_base = 0; c->H_valid = true; c->launches = 0; c->timing = false;
   for (int i = 0; i < KC_N; ++i) { c->t_ms[i] = 0; c->t_n[i] = 0; }
   *out = c;
   return GANDALF_OK;
@@ -281,7 +304,7 @@ static int ensure_io(gandalf_ctx* c, size_t bytes) {
 
 // hybrid copy of S0 (z in real space) -- the form the RHS pipeline consumes
 static int make_hybrid(gandalf_ctx* c, const cd* S) {
-  GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(c->d, +1, S, c->H, c->twz, c->d.F, c->st); }));
+  GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(c->d, S, c->H, c->twz, c->d.F, c->st); }));
   return GANDALF_OK;
 }
 
@@ -291,12 +314,12 @@ static int rhs_pipeline(gandalf_ctx* c, bool want_cfl) {
   if (!c->p.nonlinear && !want_cfl) return GANDALF_OK;
   // nonlinear == 0 with the CFL dt: Eq. 16 still needs max|grad Phi|, so P1/P2 run and the brackets are discarded
   if (want_cfl) GD_CUDA(c, timed(c, -1, 1, [&] { return launch_zero_u64(c->maxbits, c->st); }));
-  GD_CUDA(c, timed(c, KC_YINV, d.M > 0 ? 2 : 1, [&] { return launch_yinv(d, c->H, c->D, c->twy, c->st); }));
+  GD_CUDA(c, timed(c, KC_YINV, d.M > 0 ? 2 : 1, [&] { return launch_yinv(d, c->H, c->D, c->twy, c->num_sms, c->st); }));
   GD_CUDA(c, timed(c, KC_XPASS, 1, [&] {
     return launch_xpass(d, c->D, c->E, c->twx, c->cdn, c->cup, want_cfl ? c->maxbits : nullptr, c->st, false);
   }));
   if (!c->p.nonlinear) return GANDALF_OK;
-  GD_CUDA(c, timed(c, KC_YFWD, d.M > 0 ? 2 : 1, [&] { return launch_yfwd(d, c->E, c->Gh, c->twy, c->st); }));
+  GD_CUDA(c, timed(c, KC_YFWD, d.M > 0 ? 2 : 1, [&] { return launch_yfwd(d, c->E, c->Gh, c->twy, c->num_sms, c->st); }));
   return GANDALF_OK;
 }
 
@@ -309,20 +332,68 @@ static int stage_update(gandalf_ctx* c, int mode, const cd* Wn, const cd* Ws, cd
   return GANDALF_OK;
 }
 
-static int ensure_hist(gandalf_ctx* c, long long need) {
+static int ensure_hist(gandalf_ctx* c, long long need) {   // need: records, counted from hist_base
   if (need <= c->hist_cap) return GANDALF_OK;
   long long cap = c->hist_cap;
   while (cap < need) cap *= 2;
   double* nh = nullptr;
   GD_CUDA(c, cudaMalloc((void**)&nh, (size_t)cap * 7 * sizeof(double)));
-  GD_CUDA(c, cudaMemcpyAsync(nh, c->hist, (size_t)c->step * 7 * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
+  GD_CUDA(c, cudaMemcpyAsync(nh, c->hist, (size_t)(c->step - c->hist_base) * 7 * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
   GD_CUDA(c, cudaStreamSynchronize(c->st));
   cudaFree(c->hist);
   c->hist = nh; c->hist_cap = cap;
   return GANDALF_OK;
 }
 
+// sticky device-side error flag (Eq. 16 without a flow and without dt_max); call after the stream is synchronised
+static int check_device_flags(gandalf_ctx* c) {
+  double s[SC_COUNT];
+  GD_CUDA(c, cudaMemcpyAsync(s, c->scal, sizeof(s), cudaMemcpyDeviceToHost, c->st));
+  GD_CUDA(c, cudaStreamSynchronize(c->st));
+  if (s[SC_ERR] != 0.0) GD_FAIL(c, GANDALF_ERR_CFL, "CFL step (Eq. 16): max|grad Phi| is zero and dt_max is not set; the state was left untouched");
+  return GANDALF_OK;
+}
+
 extern "C" {
+
+int gandalf_state_raw_doubles(const gandalf_ctx* c, long long* n) {
+  if (!c || !n) return GANDALF_ERR_INVALID;
+  *n = 2LL * (long long)c->d.F * (long long)c->d.PS;
+  return GANDALF_OK;
+}
+
+int gandalf_get_state_raw(gandalf_ctx* c, double* out, int on_device) {
+  if (!c) return GANDALF_ERR_INVALID;
+  if (!out) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_get_state_raw: NULL array");
+  GD_CUDA(c, cudaSetDevice(c->p.device));
+  const size_t bytes = (size_t)c->d.F * c->d.PS * sizeof(cd);
+  GD_CUDA(c, cudaMemcpyAsync(out, c->S0, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->st));
+  if (!on_device) GD_CUDA(c, cudaStreamSynchronize(c->st));
+  return GANDALF_OK;
+}
+
+int gandalf_set_state_raw(gandalf_ctx* c, const double* in, int on_device) {
+  if (!c) return GANDALF_ERR_INVALID;
+  if (!in) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_set_state_raw: NULL array");
+  GD_CUDA(c, cudaSetDevice(c->p.device));
+  const size_t bytes = (size_t)c->d.F * c->d.PS * sizeof(cd);
+  GD_CUDA(c, cudaMemcpyAsync(c->S0, in, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->st));
+  int rc = make_hybrid(c, c->S0);
+  if (rc) return rc;
+  c->H_valid = true;
+  if (!on_device) GD_CUDA(c, cudaStreamSynchronize(c->st));
+  return GANDALF_OK;
+}
+
+int gandalf_set_time(gandalf_ctx* c, double t, long long step) {
+  if (!c) return GANDALF_ERR_INVALID;
+  if (step < 0 || !std::isfinite(t)) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_set_time: bad time or step");
+  GD_CUDA(c, cudaSetDevice(c->p.device));
+  GD_CUDA(c, cudaMemcpyAsync(c->scal + SC_T, &t, sizeof(double), cudaMemcpyHostToDevice, c->st));
+  GD_CUDA(c, cudaStreamSynchronize(c->st));     // t lives on this stack frame
+  c->step = step; c->hist_base = step;          // the history restarts at the resumed step
+  return GANDALF_OK;
+}
 
 int gandalf_set_state(gandalf_ctx* c, const double* zeta_hat, const double* g_hat, int on_device) {
   if (!c) return GANDALF_ERR_INVALID;
@@ -342,7 +413,7 @@ int gandalf_set_state(gandalf_ctx* c, const double* zeta_hat, const double* g_ha
   GD_CUDA(c, timed(c, -1, 1, [&] { return launch_pack(d, zin, c->S0, 2, 2, c->st); }));
   if (d.M > 0) GD_CUDA(c, timed(c, -1, 1, [&] { return launch_pack(d, gin, c->S0 + 2 * d.PS, d.M, 0, c->st); }));
   GD_CUDA(c, cudaMemsetAsync(c->scal, 0, SC_COUNT * sizeof(double), c->st));
-  c->step = 0;
+  c->step = 0; c->hist_base = 0;
   int rc = make_hybrid(c, c->S0);
   if (rc) return rc;
   c->H_valid = true;
@@ -395,7 +466,7 @@ int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
   if (nsteps < 0 || !std::isfinite(dt)) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_step: bad dt or nsteps");
   GD_CUDA(c, cudaSetDevice(c->p.device));
   const Dims& d = c->d;
-  int rc = ensure_hist(c, c->step + nsteps);
+  int rc = ensure_hist(c, c->step - c->hist_base + nsteps);
   if (rc) return rc;
   const bool adaptive = !(dt > 0.0);
   const double cfl_dxy = c->p.cfl * std::fmin(c->p.Lx / d.nx, c->p.Ly / d.ny);
@@ -406,7 +477,7 @@ int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
     rc = rhs_pipeline(c, adaptive);
     if (rc) return rc;
     GD_CUDA(c, timed(c, -1, 1, [&] {
-      return launch_prepare_dt(adaptive ? 0.0 : dt, cfl_dxy, c->maxbits, c->scal, c->crate, c->collfac, d.M, c->st);
+      return launch_prepare_dt(adaptive ? 0.0 : dt, cfl_dxy, c->p.dt_max, c->maxbits, c->scal, c->crate, c->collfac, d.M, c->st);
     }));
     GD_CUDA(c, timed(c, -1, 1, [&] { return launch_tables(d, c->ph, c->scal, c->tabz, c->tabp, c->st); }));
     rc = stage_update(c, 1, c->S0, c->S0, c->S1, c->p.nonlinear);
@@ -422,17 +493,17 @@ int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
         return launch_forcing(d, c->S0, c->pairs, c->npairs, c->force_amp, c->p.seed, c->step, c->scal, c->st);
       }));
       // the forcing touches w+- only: refresh the hybrid copy of those two fields
-      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, +1, c->S0, c->H, c->twz, 2, c->st); }));
+      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0, c->H, c->twz, 2, c->st); }));
     }
     if (c->p.force_g_amp > 0.0) {
       GD_CUDA(c, timed(c, -1, 1, [&] {
         return launch_forcing_g(d, c->S0, c->p.force_g_nz, c->p.force_g_amp, c->p.seed, c->step, c->scal, c->st);
       }));
       // the forcing touches g_0 only: refresh the hybrid copy of that field
-      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, +1, c->S0 + 2 * d.PS, c->H + 2 * d.PH, c->twz, 1, c->st); }));
+      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0 + 2 * d.PS, c->H + 2 * d.PH, c->twz, 1, c->st); }));
     }
     GD_CUDA(c, timed(c, -1, 2, [&] {
-      return launch_energy(d, c->S0, c->partial, kEnergyBlocks, c->hist + (size_t)c->step * 7, c->scal, 1, c->st);
+      return launch_energy(d, c->S0, c->partial, kEnergyBlocks, c->hist + (size_t)(c->step - c->hist_base) * 7, c->scal, 1, c->st);
     }));
     c->step += 1;
   }
@@ -450,7 +521,7 @@ int gandalf_energy(gandalf_ctx* c, double out[6]) {
   bool ok = true;
   for (int i = 0; i < 6; ++i) { out[i] = rec[i + 1]; ok = ok && std::isfinite(out[i]); }
   if (!ok) GD_FAIL(c, GANDALF_ERR_NONFINITE, "non-finite energy");
-  return GANDALF_OK;
+  return check_device_flags(c);
 }
 
 int gandalf_kperp_spectrum(gandalf_ctx* c, int nbins, int literal_eq26, double* out) {
@@ -504,13 +575,14 @@ int gandalf_kpar_spectrum(gandalf_ctx* c, int nbins, double* out) {
 int gandalf_energy_history(gandalf_ctx* c, int max_records, double* t_and_E, int* n) {
   if (!c || !n || max_records < 0 || (max_records > 0 && !t_and_E)) return GANDALF_ERR_INVALID;
   GD_CUDA(c, cudaSetDevice(c->p.device));
-  const long long k = c->step < max_records ? c->step : max_records;
+  const long long have = c->step - c->hist_base;
+  const long long k = have < max_records ? have : max_records;
   if (k > 0) GD_CUDA(c, cudaMemcpyAsync(t_and_E, c->hist, (size_t)k * 7 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
   GD_CUDA(c, cudaStreamSynchronize(c->st));
   *n = (int)k;
   for (long long i = 0; i < k * 7; ++i)
     if (!std::isfinite(t_and_E[i])) GD_FAIL(c, GANDALF_ERR_NONFINITE, "non-finite value in the energy history");
-  return GANDALF_OK;
+  return check_device_flags(c);
 }
 
 int gandalf_get_time(gandalf_ctx* c, double* t, long long* step, double* last_dt) {
@@ -523,6 +595,7 @@ int gandalf_get_time(gandalf_ctx* c, double* t, long long* step, double* last_dt
   if (step) *step = c->step;
   if (last_dt) *last_dt = s[SC_LASTDT];
   if (!std::isfinite(s[SC_T])) GD_FAIL(c, GANDALF_ERR_NONFINITE, "non-finite time (CFL dt)");
+  if (s[SC_ERR] != 0.0) GD_FAIL(c, GANDALF_ERR_CFL, "CFL step (Eq. 16): max|grad Phi| is zero and dt_max is not set; the state was left untouched");
   return GANDALF_OK;
 }
 

@@ -59,7 +59,19 @@ __device__ __forceinline__ bool mbar_try_wait(unsigned long long* bar, unsigned 
                : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
   return ok != 0;
 }
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) { while (!mbar_try_wait(bar, parity)) {} }
+// try_wait is the suspending form: the hardware parks the thread for a bounded time before it returns false, so the
+// retry loop does not burn issue slots.  -DGD_DEBUG_MBAR builds trap after ~2^26 retries (a faulted bulk copy then
+// surfaces as a launch error instead of hanging the stream).
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+#ifdef GD_DEBUG_MBAR
+  unsigned long long spins = 0;
+#endif
+  while (!mbar_try_wait(bar, parity)) {
+#ifdef GD_DEBUG_MBAR
+    if (++spins > (1ull << 26)) __trap();
+#endif
+  }
+}
 // global -> shared, `bytes` a multiple of 16, both addresses 16-byte aligned; completion counted on `bar`
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, unsigned bytes, unsigned long long* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -83,7 +95,7 @@ struct PhysParams {
 };
 
 // device scalars owned by the context
-enum { SC_DT = 0, SC_T = 1, SC_LASTDT = 2, SC_COUNT = 8 };
+enum { SC_DT = 0, SC_T = 1, SC_LASTDT = 2, SC_ERR = 3, SC_COUNT = 8 };   // SC_ERR != 0: Eq. 16 had no flow to bound dt (sticky)
 
 // Launch geometry of the z transforms: GD_Z_THREADS lanes per CTA = GD_Z_THREADS/T adjacent (cy,cx) columns.
 #define GD_Z_THREADS 128

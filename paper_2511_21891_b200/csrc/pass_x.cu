@@ -45,6 +45,10 @@ struct XGeom {
   // parked R_{m-2}.  Warps sharing a lane quarter take consecutive column slots.
   static constexpr int TM_PHI = 0, TM_RD = 8 * E, TM_SLOT = 10 * E;
   static_assert(TM_SLOT * (THREADS / 128) <= 512, "TMEM columns");
+  // columns to allocate: the next power of two >= what the CTA uses (>= 32), so that small-nx CTAs sharing an SM, or other
+  // tensor-memory users on the device, are not locked out by a 512-column allocation
+  static constexpr int tm_pow2(int n) { int p = 32; while (p < n) p *= 2; return p; }
+  static constexpr int TM_COLS = tm_pow2(TM_SLOT * (THREADS / 128));
 };
 
 // ---- tensor-memory helpers (b32 columns <-> doubles) ------------------------------------------------------
@@ -106,7 +110,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
     }
   }
   if (warp == 0) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&s_tmem_base)), "r"(512) : "memory");
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&s_tmem_base)), "r"(X::TM_COLS) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -317,7 +321,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem_base), "r"(512) : "memory");
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem_base), "r"(X::TM_COLS) : "memory");
 }
 
 // lines per x-pass CTA (the block size of the D layout)

@@ -1,8 +1,7 @@
 // passes_zy.cu -- the z transforms and the y passes of the RHS pipeline.
 //
-//   k_zfft<+1>  : S[f][cz][cy][cx] -> H[f][z][cy][cx]  inverse c2c along z, zero-padded; only after
-//                 set_state and after a forcing increment (k_zfft<-1>, the stand-alone forward transform, is kept for tests
-//                 of the building block but is not on the step path any more)
+//   k_zfft      : S[f][cz][cy][cx] -> H[f][z][cy][cx]  inverse c2c along z, zero-padded; only after
+//                 set_state and after a forcing increment
 //   k_zstep     : P4.  Gh -> S', H': forward z transform + stage update + inverse z transform in one kernel
 //   k_yinv      : P1.  H -> D: for every source field the two arrays U = kx f + df/dy, V = df/dy - kx f (Eq. 10,
 //                 PAPER.md:134; for w+- also of xi = -w/kperp^2), inverse c2c along y
@@ -14,7 +13,7 @@
 #include <vector>
 #include "common.cuh"
 
-template <int NZ, int DIR>
+template <int NZ>
 __global__ void __launch_bounds__(GD_Z_THREADS) k_zfft(Dims d, const cd* __restrict__ in, cd* __restrict__ out,
                                                        const cd* __restrict__ tw, int ncols) {
   using G = FftGeom<NZ>;
@@ -30,32 +29,17 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zfft(Dims d, const cd* __restr
   const int f = active ? gid / plane : 0, rem = active ? gid % plane : 0;
   const int planeH = d.Ky * d.Kxp, remH = (rem / d.Kx) * d.Kxp + rem % d.Kx;       // hybrid rows are padded to Kxp
   cd v[E];
-  if (DIR > 0) {   // compact -> hybrid
-    const cd* src = in + (size_t)f * d.PS + rem;
+  const cd* src = in + (size_t)f * d.PS + rem;
 #pragma unroll
-    for (int q = 0; q < E; ++q) {
-      const int cz = fft2c(t + T * q, NZ, d.hz3, d.Kz);
-      v[q] = (active && cz >= 0) ? ldg_cd(src + (size_t)cz * plane) : cmake(0.0, 0.0);
-    }
-    fft_lanes<NZ, +1>(v, t, buf, tws);
-    if (active) {
-      cd* dst = out + (size_t)f * d.PH + remH;
+  for (int q = 0; q < E; ++q) {
+    const int cz = fft2c(t + T * q, NZ, d.hz3, d.Kz);
+    v[q] = (active && cz >= 0) ? ldg_cd(src + (size_t)cz * plane) : cmake(0.0, 0.0);
+  }
+  fft_lanes<NZ, +1>(v, t, buf, tws);
+  if (active) {
+    cd* dst = out + (size_t)f * d.PH + remH;
 #pragma unroll
-      for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * planeH, v[q]);
-    }
-  } else {         // hybrid -> compact, masked, scaled by 1/(nx ny nz)
-    const cd* src = in + (size_t)f * d.PH + remH;
-#pragma unroll
-    for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * planeH) : cmake(0.0, 0.0);
-    fft_lanes<NZ, -1>(v, t, buf, tws);
-    if (active) {
-      cd* dst = out + (size_t)f * d.PS + rem;
-#pragma unroll
-      for (int q = 0; q < E; ++q) {
-        const int cz = fft2c(t + T * q, NZ, d.hz3, d.Kz);
-        if (cz >= 0) st_cd(dst + (size_t)cz * plane, cscale(v[q], d.inv_n));
-      }
-    }
+    for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * planeH, v[q]);
   }
 }
 
@@ -500,7 +484,6 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, 1) k_yfwd_pair(Dims d, con
   }
 }
 
-static int g_num_sms = 148;   // persistent kernels launch 2 CTAs per SM
 
 // ---- launchers ------------------------------------------------------------------------------------
 template <int N> static size_t fft_smem() { return ((size_t)(GD_Z_THREADS / FftGeom<N>::T) * (FftGeom<N>::BUF + 1) + FftTw<N>::COUNT) * sizeof(cd); }
@@ -514,11 +497,9 @@ template <int N> static int fft_blocks(long long ncols) { const int gpb = GD_Z_T
     default: return cudaErrorInvalidValue;                                            \
   }
 
-cudaError_t launch_zfft(const Dims& d, int dir, const cd* in, cd* out, const cd* tw, int nfields, cudaStream_t st) {
+cudaError_t launch_zfft(const Dims& d, const cd* in, cd* out, const cd* tw, int nfields, cudaStream_t st) {
   const long long ncols = (long long)nfields * d.Ky * d.Kx;
-#define ZCASE(NN)                                                                                         \
-  if (dir > 0) k_zfft<NN, +1><<<fft_blocks<NN>(ncols), GD_Z_THREADS, fft_smem<NN>(), st>>>(d, in, out, tw, (int)ncols); \
-  else k_zfft<NN, -1><<<fft_blocks<NN>(ncols), GD_Z_THREADS, fft_smem<NN>(), st>>>(d, in, out, tw, (int)ncols);
+#define ZCASE(NN) k_zfft<NN><<<fft_blocks<NN>(ncols), GD_Z_THREADS, fft_smem<NN>(), st>>>(d, in, out, tw, (int)ncols);
   GD_DISPATCH(d.nz, ZCASE)
   return cudaGetLastError();
 }
@@ -536,11 +517,11 @@ cudaError_t launch_zstep(const Dims& d, int mode, int if_variant, int g_sign, co
   GD_DISPATCH(d.nz, ZSCASE)
   return cudaGetLastError();
 }
-cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStream_t st) {
+cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, int num_sms, cudaStream_t st) {   // persistent: CTAS per SM
 #define YICASE(NN)                                                                                         \
   {                                                                                                        \
     const int ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;                                    \
-    const int cap = YGeom<NN>::CTAS * g_num_sms;                                                           \
+    const int cap = YGeom<NN>::CTAS * num_sms;                                                           \
     const int ne = 2 * d.nz * ncb, nm = d.M * d.nz * ncb;                                                  \
     k_yinv<NN, true><<<ne < cap ? ne : cap, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, ne);                 \
     if (nm > 0) k_yinv<NN, false><<<nm < cap ? nm : cap, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, nm);    \
@@ -548,28 +529,23 @@ cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, cudaStr
   GD_DISPATCH(d.ny, YICASE)
   return cudaGetLastError();
 }
-cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, cudaStream_t st) {
+cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, int num_sms, cudaStream_t st) {
 #define YFCASE(NN)                                                                                         \
   {                                                                                                        \
     const int ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;                                    \
     const int np = d.nz * ncb;                                                                             \
-    k_yfwd_pair<NN><<<np < g_num_sms ? np : g_num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, np);   \
+    k_yfwd_pair<NN><<<np < num_sms ? np : num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, np);   \
     const int nitems = d.M * d.nz * ncb;                                                                   \
-    if (d.M > 0) k_yfwd<NN><<<nitems < YGeom<NN>::CTAS * g_num_sms ? nitems : YGeom<NN>::CTAS * g_num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, nitems); \
+    if (d.M > 0) k_yfwd<NN><<<nitems < YGeom<NN>::CTAS * num_sms ? nitems : YGeom<NN>::CTAS * num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, nitems); \
   }
   GD_DISPATCH(d.ny, YFCASE)
   return cudaGetLastError();
 }
 // opt-in dynamic shared memory above 48 KB for every instantiation
 cudaError_t prepare_passes_zy(int ny, int nz) {
-  int dev = 0;
-  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-  if (g_num_sms <= 0) g_num_sms = 148;
 #define ZPCASE(NN)                                                                                                         \
   {                                                                                                                        \
-    cudaError_t e = cudaFuncSetAttribute(k_zfft<NN, +1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<NN>());  \
-    if (e != cudaSuccess) return e;                                                                                        \
-    e = cudaFuncSetAttribute(k_zfft<NN, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<NN>());             \
+    cudaError_t e = cudaFuncSetAttribute(k_zfft<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<NN>());      \
     if (e != cudaSuccess) return e;                                                                                        \
     e = cudaFuncSetAttribute(k_zstep<NN, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);        \
     if (e != cudaSuccess) return e;                                                                                        \

@@ -39,15 +39,20 @@ __global__ void __launch_bounds__(256) k_tables(Dims d, PhysParams p, const doub
 }
 
 // dt for this step and the per-moment collision factors exp(-nu (m/M)^(2p) dt) (Eq. 19).
-// fixed_dt > 0: use it; else Eq. 16 from the max |grad Phi|^2 the x-pass left in maxbits.
-__global__ void k_prepare_dt(double fixed_dt, double cfl_dxy, const unsigned long long* maxbits, double* scal,
+// fixed_dt > 0: use it; else Eq. 16 from the max |grad Phi|^2 the x-pass left in maxbits, capped by dt_max (> 0).
+// No flow and no dt_max: Eq. 16 gives no step -- dt = 0 makes this and every later step a no-op (the state survives, as
+// in the oracle) and the sticky flag scal[SC_ERR] is reported by the next synchronising call (GANDALF_ERR_CFL).
+__global__ void k_prepare_dt(double fixed_dt, double cfl_dxy, double dt_max, const unsigned long long* maxbits, double* scal,
                              const double* __restrict__ crate, double* __restrict__ collfac, int M) {
   __shared__ double sdt;
   if (threadIdx.x == 0) {
     double dt = fixed_dt;
     if (!(fixed_dt > 0.0)) {
       const double g2 = __longlong_as_double((long long)*maxbits);
-      dt = cfl_dxy / sqrt(g2);
+      if (scal[SC_ERR] != 0.0) dt = 0.0;
+      else if (g2 > 0.0) { dt = cfl_dxy / sqrt(g2); if (dt_max > 0.0 && dt > dt_max) dt = dt_max; }
+      else if (dt_max > 0.0) dt = dt_max;
+      else { dt = 0.0; scal[SC_ERR] = 1.0; }
     }
     scal[SC_DT] = dt;
     sdt = dt;
@@ -316,9 +321,9 @@ cudaError_t launch_tables(const Dims& d, const PhysParams& p, const double* scal
   k_tables<<<nblk((size_t)n, 256), 256, 0, st>>>(d, p, scal, tabz, tabp);
   return cudaGetLastError();
 }
-cudaError_t launch_prepare_dt(double fixed_dt, double cfl_dxy, const unsigned long long* maxbits, double* scal,
+cudaError_t launch_prepare_dt(double fixed_dt, double cfl_dxy, double dt_max, const unsigned long long* maxbits, double* scal,
                               const double* crate, double* collfac, int M, cudaStream_t st) {
-  k_prepare_dt<<<1, 128, 0, st>>>(fixed_dt, cfl_dxy, maxbits, scal, crate, collfac, M);
+  k_prepare_dt<<<1, 128, 0, st>>>(fixed_dt, cfl_dxy, dt_max, maxbits, scal, crate, collfac, M);
   return cudaGetLastError();
 }
 cudaError_t launch_zero_u64(unsigned long long* p, cudaStream_t st) { k_zero_u64<<<1, 1, 0, st>>>(p); return cudaGetLastError(); }

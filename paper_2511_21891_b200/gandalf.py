@@ -13,7 +13,7 @@ import numpy as np
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libgandalf.so")
 
-OK, ERR_INVALID, ERR_CUDA, ERR_NONFINITE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4
+OK, ERR_INVALID, ERR_CUDA, ERR_NONFINITE, ERR_UNSUPPORTED, ERR_CFL = 0, -1, -2, -3, -4, -5
 KERNEL_CLASSES = ("z_inverse", "y_inverse_P1", "x_pass_P2", "y_forward_P3", "z_step_P4")
 
 
@@ -34,6 +34,7 @@ class GandalfParams(C.Structure):
         ("cfl", C.c_double),
         ("force_g_amp", C.c_double), ("force_g_nz", C.c_int),
         ("nspecies", C.c_int),
+        ("dt_max", C.c_double), ("hermite_exact", C.c_int),
         ("device", C.c_int),
         ("stream", C.c_void_p),
     ]
@@ -64,6 +65,10 @@ def load_library():
     lib.gandalf_destroy.argtypes = [V]
     lib.gandalf_set_state.argtypes = [V, V, V, I]
     lib.gandalf_get_state.argtypes = [V, V, V, I]
+    lib.gandalf_state_raw_doubles.argtypes = [V, C.POINTER(C.c_longlong)]
+    lib.gandalf_get_state_raw.argtypes = [V, V, I]
+    lib.gandalf_set_state_raw.argtypes = [V, V, I]
+    lib.gandalf_set_time.argtypes = [V, D, C.c_longlong]
     lib.gandalf_rhs.argtypes = [V, V, V, I]
     lib.gandalf_step.argtypes = [V, D, I]
     lib.gandalf_energy.argtypes = [V, PD]
@@ -164,6 +169,37 @@ class Gandalf:
         g, gp = self._out(device, self.M)
         self._ck(self._lib.gandalf_get_state(self._h, zp, gp, int(bool(device))))
         return z, g[: self.M]
+
+    def state_raw_doubles(self):
+        n = C.c_longlong(0)
+        self._ck(self._lib.gandalf_state_raw_doubles(self._h, C.byref(n)))
+        return n.value
+
+    def get_state_raw(self, device=False):
+        """The evolved variables w+-, g_m on the retained modes (exact checkpoint), a flat float64 array."""
+        n = self.state_raw_doubles()
+        if device:
+            import torch
+            t = torch.empty(n, dtype=torch.float64, device=f"cuda:{self.params.device}")
+            self._ck(self._lib.gandalf_get_state_raw(self._h, C.c_void_p(t.data_ptr()), 1))
+            return t
+        a = np.empty(n, dtype=np.float64)
+        self._ck(self._lib.gandalf_get_state_raw(self._h, C.c_void_p(a.ctypes.data), 0))
+        return a
+
+    def set_state_raw(self, raw):
+        n = self.state_raw_doubles()
+        if _is_torch(raw):
+            import torch
+            assert raw.is_cuda and raw.dtype == torch.float64 and raw.is_contiguous() and raw.numel() == n
+            self._ck(self._lib.gandalf_set_state_raw(self._h, C.c_void_p(raw.data_ptr()), 1))
+        else:
+            a = np.ascontiguousarray(raw, dtype=np.float64)
+            assert a.size == n
+            self._ck(self._lib.gandalf_set_state_raw(self._h, C.c_void_p(a.ctypes.data), 0))
+
+    def set_time(self, t, step):
+        self._ck(self._lib.gandalf_set_time(self._h, float(t), int(step)))
 
     def rhs(self, device=False):
         dw, wp = self._out(device, 2)

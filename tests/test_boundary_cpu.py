@@ -39,7 +39,10 @@ def test_default_params_layout_matches_binding(lib):
 
 
 @pytest.mark.parametrize("bad", [dict(nx=48), dict(nx=4), dict(nz=1), dict(ny=1024), dict(M=-1), dict(Lx=0.0),
-                                 dict(r=0), dict(g_sign=0), dict(eta=-1.0), dict(closure=2)])
+                                 dict(r=0), dict(g_sign=0), dict(eta=-1.0), dict(closure=2), dict(dt_max=-1.0), dict(cfl=0.0),
+                                 dict(hermite_exact=2), dict(nspecies=3),
+                                 dict(force_eps=1.0, force_nz_max=-1), dict(force_eps=1.0, force_nperp_min=3, force_nperp_max=2),
+                                 dict(force_eps=1.0, force_nperp_max=20)])
 def test_create_rejects_bad_parameters_before_touching_cuda(lib, bad):
     from paper_2511_21891_b200.gandalf import GandalfParams
     p = GandalfParams()
@@ -63,6 +66,8 @@ def test_unsupported_combination(lib):
 def test_null_handles(lib):
     assert lib.gandalf_step(None, 0.1, 1) == -1
     assert lib.gandalf_destroy(None) == -1
+    assert lib.gandalf_set_time(None, 0.0, 0) == -1 and lib.gandalf_set_state_raw(None, None, 0) == -1
+    assert lib.gandalf_get_state_raw(None, None, 0) == -1 and lib.gandalf_state_raw_doubles(None, None) == -1
     assert lib.gandalf_last_error(None) == b"null context"
 
 
