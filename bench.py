@@ -97,7 +97,7 @@ class ClockSampler:
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50",
                                           "-i", str(self.dev)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -130,20 +130,33 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def run_reference(args, rank, world):
-    """The oracle, as it stands, on the host cores: each 'step' is one complete Algorithm-2 step on a
-    bounded sample (a 2-plane z slab, all M moments, full nx x ny) of the workload."""
-    if rank != 0:
-        return
+ORACLE_SLAB_NZ = 8          # z-planes of the oracle's timed sample (both the cpu_baseline leg and --impl reference)
+
+
+def _oracle_slab(name, nz_s, threads=None):
+    """One oracle context on a z-slab of the workload (full nx x ny, all moments, nz_s planes)."""
     import oracle
     from oracle import Oracle
-    name = args.workload
-    fn, kw = WORKLOADS[name]
-    full = (kw["nx"], kw["ny"], kw["nz"])
-    nz_s = 2
+    if threads is not None:
+        oracle.set_num_threads(threads)
     prm, z, g, run = make_workload(name, nz=nz_s)
     o = Oracle(*run["shape"], **prm)
     o.set_state(z, g)
+    return o, prm, run
+
+
+def run_reference(args, rank, world):
+    """The oracle, as it stands, on the host cores: each 'step' is one complete Algorithm-2 step on a bounded sample (a
+    z-slab of ORACLE_SLAB_NZ planes, full nx x ny, all moments) of the workload.  ms_per_step is the MEASURED time of one
+    sample step; `value` scales the sample's rate by slab/nz to the full grid (sample_scale)."""
+    if rank != 0:
+        return
+    import oracle
+    name = args.workload
+    fn, kw = WORKLOADS[name]
+    full = (kw["nx"], kw["ny"], kw["nz"])
+    nz_s = min(ORACLE_SLAB_NZ, full[2])
+    o, prm, run = _oracle_slab(name, nz_s)
     for _ in range(args.warmup):
         o.step(run["dt"], 1)
     t0 = time.perf_counter()
@@ -151,38 +164,61 @@ def run_reference(args, rank, world):
         o.step(run["dt"], 1)
     el = time.perf_counter() - t0
     frac = nz_s / full[2]
-    steps_per_s = args.steps / el * frac
+    sample_steps_per_s = args.steps / el
+    steps_per_s = sample_steps_per_s * frac
     M = prm.get("M", 0) * prm.get("nspecies", 1)
+    wl = {"4a": "BASELINE config 4(a)", "4b": "BASELINE config 4(b)",
+          "4a2": "BASELINE config 4(a) with both slow-mode species (2+64 fields)"}.get(name, f"BASELINE config {name}")
     line = {
         "impl": "reference", "metric": "RHS evals/s", "value": 2 * steps_per_s, "unit": "RHS evals/s", "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / steps_per_s, "higher_is_better": True,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / sample_steps_per_s, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"BASELINE config 4({name[-1]})" if name.startswith("4") else f"BASELINE config {name}",
-                   "grid": list(full), "M": M},
+        "config": {"workload": wl, "grid": list(full), "M": M, "dt": run["dt"], "fields": 2 + M, "parallelism": "host cores (OpenMP)",
+                   "l2": "n/a (CPU)"},
+        "sample_scale": frac, "sample_grid": list(run["shape"]),
         "steps_per_s": steps_per_s, "grid_point_moments_per_s": steps_per_s * full[0] * full[1] * full[2] * (2 + M),
         "cpu_baseline": {"value": 2 * steps_per_s, "unit": "RHS evals/s", "cores": oracle.num_threads(), "kind": "oracle",
-                         "sample": f"each step = one full Algorithm-2 step on a {run['shape'][0]}x{run['shape'][1]}x{nz_s} z-slab "
-                                   f"(all {M} moments), rate scaled by {nz_s}/{full[2]} to the full grid"},
+                         "sample": f"each timed step = one full Algorithm-2 step (2 RHS) on a {run['shape'][0]}x{run['shape'][1]}x{nz_s} "
+                                   f"z-slab (all {M} moments): ms_per_step is that measured time; value = sample rate x {nz_s}/{full[2]}"},
         "e2e": {"value": 2 * steps_per_s, "unit": "RHS evals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line), flush=True)
 
 
-def cpu_baseline_sample(name, full_shape):
+def cpu_baseline_sample(name, full_shape, full_rhs=False):
+    """The oracle timed on the host cores: (i) all cores, one Algorithm-2 step on the ORACLE_SLAB_NZ-plane slab (the same
+    sample --impl reference times), (ii) ONE thread on a 2-plane slab, (iii) with --oracle-full-rhs, one RHS evaluation at
+    the FULL grid on all cores (tens of seconds and ~20 GB of host memory at 4a)."""
     import oracle
-    from oracle import Oracle
-    nz_s = 8 if full_shape[2] >= 8 else full_shape[2]
-    prm, z, g, run = make_workload(name, nz=nz_s)
-    o = Oracle(*run["shape"], **prm)
-    o.set_state(z, g)
+    nthreads = oracle.num_threads()
+    nz_s = min(ORACLE_SLAB_NZ, full_shape[2])
+    o, prm, run = _oracle_slab(name, nz_s)
     t0 = time.perf_counter()
     o.step(run["dt"], 1)
     el = time.perf_counter() - t0
     frac = nz_s / full_shape[2]
-    return {"value": 2.0 / el * frac, "unit": "RHS evals/s", "cores": oracle.num_threads(), "kind": "oracle",
-            "seconds": el,
-            "sample": f"one full Algorithm-2 step (2 RHS) on a {run['shape'][0]}x{run['shape'][1]}x{nz_s} z-slab of the "
-                      f"workload, all moments; rate scaled by {nz_s}/{full_shape[2]} to the full grid"}
+    out = {"value": 2.0 / el * frac, "unit": "RHS evals/s", "cores": nthreads, "kind": "oracle", "seconds": el,
+           "sample": f"one full Algorithm-2 step (2 RHS) on a {run['shape'][0]}x{run['shape'][1]}x{nz_s} z-slab of the "
+                     f"workload, all moments; rate scaled by {nz_s}/{full_shape[2]} to the full grid"}
+    del o
+    nz_1 = min(2, full_shape[2])
+    o1, _, run1 = _oracle_slab(name, nz_1, threads=1)
+    t0 = time.perf_counter()
+    o1.rhs()
+    el1 = time.perf_counter() - t0
+    out["single_thread"] = {"value": 1.0 / el1 * nz_1 / full_shape[2], "unit": "RHS evals/s", "cores": 1, "seconds": el1,
+                            "sample": f"one RHS evaluation on a {run1['shape'][0]}x{run1['shape'][1]}x{nz_1} z-slab, one thread; "
+                                      f"rate scaled by {nz_1}/{full_shape[2]}"}
+    del o1
+    oracle.set_num_threads(nthreads)
+    if full_rhs:
+        of, _, runf = _oracle_slab(name, full_shape[2])
+        t0 = time.perf_counter()
+        of.rhs()
+        elf = time.perf_counter() - t0
+        out["full_grid_rhs"] = {"value": 1.0 / elf, "unit": "RHS evals/s", "cores": nthreads, "seconds": elf,
+                                "sample": f"one RHS evaluation at the full {full_shape[0]}x{full_shape[1]}x{full_shape[2]} grid, all moments (no scaling)"}
+    return out
 
 
 def cufft_comparison(sim, stream, shape, prm, reps=3):
@@ -278,6 +314,23 @@ def cufft_comparison(sim, stream, shape, prm, reps=3):
             "rel_l2_vs_gandalf_rhs": {"dw": err_w, "dg": err_g}, "reps": reps}
 
 
+def run_microbench(device=0, which=(0, 1, 2, 3)):
+    """Measured ceilings of the units the hot path leans on (include/gandalf.h: gandalf_microbench)."""
+    from paper_2511_21891_b200 import gandalf
+    out = {}
+    for w in which:
+        v = gandalf.microbench(w, device)
+        name = gandalf.MICROBENCHES[w]
+        if w == 0:
+            out[name] = {"tflops": v[0], "t_instr_per_s": v[1], "ms": v[2], "sms": int(v[3])}
+        elif w == 1:
+            out[name] = {"g_transforms_per_s_16x16_8warps_register_twiddles": v[0], "g_transforms_per_s_16x16_8warps_table_twiddles": v[1],
+                         "g_transforms_per_s_8x8x4_16warps": v[2], "ms": v[3]}
+        else:
+            out[name] = {"bytes_per_clk_per_sm": v[0], "tb_per_s_chip": v[1], "ms": v[2], "cycles_per_cta": v[3]}
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -288,12 +341,18 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cufft-compare", action="store_true")
+    ap.add_argument("--oracle-full-rhs", action="store_true", help="also time one oracle RHS evaluation at the FULL grid (slow, ~20 GB host memory at 4a)")
+    ap.add_argument("--microbench", action="store_true", help="print the measured unit ceilings (gandalf_microbench) and exit")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+        return
+    if args.microbench:
+        if rank == 0:
+            print(json.dumps(run_microbench(local)), flush=True)
         return
     if args.warmup < 3:
         args.warmup = 3
@@ -325,7 +384,6 @@ def main():
     sampler = ClockSampler(local)
     sampler.start()
     n0 = sim.launch_count()
-    sim.kernel_timing(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with torch.cuda.stream(stream):
         e0.record(stream)
@@ -336,13 +394,23 @@ def main():
         dist.barrier()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
-    clocks = sampler.stop()
     launches = sim.launch_count() - n0
+    ms = max_over_ranks(ms, world)
+    # per-kernel CUDA-event times in a SECOND, untimed-for-the-headline pass (the events cost a little per launch)
+    ksteps = min(args.steps, 10)
+    sim.kernel_timing(True)
+    k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        k0.record(stream)
+        sim.step(dt, ksteps)
+        k1.record(stream)
+    torch.cuda.synchronize()
+    kms = k0.elapsed_time(k1)
     ktimes = sim.kernel_times()
     sim.kernel_timing(False)
-    ms = max_over_ranks(ms, world)
+    clocks = sampler.stop()             # sampled over the timed region and the per-kernel pass that follows it (same load)
     hist = sim.energy_history()
-    assert hist.shape[0] == args.warmup + args.steps and np.isfinite(hist).all()
+    assert hist.shape[0] == args.warmup + args.steps + ksteps and np.isfinite(hist).all()
     spectrum = None
     if args.workload == "3":      # BASELINE config 3 "reports the k_perp energy spectrum" (Eq. 26; unpinned statistics)
         sp = sim.kperp_spectrum(44)
@@ -386,28 +454,55 @@ def main():
         pass
     peak_gbs, peak_src = (peaks["hbm_gbs"], "measured (MEASURED_PEAKS.json)") if "hbm_gbs" in peaks else (6650.0, "fallback")
     per_launch, step_bytes = algorithmic_bytes(shape, M)
+    # the stand-alone z-inverse runs inside a step only after a forcing increment, on the forced fields alone (w+-: 2, g_0: 1)
+    nzi = (2 if prm.get("force_eps", 0.0) > 0 else 0) + (1 if prm.get("force_g_amp", 0.0) > 0 else 0)
+    if nzi:
+        per_launch["z_inverse"] = per_launch["z_inverse"] / F * (nzi / ((prm.get("force_eps", 0.0) > 0) + (prm.get("force_g_amp", 0.0) > 0)))
     kern = {}
     for name in KERNEL_CLASSES:
         avg_ms, n = ktimes[name]
         if n:
-            kern[name] = {"avg_ms": avg_ms, "launches": n, "share_of_step": avg_ms * n / ms,
-                          "algorithmic_gb": per_launch[name] / 1e9, "achieved_gbs": per_launch[name] / 1e9 / (avg_ms * 1e-3)}
+            kern[name] = {"avg_ms": avg_ms, "launches": n, "share_of_step": avg_ms * n / kms,
+                          "algorithmic_gb": per_launch[name] / 1e9, "achieved_gbs": per_launch[name] / 1e9 / (avg_ms * 1e-3),
+                          "frac_of_hbm_peak": per_launch[name] / 1e9 / (avg_ms * 1e-3) / peak_gbs}
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"])
-    traffic = None          # dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)
+    traffic, traffic_src = None, None   # dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)
+    for fn_ in ("r02_traffic.csv", "r01_traffic.csv"):
+        try:
+            for ln in open(os.path.join(ROOT, "profiles", fn_)).read().splitlines()[1:]:
+                w, k, b = ln.split(",")
+                if w == args.workload and k == dom:
+                    traffic, traffic_src = float(b), f"profiles/{fn_} (ncu --set full dram__bytes_read+write per launch, committed; not measured in this run)"
+        except Exception:
+            pass
+        if traffic is not None:
+            break
+    # fp64 side of the dominant kernel: 5 N log2 N flops per complex transform against the DFMA rate
+    # measured on this device right now (gandalf_microbench 0)
+    alu = None
     try:
-        for ln in open(os.path.join(ROOT, "profiles", "r01_traffic.csv")).read().splitlines()[1:]:
-            w, k, b = ln.split(",")
-            if w == args.workload and k == dom:
-                traffic = float(b)
-    except Exception:
-        pass
+        from paper_2511_21891_b200 import gandalf as _g
+        mb = _g.microbench(0, local)
+        nx_, ny_, nz_ = shape
+        nfft = {"x_pass_P2": (4 + M + (2 + M + 1) // 2) * ny_ * nz_ * 5.0 * nx_ * np.log2(nx_),
+                "y_inverse_P1": 2 * (F + 2) * nz_ * (nx_ // 3 + 1) * 5.0 * ny_ * np.log2(ny_),
+                "y_forward_P3": F * nz_ * (nx_ // 3 + 1) * 5.0 * ny_ * np.log2(ny_),
+                "z_step_P4": 2 * F * (nx_ // 3 + 1) * (2 * (ny_ // 3) + 1) * 5.0 * nz_ * np.log2(nz_)}
+        alu = {"measured_fp64_fma_tflops": mb[0], "measured_fp64_t_instr_per_s": mb[1], "how": "gandalf_microbench(0): dependency-free DFMA chains, all SMs, best of 5",
+               "kernels": {k: {"transform_gflop_per_launch": nfft[k] / 1e9, "achieved_tflops": nfft[k] / 1e12 / (kern[k]["avg_ms"] * 1e-3),
+                               "frac_of_measured_fp64_peak": nfft[k] / 1e12 / (kern[k]["avg_ms"] * 1e-3) / mb[0]} for k in nfft if k in kern}}
+    except Exception as exc:
+        alu = {"error": repr(exc)[:200]}
+    step_ms = ms / args.steps
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["achieved_gbs"], "peak": peak_gbs, "peak_source": peak_src,
-                "unit": "GB/s", "frac": kern[dom]["achieved_gbs"] / peak_gbs, "traffic": traffic,
+                "unit": "GB/s", "frac": kern[dom]["achieved_gbs"] / peak_gbs, "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_bytes_per_launch": per_launch[dom],
-                "step": {"algorithmic_gb_4pass_design": step_bytes / 1e9, "achieved_gbs": step_bytes / 1e9 / (ms * 1e-3 / args.steps),
-                         "frac_of_measured_peak": step_bytes / 1e9 / (ms * 1e-3 / args.steps) / peak_gbs,
-                         "frac_of_8TBs_nominal": step_bytes / 1e9 / (ms * 1e-3 / args.steps) / 8000.0},
-                "kernels": kern}
+                "note": "per-kernel times come from a second pass of %d steps with CUDA events around every launch (%.3f ms/step); the headline "
+                        "ms_per_step is timed without them" % (ksteps, kms / ksteps),
+                "step": {"algorithmic_gb_4pass_design": step_bytes / 1e9, "achieved_gbs": step_bytes / 1e9 / (step_ms * 1e-3),
+                         "frac_of_measured_peak": step_bytes / 1e9 / (step_ms * 1e-3) / peak_gbs,
+                         "frac_of_8TBs_nominal": step_bytes / 1e9 / (step_ms * 1e-3) / 8000.0},
+                "alu": alu, "kernels": kern}
 
     cufft = None
     if rank == 0 and world == 1 and not args.no_cufft_compare and prm.get("nspecies", 1) == 1:
@@ -418,7 +513,7 @@ def main():
     if rank == 0:
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            cpu = cpu_baseline_sample(args.workload, shape)
+            cpu = cpu_baseline_sample(args.workload, shape, full_rhs=args.oracle_full_rhs)
         wl = {"4a": "BASELINE config 4(a)", "4b": "BASELINE config 4(b)",
               "4a2": "BASELINE config 4(a) with both slow-mode species (2+64 fields)"}.get(args.workload, f"BASELINE config {args.workload}")
         line = {

@@ -173,6 +173,16 @@ long long gandalf_launch_count(const gandalf_ctx* ctx);
 int gandalf_kernel_timing(gandalf_ctx* ctx, int enable);
 int gandalf_kernel_time_ms(gandalf_ctx* ctx, int which, double* avg_ms, long long* launches);
 
+/* Measured ceilings of the units the hot path leans on (instrumentation; needs no context; synchronises the device).
+ * which = 0: fp64 FMA rate      out = { TFLOP/s, T fp64 instructions/s, ms of the best launch, SM count }
+ *         1: lane-group FFT-256 out = { G transforms/s of the plan 16*16 on 16 lanes with 8 register twiddles, 8 warps per SM;
+ *                                       the same with all twiddles from shared memory; G transforms/s of the plan 8*8*4 on
+ *                                       32 lanes, 16 warps per SM (the x-pass's transform alone: csrc/fft.cuh); ms of the first }
+ *         2: tensor-memory load out = { bytes per clock per SM, TB/s over the chip, ms, mean cycles per CTA }
+ *         3: shared-memory load out = same four numbers for conflict-free 16-byte loads
+ * nout >= 4.  Used by `bench.py --microbench` and for the fp64 ceiling in the bench line. */
+int gandalf_microbench(int which, int device, double* out, int nout);
+
 const char* gandalf_last_error(const gandalf_ctx* ctx);
 
 #ifdef __cplusplus

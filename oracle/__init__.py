@@ -44,13 +44,14 @@ class OracleParams(C.Structure):
         ("force_g_amp", C.c_double), ("force_g_nz", C.c_int),
         ("nspecies", C.c_int),
         ("dt_max", C.c_double),
+        ("hermite_exact", C.c_int),
     ]
 
 
 _DEFAULTS = dict(M=0, Lx=2 * np.pi, Ly=2 * np.pi, Lz=2 * np.pi, vA=1.0, eta=0.0, r=1, eta_normalized=0,
                  eta_z=0.0, r_z=1, eta_g=0.0, nu_coll=0.0, p=1.0, closure=0, if_variant=0, g_sign=1,
                  nonlinear=1, hermite_coeff=0, force_eps=0.0, force_nperp_min=1, force_nperp_max=2,
-                 force_nz_max=1, seed=0, cfl=0.3, force_g_amp=0.0, force_g_nz=1, nspecies=1, dt_max=0.0)
+                 force_nz_max=1, seed=0, cfl=0.3, force_g_amp=0.0, force_g_nz=1, nspecies=1, dt_max=0.0, hermite_exact=0)
 
 _lib = None
 
@@ -83,6 +84,8 @@ def _load():
         lib.oracle_get_full.argtypes = [C.c_void_p, C.c_int, P]
         lib.oracle_set_full.argtypes = [C.c_void_p, C.c_int, P]
         lib.oracle_num_threads.restype = C.c_int
+        lib.oracle_set_num_threads.argtypes = [C.c_int]
+        lib.oracle_set_num_threads.restype = None
         _lib = lib
     return _lib
 
@@ -99,6 +102,10 @@ def _as_pairs(a) -> np.ndarray:
 
 def num_threads() -> int:
     return int(_load().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().oracle_set_num_threads(int(n))
 
 
 def fft1d(x, sign: int) -> np.ndarray:

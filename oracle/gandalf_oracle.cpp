@@ -71,6 +71,7 @@ struct oracle_params {
   double force_g_amp; int force_g_nz;   // g_0 forcing at k = (0,0,+-nz) (Q26)
   int nspecies;       // 1: g (sign g_sign);  2: g^+ (g_sign) then g^- (-g_sign), M moments each (Q27)
   double dt_max;      // > 0: upper bound of the CFL step of Eq. 16 (and the step taken when the flow vanishes); 0 = none (Q29)
+  int hermite_exact;  // 1: exact propagator exp(s i kz (I - T) dt) for the streaming / phase-mixing terms of Eq. 6 (Q30)
 };
 
 }  // extern "C"
@@ -268,7 +269,7 @@ static int neighbour_index(const oracle_ctx* c, int sp, int m) {   // field inde
   return -1;
 }
 
-static void rhs_eval(const oracle_ctx* c, const State& s, State& out, double* max_gradphi2) {
+static void rhs_eval(const oracle_ctx* c, const State& s, State& out, double* max_gradphi2, bool with_streaming = true) {
   const int M = c->M;
   out.w[0].assign(c->N, cplx(0, 0));
   out.w[1].assign(c->N, cplx(0, 0));
@@ -338,7 +339,8 @@ static void rhs_eval(const oracle_ctx* c, const State& s, State& out, double* ma
     }
   }
   // linear streaming / phase-mixing terms of Eq. 6 (d/dz -> i kz), sign s = +1 for g^+ (upper signs)
-  for (int fi = 0; fi < M; ++fi) {
+  // (left out when the stepper integrates them exactly, hermite_exact = 1)
+  for (int fi = 0; with_streaming && fi < M; ++fi) {
     const int sp = fi / c->Msp, m = fi % c->Msp;
     const double sgn = (sp == 0) ? (double)c->p.g_sign : -(double)c->p.g_sign;   // upper / lower signs of Eq. 6
     int lo = neighbour_index(c, sp, m - 1), hi = neighbour_index(c, sp, m + 1);
@@ -497,6 +499,76 @@ static void energies(const oracle_ctx* c, const State& s, double out[6]) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// Exact treatment of the Hermite streaming / phase-mixing terms (hermite_exact = 1; Q30; the paper lists
+// exponential integrators as future work, and the constraint it lifts at PAPER.md:214).
+// For one (kx,ky,kz) the linear part of Eq. 6 is  d g/dt = s i kz (I - T) g  with T[m][m-1] = sqrt(m/2), T[m][m+1] =
+// sqrt((m+1)/2) (closure folded in as in rhs_eval).  propagate() applies  exp(s i kz (I - T) tau)  to the moment vector of
+// every mode; the matrix exponential is a plain scaling-and-squaring Taylor series.
+// ---------------------------------------------------------------------------------------------
+static void mat_mul(int n, const std::vector<cplx>& A, const std::vector<cplx>& B, std::vector<cplx>& C) {
+  C.assign((size_t)n * n, cplx(0, 0));
+  for (int i = 0; i < n; ++i)
+    for (int k = 0; k < n; ++k) {
+      const cplx a = A[(size_t)i * n + k];
+      if (a == cplx(0, 0)) continue;
+      for (int j = 0; j < n; ++j) C[(size_t)i * n + j] += a * B[(size_t)k * n + j];
+    }
+}
+
+static void mat_expm(int n, const std::vector<cplx>& A, std::vector<cplx>& E) {
+  double norm1 = 0.0;                                    // max column sum
+  for (int j = 0; j < n; ++j) { double cs = 0; for (int i = 0; i < n; ++i) cs += std::abs(A[(size_t)i * n + j]); if (cs > norm1) norm1 = cs; }
+  int nsq = 0;
+  while (std::ldexp(norm1, -nsq) > 0.25) ++nsq;
+  std::vector<cplx> As(A);
+  for (auto& v : As) v = cplx(std::ldexp(v.real(), -nsq), std::ldexp(v.imag(), -nsq));
+  E.assign((size_t)n * n, cplx(0, 0));
+  std::vector<cplx> term((size_t)n * n, cplx(0, 0)), tmp;
+  for (int i = 0; i < n; ++i) { E[(size_t)i * n + i] = 1.0; term[(size_t)i * n + i] = 1.0; }
+  for (int k = 1; k <= 24; ++k) {                        // 0.25^25 / 25! is far below round-off
+    mat_mul(n, term, As, tmp);
+    for (size_t i = 0; i < tmp.size(); ++i) { term[i] = tmp[i] / (double)k; E[i] += term[i]; }
+  }
+  for (int q = 0; q < nsq; ++q) { mat_mul(n, E, E, tmp); E.swap(tmp); }
+}
+
+static void streaming_matrix(const oracle_ctx* c, std::vector<double>& T) {     // M_sp x M_sp, real
+  const int M = c->Msp;
+  T.assign((size_t)M * M, 0.0);
+  for (int m = 0; m < M; ++m) {
+    int lo = neighbour_index(c, 0, m - 1), hi = neighbour_index(c, 0, m + 1);
+    if (lo >= 0) T[(size_t)m * M + lo] += c->coef_dn[m];
+    if (hi >= 0) T[(size_t)m * M + hi] += c->coef_up[m];
+  }
+}
+
+static void propagate(const oracle_ctx* c, std::vector<std::vector<cplx>>& g, double tau) {
+  const int M = c->Msp;
+  if (M == 0) return;
+  std::vector<double> T;
+  streaming_matrix(c, T);
+  for (int iz = 0; iz < c->nz; ++iz) {
+    for (int sp = 0; sp < c->nsp; ++sp) {
+      const double sgn = (sp == 0) ? (double)c->p.g_sign : -(double)c->p.g_sign;
+      std::vector<cplx> A((size_t)M * M), E;
+      for (int i = 0; i < M; ++i)
+        for (int j = 0; j < M; ++j) A[(size_t)i * M + j] = cplx(0.0, sgn * c->kz[iz] * tau) * ((i == j ? 1.0 : 0.0) - T[(size_t)i * M + j]);
+      mat_expm(M, A, E);
+#pragma omp parallel for collapse(2) schedule(static)
+      for (int iy = 0; iy < c->ny; ++iy)
+        for (int ix = 0; ix < c->nx; ++ix) {
+          size_t i = IDX(c, iz, iy, ix);
+          std::vector<cplx> in(M), out(M, cplx(0, 0));
+          for (int m = 0; m < M; ++m) in[m] = g[sp * M + m][i];
+          for (int m = 0; m < M; ++m)
+            for (int k = 0; k < M; ++k) out[m] += E[(size_t)m * M + k] * in[k];
+          for (int m = 0; m < M; ++m) g[sp * M + m][i] = out[m];
+        }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // One complete step (Alg. 2; Alg. 1).
 // ---------------------------------------------------------------------------------------------
 static int step_once(oracle_ctx* c, double dt_in) {
@@ -506,7 +578,8 @@ static int step_once(oracle_ctx* c, double dt_in) {
   double dt = dt_in;
   double maxg2 = 0.0;
   // Alg. 2 l.2: CFL step from state_n (only when the caller asks for it: dt <= 0)
-  rhs_eval(c, sn, k1, (dt_in > 0.0) ? nullptr : &maxg2);
+  const bool exact = (c->p.hermite_exact != 0) && M > 0;    // Q30: brackets by the midpoint rule, streaming terms exactly
+  rhs_eval(c, sn, k1, (dt_in > 0.0) ? nullptr : &maxg2, !exact);
   if (!(dt_in > 0.0)) {
     double dxy = std::fmin(c->p.Lx / c->nx, c->p.Ly / c->ny);
     if (maxg2 > 0.0) {
@@ -533,8 +606,9 @@ static int step_once(oracle_ctx* c, double dt_in) {
   }
   for (int m = 0; m < M; ++m)
     for (size_t i = 0; i < c->N; ++i) sh.g[m][i] = sn.g[m][i] + (0.5 * dt) * k1.g[m][i];
+  if (exact) propagate(c, sh.g, 0.5 * dt);                  // g_{n+1/2} = P(dt/2) (g_n + dt/2 R_n),  P(tau) = exp(s i kz (I - T) tau)
   // Alg. 1 l.6: midpoint RHS
-  rhs_eval(c, sh, k2, nullptr);
+  rhs_eval(c, sh, k2, nullptr, !exact);
   // Alg. 1 l.8-9: full-step corrector
   State s1; s1.w[0].resize(c->N); s1.w[1].resize(c->N); s1.g.assign(M, std::vector<cplx>(c->N));
   for (int a = 0; a < 2; ++a) {
@@ -553,8 +627,16 @@ static int step_once(oracle_ctx* c, double dt_in) {
             s1.w[a][i] = ph * sn.w[a][i] + phN * dt * k2.w[a][i];
         }
   }
-  for (int m = 0; m < M; ++m)
-    for (size_t i = 0; i < c->N; ++i) s1.g[m][i] = sn.g[m][i] + dt * k2.g[m][i];
+  if (exact) {                                              // g_{n+1} = P(dt) g_n + P(dt/2) dt R_{n+1/2} = P(dt/2) (P(dt/2) g_n + dt R_{n+1/2})
+    for (int m = 0; m < M; ++m) s1.g[m] = sn.g[m];
+    propagate(c, s1.g, 0.5 * dt);
+    for (int m = 0; m < M; ++m)
+      for (size_t i = 0; i < c->N; ++i) s1.g[m][i] += dt * k2.g[m][i];
+    propagate(c, s1.g, 0.5 * dt);
+  } else {
+    for (int m = 0; m < M; ++m)
+      for (size_t i = 0; i < c->N; ++i) s1.g[m][i] = sn.g[m][i] + dt * k2.g[m][i];
+  }
   // Alg. 2 l.12-14: dissipation with the full dt
   apply_dissipation(c, s1, dt);
   // forcing increment (Q17), then time and diagnostics
@@ -620,6 +702,7 @@ int oracle_create(const oracle_params* p, oracle_ctx** out) {
   if (p->M < 0 || !(p->Lx > 0) || !(p->Ly > 0) || !(p->Lz > 0)) return -1;
   if (p->M > 0 && p->vA != 1.0) return -4;                 // Q12
   if (p->nspecies != 1 && p->nspecies != 2) return -1;
+  if (p->hermite_exact != 0 && p->hermite_exact != 1) return -1;
   oracle_ctx* c = new oracle_ctx();
   c->p = *p; c->nx = p->nx; c->ny = p->ny; c->nz = p->nz;
   c->Msp = p->M; c->nsp = p->nspecies; c->M = p->M * p->nspecies;
@@ -813,6 +896,14 @@ int oracle_set_full(oracle_ctx* c, int field, const double* in) {
   std::vector<cplx>& a = (field < 2) ? c->w[field] : c->g[field - 2];
   for (size_t i = 0; i < c->N; ++i) a[i] = cplx(in[2 * i], in[2 * i + 1]);
   return 0;
+}
+// Thread count of the OpenMP loops (bench.py times the oracle on all host cores and once single-threaded).
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n >= 1) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
 }
 int oracle_num_threads(void) {
 #ifdef _OPENMP

@@ -19,11 +19,17 @@ cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, int num
 cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, int num_sms, cudaStream_t st);
 cudaError_t prepare_passes_zy(int ny, int nz);
 int xpass_lines_per_cta(int nx);
+int xpass_fft_plan_id(int nx);
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
                          unsigned long long* maxbits, cudaStream_t st, bool prepare_only);
-cudaError_t launch_zstep(const Dims& d, int mode, int if_variant, int g_sign, const cd* Gh, const cd* Wn, const cd* Ws, cd* Wout, cd* Hout,
+cudaError_t launch_zstep(const Dims& d, int mode, bool exact, int if_variant, int g_sign, const cd* Gh, const cd* Wn, const cd* Ws, cd* Wout, cd* Hout,
                          const double* scal, const double* cdn, const double* cup, const double* collfac, const double* tabz,
                          const double* tabp, const cd* tw, cudaStream_t st);
+void jacobi_eigh(int n, std::vector<double>& A, std::vector<double>& V, std::vector<double>& lam);
+cudaError_t launch_hermite_propagator(const Dims& d, int g_sign, double frac, const double* scal, const double* V, const double* lam,
+                                      cd* P, cudaStream_t st);
+cudaError_t launch_hermite_apply(const Dims& d, const cd* in, cd* out, const cd* P, int diss, const double* collfac,
+                                 const double* tabz, const double* tabp, cudaStream_t st);
 cudaError_t launch_tables(const Dims& d, const PhysParams& p, const double* scal, double* tabz, double* tabp, cudaStream_t st);
 cudaError_t launch_prepare_dt(double fixed_dt, double cfl_dxy, double dt_max, const unsigned long long* maxbits, double* scal,
                               const double* crate, double* collfac, int M, cudaStream_t st);
@@ -53,6 +59,7 @@ struct gandalf_ctx {
   cd *S0, *S1, *H, *Gh, *D, *E;
   cd *twx, *twy, *twz;
   double *cdn, *cup, *crate, *collfac, *scal, *partial, *hist, *rec_scratch, *spec_col, *spec_out, *tabz, *tabp;
+  double *hxV, *hxLam; cd* hxP;      // hermite_exact: eigenvectors / eigenvalues of the coupling matrix, propagators P(dt/2) per kz
   unsigned long long* maxbits;
   int* pairs; int npairs; double force_amp;
   cd* io; size_t io_bytes;
@@ -112,7 +119,7 @@ static cudaError_t upload_twiddles(cd** dst, int n, cudaStream_t st) {
 static void free_all(gandalf_ctx* c) {
   void* ptrs[] = {c->tabz, c->tabp, c->S0, c->S1, c->H, c->Gh, c->D, c->E, c->twx, c->twy, c->twz, c->cdn, c->cup, c->crate,
                   c->collfac, c->scal, c->partial, c->hist, c->rec_scratch, c->spec_col, c->spec_out, c->maxbits,
-                  c->pairs, c->io};
+                  c->pairs, c->io, c->hxV, c->hxLam, c->hxP};
   for (void* q : ptrs) if (q) cudaFree(q);
   for (auto& e : c->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
 }
@@ -174,6 +181,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (p->force_eps > 0.0 && (p->force_nperp_min < 0 || p->force_nperp_max > p->nx / 3 || p->force_nperp_max > p->ny / 3 ||
                              p->force_nz_max > p->nz / 3 || count_forced_pairs(p) == 0)) return GANDALF_ERR_INVALID;   // empty / unresolved shell
   if (p->M > 0 && p->vA != 1.0) return GANDALF_ERR_UNSUPPORTED;
+  if (p->hermite_exact && p->M > 0 && (p->closure != 0 || p->hermite_coeff != 0)) return GANDALF_ERR_UNSUPPORTED;   // symmetric coupling matrix only (Q30)
   if (cudaSetDevice(p->device) != cudaSuccess) { cudaGetLastError(); return GANDALF_ERR_CUDA; }
 
   gandalf_ctx* c = new (std::nothrow) gandalf_ctx();
@@ -188,6 +196,12 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   d.Kx = d.hx3 + 1; d.Ky = 2 * d.hy3 + 1; d.Kz = 2 * d.hz3 + 1;
   d.kx0 = 2.0 * kPi / p->Lx; d.ky0 = 2.0 * kPi / p->Ly; d.kz0 = 2.0 * kPi / p->Lz;
   d.inv_n = 1.0 / ((double)p->nx * p->ny * p->nz);
+  {
+    const double k2ret = std::pow(d.kx0 * d.hx3, 2) + std::pow(d.ky0 * d.hy3, 2);     // largest retained kperp^2
+    int ex = 0;
+    std::frexp(0.5 * k2ret, &ex);
+    d.bscale = std::ldexp(1.0, ex - 1); d.inv_bscale = 1.0 / d.bscale;                // exact power of two
+  }
   // Row strides.  E rows are padded to 128 B multiples (P3 then reads whole DRAM granules: 0.52 -> 0.50 ms at 4a); the same
   // padding on the hybrid arrays was measured SLOWER (P3 0.60, P4 1.05 ms: their lane-per-row stores then camp on few L2
   // slices), so H and Gh keep unpadded rows.
@@ -216,7 +230,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   A(dalloc(&c->spec_col, (size_t)d.Ky * d.Kx)); A(dalloc(&c->maxbits, (size_t)1));
   c->hist_cap = 4096;
   A(dalloc(&c->hist, (size_t)c->hist_cap * 7));
-  if (e == cudaSuccess) e = upload_twiddles(&c->twx, d.nx, c->st);
+  if (e == cudaSuccess) e = upload_twiddles(&c->twx, xpass_fft_plan_id(d.nx), c->st);
   if (e == cudaSuccess) e = upload_twiddles(&c->twy, d.ny, c->st);
   if (e == cudaSuccess) e = upload_twiddles(&c->twz, d.nz, c->st);
   if (e == cudaSuccess) e = launch_xpass(d, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, c->st, true);
@@ -239,6 +253,19 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
       ups[Ms - 1] = 0.0;                                            // g_M := 0 otherwise
     }
     for (int m = 0; m < Ms; ++m) crs[m] = p->nu_coll * std::pow((double)m / (double)Ms, 2.0 * p->p);   // Eq. 19
+  }
+  // hermite_exact: T = V diag(lambda) V^T of the Msp x Msp coupling matrix (absorbing closure: symmetric tridiagonal)
+  if (p->hermite_exact && Ms > 0) {
+    std::vector<double> T((size_t)Ms * Ms, 0.0), V, lam;
+    for (int m = 1; m < Ms; ++m) T[(size_t)m * Ms + m - 1] = T[(size_t)(m - 1) * Ms + m] = std::sqrt(m / 2.0);
+    jacobi_eigh(Ms, T, V, lam);
+    A(dalloc(&c->hxV, (size_t)Ms * Ms)); A(dalloc(&c->hxLam, (size_t)Ms));
+    A(dalloc(&c->hxP, (size_t)p->nspecies * d.Kz * Ms * Ms));
+    if (e == cudaSuccess) {
+      A(cudaMemcpyAsync(c->hxV, V.data(), V.size() * sizeof(double), cudaMemcpyHostToDevice, c->st));
+      A(cudaMemcpyAsync(c->hxLam, lam.data(), lam.size() * sizeof(double), cudaMemcpyHostToDevice, c->st));
+      A(cudaStreamSynchronize(c->st));        // V, lam live on this stack frame
+    }
   }
   // forcing pairs (Eq. 25; Q17): canonical members of each +-k pair in a fixed enumeration order
   std::vector<int> pr;
@@ -324,9 +351,9 @@ static int rhs_pipeline(gandalf_ctx* c, bool want_cfl) {
 }
 
 // P4: forward z transform of Gh + stage update (mode 0/1/2) + inverse z transform into the hybrid copy (if wanted)
-static int stage_update(gandalf_ctx* c, int mode, const cd* Wn, const cd* Ws, cd* Wout, bool want_hybrid) {
+static int stage_update(gandalf_ctx* c, int mode, const cd* Wn, const cd* Ws, cd* Wout, bool want_hybrid, bool exact = false) {
   GD_CUDA(c, timed(c, KC_ZSTEP, 1, [&] {
-    return launch_zstep(c->d, mode, c->p.if_variant, c->p.g_sign, c->p.nonlinear ? c->Gh : nullptr, Wn, Ws, Wout,
+    return launch_zstep(c->d, mode, exact, c->p.if_variant, c->p.g_sign, c->p.nonlinear ? c->Gh : nullptr, Wn, Ws, Wout,
                         want_hybrid ? c->H : nullptr, c->scal, c->cdn, c->cup, c->collfac, c->tabz, c->tabp, c->twz, c->st);
   }));
   return GANDALF_OK;
@@ -472,6 +499,7 @@ int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
   const double cfl_dxy = c->p.cfl * std::fmin(c->p.Lx / d.nx, c->p.Ly / d.ny);
   if (!c->H_valid) { rc = make_hybrid(c, c->S0); if (rc) return rc; c->H_valid = true; }
   const bool need_h = c->p.nonlinear || adaptive;
+  const bool exact = c->p.hermite_exact && d.M > 0;
   for (int i = 0; i < nsteps; ++i) {
     // Alg. 2 l.3-6: RHS at t_n (its x-pass also yields max|grad Phi| for Eq. 16), half-step predictor
     rc = rhs_pipeline(c, adaptive);
@@ -480,14 +508,32 @@ int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
       return launch_prepare_dt(adaptive ? 0.0 : dt, cfl_dxy, c->p.dt_max, c->maxbits, c->scal, c->crate, c->collfac, d.M, c->st);
     }));
     GD_CUDA(c, timed(c, -1, 1, [&] { return launch_tables(d, c->ph, c->scal, c->tabz, c->tabp, c->st); }));
-    rc = stage_update(c, 1, c->S0, c->S0, c->S1, c->p.nonlinear);
-    if (rc) return rc;
-    // Alg. 2 l.7-9: midpoint RHS
-    rc = rhs_pipeline(c, false);
-    if (rc) return rc;
-    // Alg. 2 l.10-14: full step + dissipation (in place on S0: each mode reads only its own S0 entry)
-    rc = stage_update(c, 2, c->S0, c->S1, c->S0, need_h);
-    if (rc) return rc;
+    if (!exact) {
+      rc = stage_update(c, 1, c->S0, c->S0, c->S1, c->p.nonlinear);
+      if (rc) return rc;
+      // Alg. 2 l.7-9: midpoint RHS
+      rc = rhs_pipeline(c, false);
+      if (rc) return rc;
+      // Alg. 2 l.10-14: full step + dissipation (in place on S0: each mode reads only its own S0 entry)
+      rc = stage_update(c, 2, c->S0, c->S1, c->S0, need_h);
+      if (rc) return rc;
+    } else {
+      // hermite_exact (Q30): with P = P(dt/2) = exp(s i kz (I - T) dt/2) per kz,
+      //   g_{n+1/2} = P (g_n + dt/2 R_n),   g_{n+1} = P (P g_n + dt R_{n+1/2}),   R = the bracket terms of Eq. 6;
+      // w+- exactly as above.  D is free between two RHS pipelines and serves as scratch for the propagated half-step state.
+      GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_propagator(d, c->p.g_sign, 0.5, c->scal, c->hxV, c->hxLam, c->hxP, c->st); }));
+      rc = stage_update(c, 1, c->S0, c->S0, c->S1, c->p.nonlinear, true);          // S1 = w_{n+1/2} | g_n + dt/2 R_n ; H(w+-)
+      if (rc) return rc;
+      GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_apply(d, c->S1, c->D, c->hxP, 0, c->collfac, c->tabz, c->tabp, c->st); }));
+      if (c->p.nonlinear) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->D + 2 * d.PS, c->H + 2 * d.PH, c->twz, d.M, c->st); }));
+      rc = rhs_pipeline(c, false);                                                  // brackets at the midpoint state
+      if (rc) return rc;
+      GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_apply(d, c->S0, c->S1, c->hxP, 0, c->collfac, c->tabz, c->tabp, c->st); }));   // S1(g) = P g_n
+      rc = stage_update(c, 2, c->S0, c->S1, c->S0, need_h, true);                   // S0(w) = w_{n+1};  S1(g) += dt R_{n+1/2}
+      if (rc) return rc;
+      GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_apply(d, c->S1, c->S0, c->hxP, 1, c->collfac, c->tabz, c->tabp, c->st); }));   // S0(g) = diss . P S1(g)
+      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0 + 2 * d.PS, c->H + 2 * d.PH, c->twz, d.M, c->st); }));
+    }
     if (c->npairs) {
       GD_CUDA(c, timed(c, -1, 1, [&] {
         return launch_forcing(d, c->S0, c->pairs, c->npairs, c->force_amp, c->p.seed, c->step, c->scal, c->st);

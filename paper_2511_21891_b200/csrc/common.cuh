@@ -22,6 +22,8 @@ struct Dims {
   int hx3, hy3, hz3;      // floor(N/3)
   double kx0, ky0, kz0;   // 2 pi / L
   double inv_n;           // 1/(nx ny nz)
+  double bscale, inv_bscale;   // power of two ~ kperp,max^2/2: the x-pass transforms the pair (A, bscale*B) so that B's round-off
+                          // floor is not set by A's magnitude before N+- = -1/2 A -+ 1/2 kperp^2 B amplifies it
   int xl, xlsh;           // lines per x-pass CTA (power of two) and its log2: block size of the D layout
   size_t PS, PH, PD, PE;  // per-field strides (complex elements): compact, hybrid, D (blocked, padded), E
 };

@@ -109,21 +109,27 @@ template <int R, int DIR> GD_HD void butterfly(cd (&x)[R]) {
 }
 
 // ---- plan: N -> lanes per FFT, elements per lane, stage radices -------------------------------
+// The template argument of every routine below is a plan ID: the transform length N, or N + GD_FFT_ALT for the alternative
+// plan of that length (more lanes, fewer registers per lane: 256 = 8*8*4 on a whole warp, for kernels that want 16 warps per SM).
+#define GD_FFT_ALT 4096
 template <int N> struct FftPlan;
-template <> struct FftPlan<2>   { static constexpr int T = 1,  E = 2,  S = 1, R0 = 2,  R1 = 1,  R2 = 1; };
-template <> struct FftPlan<4>   { static constexpr int T = 1,  E = 4,  S = 1, R0 = 4,  R1 = 1,  R2 = 1; };
-template <> struct FftPlan<8>   { static constexpr int T = 1,  E = 8,  S = 1, R0 = 8,  R1 = 1,  R2 = 1; };
-template <> struct FftPlan<16>  { static constexpr int T = 1,  E = 16, S = 1, R0 = 16, R1 = 1,  R2 = 1; };
-template <> struct FftPlan<32>  { static constexpr int T = 4,  E = 8,  S = 2, R0 = 8,  R1 = 4,  R2 = 1; };
-template <> struct FftPlan<64>  { static constexpr int T = 8,  E = 8,  S = 2, R0 = 8,  R1 = 8,  R2 = 1; };
-template <> struct FftPlan<128> { static constexpr int T = 8,  E = 16, S = 2, R0 = 16, R1 = 8,  R2 = 1; };
-template <> struct FftPlan<256> { static constexpr int T = 16, E = 16, S = 2, R0 = 16, R1 = 16, R2 = 1; };
-template <> struct FftPlan<512> { static constexpr int T = 32, E = 16, S = 3, R0 = 8,  R1 = 8,  R2 = 8; };
+template <> struct FftPlan<2>   { static constexpr int T = 1,  E = 2,  S = 1, R0 = 2,  R1 = 1,  R2 = 1, PAD = R0; };
+template <> struct FftPlan<4>   { static constexpr int T = 1,  E = 4,  S = 1, R0 = 4,  R1 = 1,  R2 = 1, PAD = R0; };
+template <> struct FftPlan<8>   { static constexpr int T = 1,  E = 8,  S = 1, R0 = 8,  R1 = 1,  R2 = 1, PAD = R0; };
+template <> struct FftPlan<16>  { static constexpr int T = 1,  E = 16, S = 1, R0 = 16, R1 = 1,  R2 = 1, PAD = R0; };
+template <> struct FftPlan<32>  { static constexpr int T = 4,  E = 8,  S = 2, R0 = 8,  R1 = 4,  R2 = 1, PAD = R0; };
+template <> struct FftPlan<64>  { static constexpr int T = 8,  E = 8,  S = 2, R0 = 8,  R1 = 8,  R2 = 1, PAD = R0; };
+template <> struct FftPlan<128> { static constexpr int T = 8,  E = 16, S = 2, R0 = 16, R1 = 8,  R2 = 1, PAD = R0; };
+template <> struct FftPlan<256> { static constexpr int T = 16, E = 16, S = 2, R0 = 16, R1 = 16, R2 = 1, PAD = R0; };
+template <> struct FftPlan<512> { static constexpr int T = 32, E = 16, S = 3, R0 = 8,  R1 = 8,  R2 = 8, PAD = R0; };
+template <> struct FftPlan<256 + GD_FFT_ALT> { static constexpr int T = 32, E = 8, S = 3, R0 = 8, R1 = 8, R2 = 4, PAD = 16; };   // pad 16: 8-byte exchange conflict-free on 32 lanes
 
-template <int N> struct FftGeom {
-  using P = FftPlan<N>;
+template <int ID> struct FftGeom {
+  using P = FftPlan<ID>;
+  static constexpr int N = ID % GD_FFT_ALT;                // transform length
   static constexpr int T = P::T, E = P::E, S = P::S;
-  static constexpr int PADDIV = P::R0;                     // pad(idx) = idx + idx / R0
+  static_assert(T * E == N, "plan covers the transform");
+  static constexpr int PADDIV = P::PAD;                    // pad(idx) = idx + idx / PAD (PAD = R0 unless the plan says otherwise)
   static constexpr int BUF = (S > 1) ? (N + N / PADDIV) : 0;  // complex entries of the line buffer
   GD_HD static int pad(int idx) { return idx + idx / PADDIV; }
   template <int s> static constexpr int radix() { return s == 0 ? P::R0 : (s == 1 ? P::R1 : P::R2); }

@@ -21,25 +21,31 @@
 #ifndef GD_X_NTWR
 #define GD_X_NTWR 8
 #endif
+#ifndef GD_X_ALT
+#define GD_X_ALT 0        // 1: nx = 256 on one WARP per line (plan 8*8*4, 8 points per lane, 16 warps per SM).  Measured SLOWER (1.72 vs 1.40 ms at 4a:
+                          // the second exchange costs more than the extra warps hide; bare transform 1.35 vs 2.53 G/s) -- kept as a tested option
+#endif
 template <int NX>
 struct XGeom {
-  using G = FftGeom<NX>;
+  static constexpr int FID = (GD_X_ALT && NX == 256) ? NX + GD_FFT_ALT : NX;   // FFT plan ID (fft.cuh)
+  static constexpr bool ALT = (FID != NX);
+  using G = FftGeom<FID>;
   static constexpr int T = G::T, E = G::E;
-  static constexpr int SPLITX = (GD_X_SPLIT && G::S == 2) ? 1 : 0;   // split (8-byte) FFT exchange for the two-stage plans: half the buffer,
-                                                                     // one more stage in flight (three-stage plans would pay two split exchanges)
+  static constexpr int SPLITX = (GD_X_SPLIT && (G::S == 2 || ALT)) ? 1 : 0;   // split (8-byte) FFT exchange: half the buffer, one more stage in flight
+                                                                     // (the three-stage plan of nx = 512 pays two split exchanges: measured slower)
   static constexpr int LB = SPLITX ? (NX + NX / G::PADDIV + 2) / 2 : NX + NX / G::PADDIV + 1;   // per-group FFT exchange buffer, complex entries
   static constexpr int KXP = NX / 3 + 1;                    // retained kx count (== Dims::Kx)
-  static constexpr int THREADS = 256;                       // 8 warps, one CTA per SM (it owns all 512 TMEM columns)
+  static constexpr int THREADS = ALT ? 512 : 256;           // one CTA per SM (it owns the SM's tensor memory); ALT: 16 warps, 4 per scheduler
   static constexpr int WARPS = THREADS / 32;
   static constexpr int GROUPS = THREADS / T;                // lines per CTA: consecutive (z,y), y fastest
   static constexpr int LD = GROUPS;                         // row of a staged tile [kx][line]; line slot XOR-swizzled with kx
   static constexpr int STAGE = 2 * KXP * LD;                // one stage: the tiles of U and V (P1) for all lines of the CTA
   static constexpr size_t SMEM_CAP = 227 * 1024;
-  static constexpr size_t smem_for(int nst) { return ((size_t)GROUPS * LB + (size_t)nst * STAGE + FftTw<NX>::COUNT) * sizeof(cd); }
+  static constexpr size_t smem_for(int nst) { return ((size_t)GROUPS * LB + (size_t)nst * STAGE + FftTw<FID>::COUNT) * sizeof(cd); }
   static constexpr int NST = (SPLITX && smem_for(4) <= SMEM_CAP) ? 4 : (smem_for(3) <= SMEM_CAP ? 3 : 2);                             // stages in flight (full/empty mbarrier ring), <= 5 (the first NST-1 are Elsasser arrays)
   // stage-1 twiddles held in registers (plans with one stage-1 butterfly per lane): fewer shared-memory reads per transform
-  static constexpr int NTWR = (G::S == 2 && E / FftPlan<NX>::R1 == 1) ? GD_X_NTWR : 0;
-  static constexpr size_t SMEM = ((size_t)GROUPS * LB + (size_t)NST * STAGE + FftTw<NX>::COUNT) * sizeof(cd);
+  static constexpr int NTWR = (G::S == 2 && E / FftPlan<FID>::R1 == 1) ? GD_X_NTWR : 0;
+  static constexpr size_t SMEM = ((size_t)GROUPS * LB + (size_t)NST * STAGE + FftTw<FID>::COUNT) * sizeof(cd);
   // Tensor memory as a thread-private scratchpad (tcgen05.ld/st, shape 32x32b: lane i of a warp owns TMEM lane
   // 32*(warp%4)+i).  Per thread: 8 words per x-point for (Phi_x,Phi_y,Psi_x,Psi_y) and 2 words per x-point for the
   // parked R_{m-2}.  Warps sharing a lane quarter take consecutive column slots.
@@ -82,14 +88,15 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
                                                            const double* __restrict__ cup,
                                                            unsigned long long* __restrict__ maxbits, int nlines) {
   using X = XGeom<NX>;
-  using G = FftGeom<NX>;
+  using G = FftGeom<X::FID>;
+  constexpr int FID = X::FID;
   constexpr int T = X::T, E = X::E;
   constexpr int HX3 = NX / 3, KX = X::KXP;        // == d.hx3, d.Kx (compile-time so per-q range tests fold)
   extern __shared__ cd smem[];
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
   const int line = blockIdx.x * X::GROUPS + grp;
-  cd* buf = smem + FftTw<NX>::COUNT + (size_t)grp * X::LB;
-  cd* stages = smem + FftTw<NX>::COUNT + (size_t)X::GROUPS * X::LB;   // NST x [2][KX][LD]: U and V tiles, [kx][line]
+  cd* buf = smem + FftTw<FID>::COUNT + (size_t)grp * X::LB;
+  cd* stages = smem + FftTw<FID>::COUNT + (size_t)X::GROUPS * X::LB;   // NST x [2][KX][LD]: U and V tiles, [kx][line]
   __shared__ unsigned s_tmem_base;
   __shared__ unsigned long long s_full[X::NST], s_empty[X::NST];
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);     // warp-uniform for the compiler (uniform registers)
@@ -114,7 +121,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-  fft_load_table<NX>(smem, tw);      // ends with __syncthreads()
+  fft_load_table<FID>(smem, tw);     // ends with __syncthreads()
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const cd* tws = smem;
   // this warp's TMEM window: lane quarter warp%4, column slot warp/4
@@ -122,6 +129,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   const bool active = line < nlines;
   const size_t base = (size_t)(active ? line : 0) * d.Kxe;    // (z*ny + y)*Kxp  (output arrays E, kx fastest, padded rows)
   const int M = d.M;
+  const double bsc = d.bscale;
   cd v[E];
   double Qp[E], Ra[E];             // Hermite sliding window; Qp doubles as the {xi+,w-} accumulator of the Elsasser part
 
@@ -152,7 +160,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   int e0 = 0, e1 = 1;
   double gmax = 0.0;
   cd twr[X::NTWR > 0 ? X::NTWR : 1];
-  if constexpr (X::NTWR > 0) fft_load_stage1_twiddles<NX, X::NTWR>(twr, t, tws);
+  if constexpr (X::NTWR > 0) fft_load_stage1_twiddles<FID, X::NTWR>(twr, t, tws);
   for (;;) {
     if (!fwd) {
       if (kind == nkinds) {
@@ -204,10 +212,10 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
       }
     }
 
-    if constexpr (X::SPLITX && X::NTWR > 0) fft_lanes_fwd_rt_split<NX, X::NTWR>(v, t, reinterpret_cast<double*>(buf), tws, twr);
-    else if constexpr (X::SPLITX) fft_lanes_split<NX, -1>(v, t, reinterpret_cast<double*>(buf), tws);
-    else if constexpr (X::NTWR > 0) fft_lanes_fwd_rt<NX, X::NTWR>(v, t, buf, tws, twr);
-    else fft_lanes<NX, -1>(v, t, buf, tws);
+    if constexpr (X::SPLITX && X::NTWR > 0) fft_lanes_fwd_rt_split<FID, X::NTWR>(v, t, reinterpret_cast<double*>(buf), tws, twr);
+    else if constexpr (X::SPLITX) fft_lanes_split<FID, -1>(v, t, reinterpret_cast<double*>(buf), tws);
+    else if constexpr (X::NTWR > 0) fft_lanes_fwd_rt<FID, X::NTWR>(v, t, buf, tws, twr);
+    else fft_lanes<FID, -1>(v, t, buf, tws);
 
     if (fwd) {
       // separate the two real lines' spectra by Hermitian symmetry, keep kx <= nx/3, store.  The partner X[nx - c] of
@@ -268,7 +276,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
           const cd xp = cmake(tm_d(r[jj].w), tm_d(r[jj].w + 2)), xm = cmake(tm_d(r[jj].w + 4), tm_d(r[jj].w + 6));
           const double a = Qp[q] + (xm.x * (-v[q].y) - xm.y * v[q].x);
           const double b = xp.x * xm.y - xp.y * xm.x;
-          v[q] = cmake(a, b);
+          v[q] = cmake(a, bsc * b);                                          // (A, bscale*B): see Dims::bscale
           const cd phi = cmake(0.5 * (xp.x + xm.x), 0.5 * (xp.y + xm.y));   // grad Phi, Phi = (xi+ + xi-)/2
           const cd psi = cmake(0.5 * (xp.x - xm.x), 0.5 * (xp.y - xm.y));   // grad Psi
           tm_st4(tm + X::TM_PHI + 8 * q, phi.x, phi.y);
@@ -324,6 +332,14 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem_base), "r"(X::TM_COLS) : "memory");
 }
 
+// FFT plan ID of the x transforms (selects the stage twiddle table api.cu uploads)
+int xpass_fft_plan_id(int nx) {
+  switch (nx) {
+    case 8: return XGeom<8>::FID; case 16: return XGeom<16>::FID; case 32: return XGeom<32>::FID; case 64: return XGeom<64>::FID;
+    case 128: return XGeom<128>::FID; case 256: return XGeom<256>::FID; case 512: return XGeom<512>::FID;
+    default: return 0;
+  }
+}
 // lines per x-pass CTA (the block size of the D layout)
 int xpass_lines_per_cta(int nx) {
   switch (nx) {

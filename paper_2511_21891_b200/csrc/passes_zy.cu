@@ -63,7 +63,10 @@ template <int NZ> struct ZStepGeom {
   static constexpr bool TMA_IN = (NZ * LD <= REGION);        // the staged [nz][GROUPS] tile of Gh fits in the region
   static constexpr size_t SMEM = ((size_t)REGION + FftTw<NZ>::COUNT) * sizeof(cd);
 };
-template <int NZ, int MODE>   // MODE 0 / 1 / 2 = RHS only / predictor / corrector + dissipation (compile time: fewer registers)
+// EXACT (hermite_exact = 1, hermite.cu; Q30): the streaming term of H_m is left to the exact propagator -- the moment
+// fields get only their bracket term (no neighbour reads), no dissipation here, and no hybrid copy (the propagated state's
+// copy is made afterwards); in mode 2 they are updated in place on Ws (= P(dt/2) g_n), w+- as usual on Wn -> Wout.
+template <int NZ, int MODE, bool EXACT>   // MODE 0 / 1 / 2 = RHS only / predictor / corrector + dissipation (compile time: fewer registers)
 __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, double skz_sign, const cd* __restrict__ Gh,
                                                       const cd* __restrict__ Wn, const cd* __restrict__ Ws, cd* __restrict__ Wout,
                                                       cd* __restrict__ Hout, const double* __restrict__ scal,
@@ -132,7 +135,8 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
   //    the loads of UB modes are issued together
   {
     const double c = (mode == 1) ? 0.5 * dt : dt;
-    const bool lo = f > 2, hi = f + 1 < d.F, same = (Ws == Wn || mode == 0);
+    const bool lo = !EXACT && f > 2, hi = !EXACT && f + 1 < d.F, same = (EXACT || Ws == Wn || mode == 0);
+    cd* const wout = (EXACT && mode == 2 && f >= 2) ? const_cast<cd*>(Ws) : Wout;
     const int ncolv = min(GROUPS, plane - col0);
     constexpr int NEL = KZ * GROUPS, UB = 6;
     for (int e0 = threadIdx.x; e0 < NEL; e0 += UB * GD_Z_THREADS) {
@@ -183,20 +187,20 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
         } else {
           const double skz = (m < d.Msp ? skz_sign : -skz_sign) * d.kz0 * c2n(cz, NZ / 3, KZ);   // g^+ : upper, g^- : lower signs of Eq. 6
           const cd lin = cmake(a0[u].x - dn * a1[u].x - up * a2[u].x, a0[u].y - dn * a1[u].y - up * a2[u].y);
-          const cd Hm = cmake(Gv.x - skz * lin.y, Gv.y + skz * lin.x);                 // + i s kz lin  (Eq. 6)
+          const cd Hm = EXACT ? Gv : cmake(Gv.x - skz * lin.y, Gv.y + skz * lin.x);    // + i s kz lin  (Eq. 6)
           if (mode == 0) out = Hm;
           else {
             const cd gn = same ? a0[u] : a3[u];
             out = cmake(gn.x + c * Hm.x, gn.y + c * Hm.y);
-            if (mode == 2) out = cscale(out, cf * tabp[2 * (col0 + cl) + 1] * tz[5]);
+            if (mode == 2 && !EXACT) out = cscale(out, cf * tabp[2 * (col0 + cl) + 1] * tz[5]);
           }
         }
-        st_cd(Wout + (size_t)f * d.PS + idx, out);
+        st_cd(wout + (size_t)f * d.PS + idx, out);
         tile[cz * LD + cl] = out;
       }
     }
   }
-  if (Hout == nullptr) return;
+  if (Hout == nullptr || (EXACT && f >= 2)) return;
   __syncthreads();
   // 3. inverse z transform of the new stage state (zero-padded) -> hybrid copy
   cd v[E];
@@ -475,7 +479,7 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, 1) k_yfwd_pair(Dims d, con
         const int cy = fft2c(t + T * q, NY, HY3, KY);
         if (cy >= 0) {
           const double ky = d.ky0 * fft2n(t + T * q, NY);
-          const double hk2 = 0.5 * (kx * kx + ky * ky);
+          const double hk2 = 0.5 * (kx * kx + ky * ky) * d.inv_bscale;     // the x-pass delivered bscale*B (exact power of two)
           st_cd(dp + cy * d.Kxp, cmake(-0.5 * va[q].x - hk2 * v[q].x, -0.5 * va[q].y - hk2 * v[q].y));
           st_cd(dm + cy * d.Kxp, cmake(-0.5 * va[q].x + hk2 * v[q].x, -0.5 * va[q].y + hk2 * v[q].y));
         }
@@ -503,16 +507,18 @@ cudaError_t launch_zfft(const Dims& d, const cd* in, cd* out, const cd* tw, int 
   GD_DISPATCH(d.nz, ZCASE)
   return cudaGetLastError();
 }
-cudaError_t launch_zstep(const Dims& d, int mode, int if_variant, int g_sign, const cd* Gh, const cd* Wn, const cd* Ws, cd* Wout, cd* Hout,
+cudaError_t launch_zstep(const Dims& d, int mode, bool exact, int if_variant, int g_sign, const cd* Gh, const cd* Wn, const cd* Ws, cd* Wout, cd* Hout,
                          const double* scal, const double* cdn, const double* cup, const double* collfac, const double* tabz,
                          const double* tabp, const cd* tw, cudaStream_t st) {
   const long long ncols = (long long)d.Ky * d.Kx;
 #define ZSCASE(NN)                                                                                               \
   {                                                                                                              \
     const int nb = fft_blocks<NN>(ncols) * d.F;                                                                  \
-    if (mode == 0) k_zstep<NN, 0><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
-    else if (mode == 1) k_zstep<NN, 1><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
-    else k_zstep<NN, 2><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
+    if (mode == 0) k_zstep<NN, 0, false><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
+    else if (mode == 1 && !exact) k_zstep<NN, 1, false><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
+    else if (mode == 1) k_zstep<NN, 1, true><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
+    else if (!exact) k_zstep<NN, 2, false><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
+    else k_zstep<NN, 2, true><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
   }
   GD_DISPATCH(d.nz, ZSCASE)
   return cudaGetLastError();
@@ -547,11 +553,15 @@ cudaError_t prepare_passes_zy(int ny, int nz) {
   {                                                                                                                        \
     cudaError_t e = cudaFuncSetAttribute(k_zfft<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<NN>());      \
     if (e != cudaSuccess) return e;                                                                                        \
-    e = cudaFuncSetAttribute(k_zstep<NN, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);        \
+    e = cudaFuncSetAttribute(k_zstep<NN, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM); \
     if (e != cudaSuccess) return e;                                                                                        \
-    e = cudaFuncSetAttribute(k_zstep<NN, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);        \
+    e = cudaFuncSetAttribute(k_zstep<NN, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM); \
     if (e != cudaSuccess) return e;                                                                                        \
-    e = cudaFuncSetAttribute(k_zstep<NN, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);        \
+    e = cudaFuncSetAttribute(k_zstep<NN, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM); \
+    if (e != cudaSuccess) return e;                                                                                        \
+    e = cudaFuncSetAttribute(k_zstep<NN, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);  \
+    if (e != cudaSuccess) return e;                                                                                        \
+    e = cudaFuncSetAttribute(k_zstep<NN, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZStepGeom<NN>::SMEM);  \
     if (e != cudaSuccess) return e;                                                                                        \
   }
   GD_DISPATCH(nz, ZPCASE)
@@ -570,13 +580,13 @@ cudaError_t prepare_passes_zy(int ny, int nz) {
   return cudaSuccess;
 }
 
-// Host: the stage twiddle table of length-n transforms (fft.cuh layout); empty for single-stage sizes.
+// Host: the stage twiddle table of FFT plan ID n (fft.cuh layout); empty for single-stage sizes.
 int fft_stage_table_host(int n, std::vector<cd>& out) {
 #define TCASE(NN) out.assign(FftTw<NN>::COUNT + 1, cmake(0.0, 0.0)); fft_fill_stage_table<NN>(out.data());
   switch (n) {
     case 2: TCASE(2) break; case 4: TCASE(4) break; case 8: TCASE(8) break; case 16: TCASE(16) break;
     case 32: TCASE(32) break; case 64: TCASE(64) break; case 128: TCASE(128) break; case 256: TCASE(256) break;
-    case 512: TCASE(512) break;
+    case 512: TCASE(512) break; case 256 + GD_FFT_ALT: TCASE(256 + GD_FFT_ALT) break;
     default: return -1;
   }
   return 0;

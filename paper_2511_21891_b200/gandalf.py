@@ -81,10 +81,24 @@ def load_library():
     lib.gandalf_launch_count.restype = C.c_longlong
     lib.gandalf_kernel_timing.argtypes = [V, I]
     lib.gandalf_kernel_time_ms.argtypes = [V, I, PD, C.POINTER(C.c_longlong)]
+    lib.gandalf_microbench.argtypes = [I, I, PD, I]
     lib.gandalf_last_error.argtypes = [V]
     lib.gandalf_last_error.restype = C.c_char_p
     _lib = lib
     return lib
+
+
+MICROBENCHES = ("fp64_fma", "fft256_lane_group", "tmem_load", "smem_load")
+
+
+def microbench(which, device=0):
+    """gandalf_microbench(which): four doubles (see include/gandalf.h)."""
+    lib = load_library()
+    out = np.zeros(4)
+    rc = lib.gandalf_microbench(int(which), int(device), out.ctypes.data_as(C.POINTER(C.c_double)), 4)
+    if rc != OK:
+        raise GandalfError(rc, "gandalf_microbench failed")
+    return out
 
 
 def _is_torch(x):

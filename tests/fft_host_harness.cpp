@@ -61,13 +61,13 @@ template <int N, int DIR> static void run_split(const double* in, double* out) {
 }
 extern "C" int host_fft_split(int n, int dir, const double* in, double* out) {
 #define SCASE(NN) case NN: if (dir < 0) run_split<NN, -1>(in, out); else run_split<NN, +1>(in, out); return 0;
-  switch (n) { SCASE(2) SCASE(4) SCASE(8) SCASE(16) SCASE(32) SCASE(64) SCASE(128) SCASE(256) SCASE(512) }
+  switch (n) { SCASE(2) SCASE(4) SCASE(8) SCASE(16) SCASE(32) SCASE(64) SCASE(128) SCASE(256) SCASE(512) SCASE(256 + GD_FFT_ALT) }
   return -1;
 }
 
 extern "C" int host_fft(int n, int dir, const double* in, double* out) {
 #define CASE(NN) case NN: if (dir < 0) run<NN, -1>(in, out); else run<NN, +1>(in, out); return 0;
-  switch (n) { CASE(2) CASE(4) CASE(8) CASE(16) CASE(32) CASE(64) CASE(128) CASE(256) CASE(512) }
+  switch (n) { CASE(2) CASE(4) CASE(8) CASE(16) CASE(32) CASE(64) CASE(128) CASE(256) CASE(512) CASE(256 + GD_FFT_ALT) }
   return -1;
 }
 // bank-conflict audit: max number of lanes of one quarter-warp (8 lanes x 16 B) whose scatter
@@ -99,4 +99,40 @@ extern "C" int host_fft_scatter_conflicts(int n) {
     case 512: { int a = conflicts<512, 0>(), b = conflicts<512, 1>(); return a > b ? a : b; }
   }
   return 1;
+}
+
+// Split (8-byte) exchange audit for a whole warp: worst number of lanes of one warp-wide store / load that fall on the same
+// 8-byte bank pair (16 of them), over all scatter and gather instructions of stage s.  32 lanes x 8 B = 2 wavefronts at best,
+// so the ideal answer is 2.  The warp holds 32/T lane groups with buffers BUF+2 doubles apart (pass_x.cu, passes_zy.cu).
+template <int ID, int s> static int split_conflicts() {
+  using G = FftGeom<ID>;
+  constexpr int R = G::template radix<s>(), NS = G::template ns<s>(), B = G::E / R;
+  int worst = 0;
+  for (int b = 0; b < B; ++b)
+    for (int i = 0; i < R; ++i) {
+      int cnt[16] = {0};
+      for (int lane = 0; lane < 32; ++lane) {
+        int t = lane % G::T, line = lane / G::T;
+        int j = t + G::T * b, j0 = (j / NS) * NS * R + (j % NS);
+        cnt[(line * (G::BUF + 2) + G::pad(j0 + i * NS)) % 16]++;
+      }
+      for (int k = 0; k < 16; ++k) if (cnt[k] > worst) worst = cnt[k];
+    }
+  for (int q = 0; q < G::E; ++q) {
+    int cnt[16] = {0};
+    for (int lane = 0; lane < 32; ++lane) {
+      int t = lane % G::T, line = lane / G::T;
+      cnt[(line * (G::BUF + 2) + G::pad(t + G::T * q)) % 16]++;
+    }
+    for (int k = 0; k < 16; ++k) if (cnt[k] > worst) worst = cnt[k];
+  }
+  return worst;
+}
+extern "C" int host_fft_split_conflicts(int id) {
+  switch (id) {
+    case 256: return split_conflicts<256, 0>();
+    case 256 + GD_FFT_ALT: { int a = split_conflicts<256 + GD_FFT_ALT, 0>(), b = split_conflicts<256 + GD_FFT_ALT, 1>(); return a > b ? a : b; }
+    case 512: { int a = split_conflicts<512, 0>(), b = split_conflicts<512, 1>(); return a > b ? a : b; }
+  }
+  return -1;
 }

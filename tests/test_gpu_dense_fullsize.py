@@ -86,8 +86,15 @@ def test_dense_same_grid_512x512x8(M):
     gm = synth.dense_random(*shape, M, seed=5200, decay=4.0) if M else None
     o.set_state(z, gm); g.set_state(z, gm)
     ew, eg = _rhs_err(o, g)
-    print(f"dense 512x512x8 M={M}: RHS rel L2 dw {ew:.2e} dg {eg:.2e}")
-    assert ew <= 1e-12 and eg <= 1e-12
+    exact = _exact_elsasser_rhs(o)
+    dw_o, dw_g = o.rhs()[0], g.rhs()[0]
+    e_o = max(_err_ld(dw_o[a], exact[a]) for a in range(2))
+    e_g = max(_err_ld(dw_g[a], exact[a]) for a in range(2))
+    print(f"dense 512x512x8 M={M}: RHS rel L2 gpu vs oracle dw {ew:.2e} dg {eg:.2e}; vs extended precision: oracle {e_o:.2e}, gpu {e_g:.2e}")
+    # 341 x 341 retained modes per plane: the flat round-off floor of B^ times kperp^2 (up to 5.8e4) puts BOTH sides at
+    # ~1e-12 from the exact value (printed above); the GPU must be within 1e-12 of the exact value, or no worse than the oracle
+    assert e_g <= max(1e-12, 1.25 * e_o) and ew <= 1.01 * (e_o + e_g) + 1e-15 and ew <= 3e-12
+    assert eg <= 1e-12
     o.step(1e-3, 2); g.step(1e-3, 2)
     ez, egs = _state_err(o, g)
     assert ez <= 1e-10 and egs <= 1e-10
@@ -106,70 +113,61 @@ def test_dense_same_grid_config4b_size_rhs():
     assert ew <= 1e-12
 
 
-# ---- conditioning evidence: rough spectrum, 512 points, both sides against an extended-precision evaluation ------------
-def _conv2(a, b):
-    """2-D linear convolution of longdouble-complex arrays indexed [ky][kx] (small ky extent)."""
-    out = np.zeros((a.shape[0] + b.shape[0] - 1, a.shape[1] + b.shape[1] - 1), dtype=np.clongdouble)
-    for i in range(a.shape[0]):
-        for j in range(b.shape[0]):
-            out[i + j] += np.convolve(a[i], b[j])
-    return out
-
-
-def _exact_elsasser_rhs(wp, wm, nx, ny):
-    """N+- of Eq. 1 on the kz = 0 plane from the convolution sum, in numpy.longdouble.  wp, wm: FULL spectra [ny][nx] of
-    the vorticities (FFT order).  Returns [ny][nx] arrays (retained band only)."""
-    hx, hy = nx // 3, ny // 3
-    nxs = np.arange(-hx, hx + 1)
-    nys = np.arange(-hy, hy + 1)
-    PX, PY = np.meshgrid(nxs.astype(np.longdouble), nys.astype(np.longdouble))
-    k2 = PX * PX + PY * PY
-
-    def centred(a):
-        return a[np.ix_(nys % ny, nxs % nx)].astype(np.clongdouble)
-
-    w = [centred(wp), centred(wm)]
+# ---- arbiter in extended precision ---------------------------------------------------------------------------------
+def _exact_elsasser_rhs(o):
+    """N+- of Eq. 1 at the oracle's (projected) state, evaluated pseudo-spectrally in numpy.longdouble (64-bit mantissa,
+    numpy's own FFT): a third evaluation, ~1e-19 accurate, used only to tell WHOSE round-off a GPU-vs-oracle difference
+    is.  Returns half-plane arrays (2, nz, ny, nx//2+1) as clongdouble."""
+    nx, ny, nz = o.nx, o.ny, o.nz
+    LD, CLD = np.longdouble, np.clongdouble
+    w = [o.get_full(f).astype(CLD) for f in range(2)]
+    two_pi = 2 * np.arccos(LD(-1))
+    kx = (two_pi / LD(o.params.Lx)) * np.array(synth.mode_numbers(nx), dtype=LD)[None, None, :]
+    ky = (two_pi / LD(o.params.Ly)) * np.array(synth.mode_numbers(ny), dtype=LD)[None, :, None]
+    k2 = kx * kx + ky * ky
     with np.errstate(divide="ignore", invalid="ignore"):
-        xi = [np.where(k2 > 0, -v / k2, 0) for v in w]
+        xi = [np.where(k2 > 0, -v / k2, 0).astype(CLD) for v in w]
+    n = LD(nx * ny * nz)
 
-    def bracket(f, g):          # sum_{p+q=k} (p_y q_x - p_x q_y) f(p) g(q)
-        full = _conv2(PY * f, PX * g) - _conv2(PX * f, PY * g)
-        return full[2 * hy - hy: 2 * hy + hy + 1, 2 * hx - hx: 2 * hx + hx + 1]     # centre: k in the retained band
-    A = bracket(xi[0], w[1]) + bracket(xi[1], w[0])
-    B = bracket(xi[0], xi[1])
-    Np = -0.5 * (A + k2 * B)            # -1/2 [A - lap B], lap -> -k2
-    Nm = -0.5 * (A - k2 * B)
-    out = []
-    for N in (Np, Nm):
-        full = np.zeros((ny, nx), dtype=np.clongdouble)
-        full[np.ix_(nys % ny, nxs % nx)] = N
-        out.append(full)
-    return out
+    def grad(fh):            # numpy's ifftn carries 1/N: undo it (physical normalisation, Eq. 9)
+        return (np.fft.ifftn(1j * kx * fh) * n).real, (np.fft.ifftn(1j * ky * fh) * n).real
+
+    mx = np.abs(np.array(synth.mode_numbers(nx)))[None, None, :]
+    my = np.abs(np.array(synth.mode_numbers(ny)))[None, :, None]
+    mz = np.abs(np.array(synth.mode_numbers(nz)))[:, None, None]
+    keep = (3 * mx <= nx) & (3 * my <= ny) & (3 * mz <= nz)
+
+    def bracket(P, Q):
+        return np.where(keep, np.fft.fftn((P[0] * Q[1] - P[1] * Q[0]).astype(CLD)) / n, 0)
+
+    gxi, gw = [grad(v) for v in xi], [grad(v) for v in w]
+    A = bracket(gxi[0], gw[1]) + bracket(gxi[1], gw[0])
+    B = bracket(gxi[0], gxi[1])
+    hx = nx // 2 + 1
+    return np.stack([(-0.5 * (A + k2 * B))[:, :, :hx], (-0.5 * (A - k2 * B))[:, :, :hx]])
 
 
-@pytest.mark.parametrize("shape", [(512, 8, 2), (8, 512, 2)])
-def test_rough_spectrum_512_points_oracle_and_gpu_vs_extended_precision(shape):
+def _err_ld(a, ref):
+    d = a.astype(np.clongdouble) - ref
+    return float(np.sqrt((np.abs(d) ** 2).sum()) / np.sqrt((np.abs(ref) ** 2).sum()))
+
+
+@pytest.mark.parametrize("shape,decay", [((512, 8, 2), 1.5), ((8, 512, 2), 1.5), ((512, 512, 8), 4.0)])
+def test_whose_roundoff_oracle_and_gpu_vs_extended_precision(shape, decay):
+    """Where GPU and oracle differ by more than 1e-12 (rough |n|^-1.5 spectrum at 512 points; dense |n|^-4 spectrum on a
+    512 x 512 plane) an extended-precision evaluation arbitrates: both sides sit at the same distance from the exact
+    value -- the excess is the conditioning of -+1/2 kperp^2 B^ (round-off of B^ times kperp^2 up to 6e4), not an error
+    of the kernels.  The GPU must be within 1e-12 of the exact value or at least as accurate as the oracle."""
     nx, ny, nz = shape
     o, g = _pair(shape, dict(M=0))
-    z = synth.dense_random(nx, ny, nz, 2, seed=9000 + nx, decay=1.5)
+    z = synth.dense_random(nx, ny, nz, 2, seed=9000 + nx + ny, decay=decay)
     o.set_state(z); g.set_state(z)
-    wp, wm = o.get_full(0)[0], o.get_full(1)[0]           # nz = 2: only the kz = 0 plane survives Eq. 20
-    exact = _exact_elsasser_rhs(wp, wm, nx, ny)
+    exact = _exact_elsasser_rhs(o)
     dw_o, _ = o.rhs()
     dw_g, _ = g.rhs()
-    hxp = nx // 2 + 1
-    errs = {}
-    for name, dw in (("oracle", dw_o), ("gpu", dw_g)):
-        e = 0.0
-        for a in range(2):
-            ref = exact[a][:, :hxp]
-            d = dw[a][0].astype(np.clongdouble) - ref
-            e = max(e, float(np.sqrt((np.abs(d) ** 2).sum()) / np.sqrt((np.abs(ref) ** 2).sum())))
-        errs[name] = e
+    e_o = max(_err_ld(dw_o[a], exact[a]) for a in range(2))
+    e_g = max(_err_ld(dw_g[a], exact[a]) for a in range(2))
     between = max(rel_l2(dw_g[a], dw_o[a]) for a in range(2))
-    print(f"rough |n|^-1.5 spectrum {shape}: oracle vs exact {errs['oracle']:.2e}, gpu vs exact {errs['gpu']:.2e}, "
-          f"gpu vs oracle {between:.2e}")
-    # both implementations are equally far from the exact value: the excess over 1e-12 on rough data is the conditioning
-    # of the bracket (k_perp^2 B amplifies eps * max-amplitude), not an error of either side
-    assert errs["gpu"] <= 5e-12 and errs["oracle"] <= 5e-12
-    assert errs["gpu"] <= 3.0 * errs["oracle"] + 1e-13
+    print(f"whose round-off {shape} decay {decay}: oracle vs exact {e_o:.2e}, gpu vs exact {e_g:.2e}, gpu vs oracle {between:.2e}")
+    assert e_g <= max(1e-12, 1.25 * e_o), (e_g, e_o)
+    assert between <= 1.01 * (e_o + e_g) + 1e-15 and between <= 5e-12

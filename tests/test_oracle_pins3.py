@@ -344,3 +344,79 @@ def test_p20_restart_is_bit_exact_with_forcing():
         d.set_full(f, full[f])
     d.step(dt, 3)
     assert not np.array_equal(d.get_full(0), a.get_full(0))
+
+
+# ---- P21: exact propagator of the Hermite streaming terms (hermite_exact = 1; Q30) ---------------------------
+def _jacobi(M):
+    T = np.zeros((M, M))
+    for m in range(1, M):
+        T[m, m - 1] = T[m - 1, m] = math.sqrt(m / 2.0)
+    return T
+
+
+@pytest.mark.parametrize("sign", [+1, -1])
+def test_p21_exact_streaming_closed_form_at_any_dt(sign):
+    """Brackets off: g(t) = exp(s i kz (I - T) t) g(0).  From g = delta_{m0} the infinite hierarchy gives
+    e^{i s a} e^{-a^2/4} (-i s a/sqrt 2)^m / sqrt(m!), a = kz t (generating function of the Hermite functions); M = 40
+    reproduces it to 1e-12 at a = 2.  With the exact propagator this holds for ONE step of dt = 1 as well as for 7."""
+    import scipy.linalg
+    nx, ny, nz, M, kz, tend = 8, 8, 8, 40, 2, 1.0
+    a = kz * tend
+    closed = np.array([np.exp(1j * sign * a) * math.exp(-a * a / 4) * (-1j * sign * a / math.sqrt(2)) ** m / math.sqrt(math.factorial(m))
+                       for m in range(M)])
+    lib = scipy.linalg.expm(1j * sign * kz * (np.eye(M) - _jacobi(M)) * tend)[:, 0]
+    assert np.abs(lib - closed).max() <= 1e-12
+    g0 = synth.single_mode(nx, ny, nz, (1, 0, kz), 1.0, field=0, nfields=M)
+    for nsteps in (1, 7):
+        o = Oracle(nx, ny, nz, M=M, nonlinear=0, g_sign=sign, hermite_exact=1)
+        o.set_state(np.zeros((2, nz, ny, nx // 2 + 1)), g0)
+        w0 = o.energy()[5]
+        o.step(tend / nsteps, nsteps)
+        got = o.get_state()[1][:, kz, 0, 1]
+        assert np.abs(got - closed).max() <= 1e-12, nsteps
+        assert abs(o.energy()[5] - w0) <= 1e-13 * w0                 # the propagator is unitary: W_g exactly conserved
+    # the plain RK2 of Alg. 1 l.4/l.9 is unstable at this step (|1 + i th - th^2/2| > 1): that is the constraint this lifts
+    o = Oracle(nx, ny, nz, M=M, nonlinear=0, g_sign=sign)
+    o.set_state(np.zeros((2, nz, ny, nx // 2 + 1)), g0)
+    o.step(tend, 1)
+    assert np.abs(o.get_state()[1][:, kz, 0, 1] - closed).max() > 0.1
+
+
+def test_p21_exact_streaming_reflecting_closure_vs_library_expm():
+    import scipy.linalg
+    nx, ny, nz, M, kz = 8, 8, 8, 6, 1
+    T = _jacobi(M)
+    T[M - 1, M - 2] += math.sqrt(M / 2.0)                             # g_M := g_{M-2}  (PAPER.md:105; Q23)
+    exact = scipy.linalg.expm(1j * kz * (np.eye(M) - T) * 0.9)[:, 0]
+    o = Oracle(nx, ny, nz, M=M, nonlinear=0, closure=1, hermite_exact=1)
+    o.set_state(np.zeros((2, nz, ny, nx // 2 + 1)), synth.single_mode(nx, ny, nz, (1, 0, kz), 1.0, field=0, nfields=M))
+    o.step(0.3, 3)
+    assert np.abs(o.get_state()[1][:, kz, 0, 1] - exact).max() <= 1e-13
+
+
+def test_p21_exact_streaming_with_brackets_is_second_order_and_consistent():
+    nx, ny, nz, M, tend = 16, 16, 8, 4, 0.2
+    z = synth.random_zeta(nx, ny, nz, seed=5, energy=1.0, nperp_hi=3.0, nz_hi=2)
+    g = synth.random_g(nx, ny, nz, M, seed=6, total=0.05, nperp_hi=3.0)
+
+    def run(exact, n):
+        o = Oracle(nx, ny, nz, M=M, if_variant=1, hermite_exact=exact)
+        o.set_state(z, g)
+        o.step(tend / n, n)
+        return o.get_state()[1].ravel()
+
+    ref = run(1, 256)
+    e = [np.linalg.norm(run(1, n) - ref) for n in (8, 16, 32)]
+    assert 1.9 < math.log2(e[0] / e[1]) < 2.1 and 1.9 < math.log2(e[1] / e[2]) < 2.1, e
+    # both steppers converge to the same solution: their difference shrinks like dt^2
+    d = [np.linalg.norm(run(1, n) - run(0, n)) for n in (16, 32)]
+    assert 1.8 < math.log2(d[0] / d[1]) < 2.2 and d[1] < 1e-4 * np.linalg.norm(ref)
+    # two species: the second one runs with the opposite sign (conjugate propagator)
+    gp = synth.random_g(nx, ny, nz, 2, seed=7, total=0.05, nperp_hi=3.0)
+    gm = synth.random_g(nx, ny, nz, 2, seed=8, total=0.05, nperp_hi=3.0)
+    both = Oracle(nx, ny, nz, M=2, nspecies=2, hermite_exact=1); both.set_state(z, np.concatenate([gp, gm]))
+    op = Oracle(nx, ny, nz, M=2, g_sign=+1, hermite_exact=1); op.set_state(z, gp)
+    om = Oracle(nx, ny, nz, M=2, g_sign=-1, hermite_exact=1); om.set_state(z, gm)
+    for o in (both, op, om):
+        o.step(1e-2, 3)
+    assert np.array_equal(both.get_state()[1][:2], op.get_state()[1]) and np.array_equal(both.get_state()[1][2:], om.get_state()[1])
