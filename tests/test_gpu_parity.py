@@ -357,3 +357,34 @@ def test_finding_q28_advective_cfl_is_not_sufficient_with_moments():
     g2.step(0.0, 400)
     h = g2.energy_history()
     assert np.isfinite(h).all() and h[-1, 6] < 0.05 and 1.0 < h[-1, 1] < 3.0
+
+
+@pytest.mark.parametrize("shape,M,extra,dt", [
+    ((32, 16, 8), 4, dict(), 2e-3),
+    ((16, 32, 16), 9, dict(if_variant=1, g_sign=-1, nu_coll=0.7, p=1.5, eta=0.5, r=2, eta_normalized=1, eta_g=0.3), 2e-3),
+    ((32, 32, 8), 3, dict(nspecies=2), 2e-3),
+    ((16, 16, 32), 16, dict(nonlinear=0), 0.4),            # a step the plain RK2 of Alg. 1 cannot take (dt kz sqrt(2M) >> 1)
+    ((64, 64, 32), 16, dict(nu_coll=1.0, p=2.0, eta=1.0, r=2, eta_normalized=1), 5e-4),   # config 2's shape
+])
+def test_hermite_exact_propagator_matches_oracle(shape, M, extra, dt):
+    """hermite_exact = 1 (Q30; PAPER.md:657, 829 name exponential integrators as future work): the streaming /
+    phase-mixing terms of Eq. 6 by exp(s i kz (I - T) dt) per kz -- k_hermite_propagator / k_hermite_apply against the
+    oracle's eigen-decomposition route, brackets by the midpoint rule on both sides."""
+    prm = dict(M=M, hermite_exact=1, **extra)
+    o, g = _pair(shape, prm)
+    nsp = extra.get("nspecies", 1)
+    z = synth.dense_random(*shape, 2, seed=31, decay=2.0)
+    gm = synth.dense_random(*shape, M * nsp, seed=32, decay=2.0)
+    o.set_state(z, gm); g.set_state(z, gm)
+    o.step(dt, 10); g.step(dt, 10)
+    _check_state(o, g, TOL_10STEPS)
+    _check_history(o, g)
+    if extra.get("nonlinear", 1) == 0 and not extra.get("nu_coll"):
+        h = g.energy_history()
+        assert abs(h[-1, 6] - h[0, 6]) <= 1e-12 * h[0, 6]      # unitary propagator: W_g conserved at any dt
+
+
+def test_hermite_exact_rejects_unsupported_closure():
+    from paper_2511_21891_b200.gandalf import Gandalf, GandalfError
+    with pytest.raises(GandalfError):
+        Gandalf(16, 16, 8, M=4, hermite_exact=1, closure=1)
