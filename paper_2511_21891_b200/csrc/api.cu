@@ -21,7 +21,7 @@ cudaError_t prepare_passes_zy(int ny, int nz);
 int xpass_lines_per_cta(int nx);
 int xpass_fft_plan_id(int nx);
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
-                         unsigned long long* maxbits, cudaStream_t st, bool prepare_only);
+                         unsigned long long* maxbits, int num_sms, cudaStream_t st, bool prepare_only);
 cudaError_t launch_zstep(const Dims& d, int mode, bool exact, int if_variant, int g_sign, const cd* Gh, const cd* Wn, const cd* Ws, cd* Wout, cd* Hout,
                          const double* scal, const double* cdn, const double* cup, const double* collfac, const double* tabz,
                          const double* tabp, const cd* tw, cudaStream_t st);
@@ -233,7 +233,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (e == cudaSuccess) e = upload_twiddles(&c->twx, xpass_fft_plan_id(d.nx), c->st);
   if (e == cudaSuccess) e = upload_twiddles(&c->twy, d.ny, c->st);
   if (e == cudaSuccess) e = upload_twiddles(&c->twz, d.nz, c->st);
-  if (e == cudaSuccess) e = launch_xpass(d, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, c->st, true);
+  if (e == cudaSuccess) e = launch_xpass(d, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, c->st, true);
   if (e == cudaSuccess) e = prepare_passes_zy(d.ny, d.nz);
   c->num_sms = 0;
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, p->device);
@@ -343,7 +343,7 @@ static int rhs_pipeline(gandalf_ctx* c, bool want_cfl) {
   if (want_cfl) GD_CUDA(c, timed(c, -1, 1, [&] { return launch_zero_u64(c->maxbits, c->st); }));
   GD_CUDA(c, timed(c, KC_YINV, d.M > 0 ? 2 : 1, [&] { return launch_yinv(d, c->H, c->D, c->twy, c->num_sms, c->st); }));
   GD_CUDA(c, timed(c, KC_XPASS, 1, [&] {
-    return launch_xpass(d, c->D, c->E, c->twx, c->cdn, c->cup, want_cfl ? c->maxbits : nullptr, c->st, false);
+    return launch_xpass(d, c->D, c->E, c->twx, c->cdn, c->cup, want_cfl ? c->maxbits : nullptr, c->num_sms, c->st, false);
   }));
   if (!c->p.nonlinear) return GANDALF_OK;
   GD_CUDA(c, timed(c, KC_YFWD, d.M > 0 ? 2 : 1, [&] { return launch_yfwd(d, c->E, c->Gh, c->twy, c->num_sms, c->st); }));

@@ -121,7 +121,14 @@ template <> struct FftPlan<32>  { static constexpr int T = 4,  E = 8,  S = 2, R0
 template <> struct FftPlan<64>  { static constexpr int T = 8,  E = 8,  S = 2, R0 = 8,  R1 = 8,  R2 = 1, PAD = R0; };
 template <> struct FftPlan<128> { static constexpr int T = 8,  E = 16, S = 2, R0 = 16, R1 = 8,  R2 = 1, PAD = R0; };
 template <> struct FftPlan<256> { static constexpr int T = 16, E = 16, S = 2, R0 = 16, R1 = 16, R2 = 1, PAD = R0; };
-template <> struct FftPlan<512> { static constexpr int T = 32, E = 16, S = 3, R0 = 8,  R1 = 8,  R2 = 8, PAD = R0; };
+// 512 = 16*4*8: measured against 8*8*8, 16*16*2 and 16*8*4 at config 4b (P1 1.03 / 0.87 / 0.87 / 0.84 ms: the radix-16 first stage
+// keeps k_yinv<512> from spilling and its split exchange is conflict-free, 2 wavefronts per 8-byte access instead of 3)
+#ifndef GD_FFT512_R0
+#define GD_FFT512_R0 16
+#define GD_FFT512_R1 4
+#define GD_FFT512_R2 8
+#endif
+template <> struct FftPlan<512> { static constexpr int T = 32, E = 16, S = 3, R0 = GD_FFT512_R0, R1 = GD_FFT512_R1, R2 = GD_FFT512_R2, PAD = R0; };
 template <> struct FftPlan<256 + GD_FFT_ALT> { static constexpr int T = 32, E = 8, S = 3, R0 = 8, R1 = 8, R2 = 4, PAD = 16; };   // pad 16: 8-byte exchange conflict-free on 32 lanes
 
 template <int ID> struct FftGeom {

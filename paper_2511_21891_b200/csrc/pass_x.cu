@@ -21,6 +21,9 @@
 #ifndef GD_X_NTWR
 #define GD_X_NTWR 8
 #endif
+#ifndef GD_X_STAGGER_NS
+#define GD_X_STAGGER_NS 0
+#endif
 #ifndef GD_X_ALT
 #define GD_X_ALT 0        // 1: nx = 256 on one WARP per line (plan 8*8*4, 8 points per lane, 16 warps per SM).  Measured SLOWER (1.72 vs 1.40 ms at 4a:
                           // the second exchange costs more than the extra warps hide; bare transform 1.35 vs 2.53 G/s) -- kept as a tested option
@@ -94,7 +97,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   constexpr int HX3 = NX / 3, KX = X::KXP;        // == d.hx3, d.Kx (compile-time so per-q range tests fold)
   extern __shared__ cd smem[];
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
-  const int line = blockIdx.x * X::GROUPS + grp;
+  const int nblocks = (nlines + X::GROUPS - 1) / X::GROUPS;   // line blocks; a CTA takes blocks blockIdx.x, + gridDim.x, ... (persistent when the grid is smaller)
   cd* buf = smem + FftTw<FID>::COUNT + (size_t)grp * X::LB;
   cd* stages = smem + FftTw<FID>::COUNT + (size_t)X::GROUPS * X::LB;   // NST x [2][KX][LD]: U and V tiles, [kx][line]
   __shared__ unsigned s_tmem_base;
@@ -126,8 +129,6 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   const cd* tws = smem;
   // this warp's TMEM window: lane quarter warp%4, column slot warp/4
   const unsigned tm = __shfl_sync(0xffffffffu, s_tmem_base, 0) + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * X::TM_SLOT);
-  const bool active = line < nlines;
-  const size_t base = (size_t)(active ? line : 0) * d.Kxe;    // (z*ny + y)*Kxp  (output arrays E, kx fastest, padded rows)
   const int M = d.M;
   const double bsc = d.bscale;
   cd v[E];
@@ -136,14 +137,14 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   // Producer (lane 0 of warp 0): the tiles of arrays a, a+1 for the lines of this CTA.  D[a][line block][kx][LD] is laid
   // out so that a CTA's tile is ONE contiguous run (line slot XOR-swizzled with kx against bank conflicts): one bulk async copy (TMA engine) per array into
   // stage kn % NST; completion on s_full, reuse gated by s_empty.
-  auto produce = [&](int kn, int a) {
+  auto produce = [&](int kn, int a, int blk) {
     const int sn = kn % X::NST;
     if (kn >= X::NST) mbar_wait(&s_empty[sn], (unsigned)((kn / X::NST - 1) & 1));
     if ((threadIdx.x & 31) == 0) {
       constexpr unsigned TILE_BYTES = (unsigned)(KX * X::LD * sizeof(cd));
       mbar_arrive_expect_tx(&s_full[sn], 2u * TILE_BYTES);
       cd* st = stages + (size_t)sn * X::STAGE;
-      const cd* src = D + (size_t)a * d.PD + (size_t)blockIdx.x * (KX * X::LD);
+      const cd* src = D + (size_t)a * d.PD + (size_t)blk * (KX * X::LD);
       bulk_g2s(st, src, TILE_BYTES, &s_full[sn]);
       bulk_g2s(st + KX * X::LD, src + d.PD, TILE_BYTES, &s_full[sn]);
     }
@@ -154,13 +155,24 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   // run as conj(FFT(conj Z)) so that ONE forward-FFT code instance serves every job (instruction cache).
   auto src_array = [&](int kind) { return kind == 0 ? 0 : kind == 1 ? 2 : kind == 2 ? 6 : kind == 3 ? 4 : 8 + 2 * (kind - 4); };
   const int nkinds = 4 + M;
+  double gmax = 0.0;
+  cd twr[X::NTWR > 0 ? X::NTWR : 1];
+  if constexpr (X::NTWR > 0) fft_load_stage1_twiddles<FID, X::NTWR>(twr, t, tws);
+#if GD_X_STAGGER_NS > 0
+  if (warp >= X::WARPS / 2) __nanosleep(GD_X_STAGGER_NS);
+#endif
+  // Persistent form: the stage ring runs on across line blocks (global job index g0 + kind), so the first tiles of the next
+  // block travel during the last jobs of the current one -- with few fields per line (RMHD only: 4 inverse + 1 forward job)
+  // a CTA per block spends a third of its life on the start-up round trip (config 4b).
+  for (int blk = blockIdx.x, g0 = 0; blk < nblocks; blk += gridDim.x, g0 += nkinds) {
+  const int line = blk * X::GROUPS + grp;
+  const bool active = line < nlines;
+  const size_t base = (size_t)(active ? line : 0) * d.Kxe;    // (z*ny + y)*Kxp  (output arrays E, kx fastest, padded rows)
   int kind = 0;
   bool fwd = false;                // the job about to run is a forward transform of the pair held in v
   bool tail_done = (M == 0);
   int e0 = 0, e1 = 1;
-  double gmax = 0.0;
-  cd twr[X::NTWR > 0 ? X::NTWR : 1];
-  if constexpr (X::NTWR > 0) fft_load_stage1_twiddles<FID, X::NTWR>(twr, t, tws);
+  double gblk = 0.0;
   for (;;) {
     if (!fwd) {
       if (kind == nkinds) {
@@ -188,8 +200,9 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
       } else {
         // wait for the staged tiles and pack conj(Z), Z = Fx + i Fy.  P1 delivers U = kx f~ + (df/dy)~ and
         // V = (df/dy)~ - kx f~, so that Z(kx) = i U(kx) and Z(-kx) = i conj(V(kx)) (Hermitian completion) need no arithmetic
-        const int sc = kind % X::NST;
-        mbar_wait(&s_full[sc], (unsigned)((kind / X::NST) & 1));
+        const int g = g0 + kind;
+        const int sc = g % X::NST;
+        mbar_wait(&s_full[sc], (unsigned)((g / X::NST) & 1));
         const cd* pU = stages + (size_t)sc * X::STAGE;            // element n of this line: pU[n * LD + (grp ^ (n & (LD-1)))]
         const cd* pV = pU + (size_t)KX * X::LD;
 #pragma unroll
@@ -208,7 +221,11 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
         }
         __syncwarp();                   // every lane of the warp has consumed the stage
         if ((threadIdx.x & 31) == 0) mbar_arrive(&s_empty[sc]);
-        if (warp == 0 && kind + X::NST - 1 < nkinds) produce(kind + X::NST - 1, src_array(kind + X::NST - 1));
+        if (warp == 0) {
+          const int kn = kind + X::NST - 1;                     // job NST-1 ahead: of this block, or of the CTA's next one
+          if (kn < nkinds) produce(g0 + kn, src_array(kn), blk);
+          else if (blk + (int)gridDim.x < nblocks) produce(g0 + kn, src_array(kn - nkinds), blk + (int)gridDim.x);
+        }
       }
     }
 
@@ -281,7 +298,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
           const cd psi = cmake(0.5 * (xp.x - xm.x), 0.5 * (xp.y - xm.y));   // grad Psi
           tm_st4(tm + X::TM_PHI + 8 * q, phi.x, phi.y);
           tm_st4(tm + X::TM_PHI + 8 * q + 4, psi.x, psi.y);
-          gmax = fmax(gmax, phi.x * phi.x + phi.y * phi.y);
+          gblk = fmax(gblk, phi.x * phi.x + phi.y * phi.y);
           Qp[q] = 0.0; Ra[q] = 0.0;
         }
       }
@@ -321,8 +338,9 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
     }
     ++kind;
   }
+  if (active) gmax = fmax(gmax, gblk);
+  }
   if (maxbits != nullptr) {
-    if (!active) gmax = 0.0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) gmax = fmax(gmax, __shfl_xor_sync(0xffffffffu, gmax, o));
     if ((threadIdx.x & 31) == 0) atomicMax(maxbits, (unsigned long long)__double_as_longlong(gmax));
@@ -350,14 +368,20 @@ int xpass_lines_per_cta(int nx) {
   }
 }
 
+#ifndef GD_X_PERSIST_MAX_KINDS
+#define GD_X_PERSIST_MAX_KINDS 1000000   // persistent CTAs (one per SM) when a line has at most this many inverse jobs (4 + M).  Measured:
+                                         // 4b (5 jobs per line) 1.44 -> 1.20 ms; 4a (53 jobs) 1.397 -> 1.386 ms -- so always on
+#endif
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
-                         unsigned long long* maxbits, cudaStream_t st, bool prepare_only) {
+                         unsigned long long* maxbits, int num_sms, cudaStream_t st, bool prepare_only) {
   const int nlines = d.ny * d.nz;
+  const bool persist = 4 + d.M <= GD_X_PERSIST_MAX_KINDS;
 #define XCASE(NN)                                                                                             \
   {                                                                                                           \
     using X = XGeom<NN>;                                                                                      \
     if (prepare_only) return cudaFuncSetAttribute(k_xpass<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X::SMEM); \
-    k_xpass<NN><<<(nlines + X::GROUPS - 1) / X::GROUPS, X::THREADS, X::SMEM, st>>>(d, D, Eo, tw, cdn, cup, maxbits, nlines); \
+    const int nb = (nlines + X::GROUPS - 1) / X::GROUPS;                                                        \
+    k_xpass<NN><<<(persist && nb > num_sms) ? num_sms : nb, X::THREADS, X::SMEM, st>>>(d, D, Eo, tw, cdn, cup, maxbits, nlines); \
   }
   switch (d.nx) {
     case 8: XCASE(8) break; case 16: XCASE(16) break; case 32: XCASE(32) break; case 64: XCASE(64) break;

@@ -53,6 +53,9 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zfft(Dims d, const cd* __restr
 // Tables (k_tables, once per step): tabz[cz] = {cos th/2, sin th/2, cos th, sin th, fz, fzg}, th = kz vA dt;
 // tabp[col] = {fperp, fperp_g}: the separable factors of exp(-(eta P_perp + eta_z P_z) dt).
 // Work items are ordered with f fastest so that the CTAs that read g_{m-1}, g_m, g_{m+1} of the same columns run together.
+#ifndef GD_Z_PREFETCH
+#define GD_Z_PREFETCH 0     // 0: off; 1: own rows (Ws[f], Wn[f]); 2: also the neighbours' rows Ws[f-1], Ws[f+1]
+#endif
 template <int NZ> struct ZStepGeom {
   using G = FftGeom<NZ>;
   static constexpr int GROUPS = GD_Z_THREADS / G::T;         // columns per CTA
@@ -97,6 +100,28 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
   const int m = f - 2;
   const double dn = f >= 2 ? cdn[m] : 0.0, up = f >= 2 ? cup[m] : 0.0;
   const double cf = (mode == 2 && f >= 2) ? collfac[m] : 1.0;
+#if GD_Z_PREFETCH
+  // The operand rows of step 2 (Ws[f], its neighbours, Wn[f]: KZ rows of this CTA's columns) are asked into L2 now, so that
+  // the loads of step 2 -- which cannot issue before the forward transform is done -- find them there instead of paying a
+  // second DRAM round trip (P4 was bound by exposed load latency).
+  if (mode != 0 || f >= 2) {
+    const int ncolv = min(GROUPS, plane - col0);
+    const unsigned nb = (unsigned)(ncolv * sizeof(cd));
+    const bool lo = !EXACT && f > 2, hi = !EXACT && f + 1 < d.F, same = (EXACT || Ws == Wn || mode == 0);
+    const cd* own = (f < 2 ? Wn : Ws) + (size_t)f * d.PS + col0;
+    for (int r = threadIdx.x; r < KZ; r += GD_Z_THREADS) {
+      const size_t o = (size_t)r * plane;
+      bulk_prefetch_l2(own + o, nb);
+      if (f >= 2) {
+#if GD_Z_PREFETCH > 1
+        if (lo) bulk_prefetch_l2(own - d.PS + o, nb);
+        if (hi) bulk_prefetch_l2(own + d.PS + o, nb);
+#endif
+        if (!same) bulk_prefetch_l2(Wn + (size_t)f * d.PS + col0 + o, nb);
+      }
+    }
+  }
+#endif
   // 1. forward z transform of the bracket term, retained kz -> tile (scaled by 1/N)
   if (Gh != nullptr) {
     cd v[E];

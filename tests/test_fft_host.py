@@ -39,7 +39,7 @@ def test_scatter_is_bank_conflict_free(lib, n):
     assert lib.host_fft_scatter_conflicts(n) == 1
 
 
-@pytest.mark.parametrize("pid", [256, 256 + ALT])
+@pytest.mark.parametrize("pid", [256, 512, 256 + ALT])
 def test_split_exchange_is_bank_conflict_free_on_a_whole_warp(lib, pid):
     """8-byte exchange of the x-pass plans: 32 lanes x 8 B = 2 wavefronts at best."""
     assert lib.host_fft_split_conflicts(pid) == 2
