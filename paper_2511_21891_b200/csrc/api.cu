@@ -22,9 +22,9 @@ int xpass_lines_per_cta(int nx);
 int xpass_fft_plan_id(int nx);
 cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const double* cdn, const double* cup,
                          unsigned long long* maxbits, int num_sms, cudaStream_t st, bool prepare_only);
-cudaError_t launch_zstep(const Dims& d, int mode, bool exact, int if_variant, int g_sign, const cd* Gh, const cd* Wn, const cd* Ws, cd* Wout, cd* Hout,
-                         const double* scal, const double* cdn, const double* cup, const double* collfac, const double* tabz,
-                         const double* tabp, const cd* tw, cudaStream_t st);
+cudaError_t launch_zstep(const Dims& d, const TMaps& tm, int mode, bool exact, int if_variant, int g_sign, bool have_G, const cd* Wn, const cd* Ws,
+                         cd* Wout, bool want_H, const double* scal, const double* cdn, const double* cup, const double* collfac,
+                         const double* tabz, const double* tabp, const cd* tw, cudaStream_t st);
 void jacobi_eigh(int n, std::vector<double>& A, std::vector<double>& V, std::vector<double>& lam);
 cudaError_t launch_hermite_propagator(const Dims& d, int g_sign, double frac, const double* scal, const double* V, const double* lam,
                                       cd* P, cudaStream_t st);
@@ -54,6 +54,7 @@ struct gandalf_ctx {
   gandalf_params p;
   Dims d;
   PhysParams ph;
+  TMaps tm;
   cudaStream_t st;
   // device buffers
   cd *S0, *S1, *H, *Gh, *D, *E;
@@ -114,6 +115,47 @@ static cudaError_t upload_twiddles(cd** dst, int n, cudaStream_t st) {
   e = cudaMemcpyAsync(*dst, h.data(), h.size() * sizeof(cd), cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) return e;
   return cudaStreamSynchronize(st);
+}
+
+// ---- tensor maps (TMA descriptors) ---------------------------------------------------------------------------
+// cuTensorMapEncodeTiled is a driver entry point; it is fetched through the runtime so the library links against cudart only.
+#ifndef GD_TMA_L2PROMO
+#define GD_TMA_L2PROMO 3      // CU_TENSOR_MAP_L2_PROMOTION_*: 0 none, 1 64 B, 2 128 B, 3 256 B
+#endif
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess) return nullptr;
+  return (EncodeTiledFn)fn;
+}
+// fp64 view of a complex array: dims[0] counts doubles; strides in complex entries (dims 1..rank-1); boxes of 8 complex columns
+// (16 doubles = 128 B) x box_rows rows, 128-byte swizzle, out-of-range elements read as zeros / are not written.
+static bool make_map(EncodeTiledFn enc, CUtensorMap* m, cd* base, int rank, const unsigned long long* dims, const unsigned long long* strides_cd,
+                     int box_rows) {
+  cuuint64_t gd[5], gs[4];
+  cuuint32_t box[5], es[5];
+  for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; box[i] = 1; es[i] = 1; }
+  for (int i = 0; i + 1 < rank; ++i) gs[i] = strides_cd[i] * sizeof(cd);
+  box[0] = 16; box[1] = (cuuint32_t)box_rows;
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, base, gd, gs, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_128B, (CUtensorMapL2promotion)GD_TMA_L2PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+static bool build_tmaps(gandalf_ctx* c) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  const Dims& d = c->d;
+  const unsigned long long plane = (unsigned long long)d.Ky * d.Kx;
+  const int zrows = tma_rb(d.nz);
+  {   // P4: (ky,kx) plane flattened (hybrid rows are unpadded: Kxp == Kx)
+    const unsigned long long dims[3] = {2 * plane, (unsigned long long)d.nz, (unsigned long long)d.F};
+    const unsigned long long str[2] = {plane, d.PH};
+    if (!make_map(enc, &c->tm.g_flat, c->Gh, 3, dims, str, zrows)) return false;
+    if (!make_map(enc, &c->tm.h_flat, c->H, 3, dims, str, zrows)) return false;
+  }
+  return true;
 }
 
 static void free_all(gandalf_ctx* c) {
@@ -235,6 +277,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (e == cudaSuccess) e = upload_twiddles(&c->twz, d.nz, c->st);
   if (e == cudaSuccess) e = launch_xpass(d, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, c->st, true);
   if (e == cudaSuccess) e = prepare_passes_zy(d.ny, d.nz);
+  if (e == cudaSuccess && !build_tmaps(c)) e = cudaErrorUnknown;
   c->num_sms = 0;
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, p->device);
   if (c->num_sms <= 0) c->num_sms = 148;
@@ -353,8 +396,8 @@ static int rhs_pipeline(gandalf_ctx* c, bool want_cfl) {
 // P4: forward z transform of Gh + stage update (mode 0/1/2) + inverse z transform into the hybrid copy (if wanted)
 static int stage_update(gandalf_ctx* c, int mode, const cd* Wn, const cd* Ws, cd* Wout, bool want_hybrid, bool exact = false) {
   GD_CUDA(c, timed(c, KC_ZSTEP, 1, [&] {
-    return launch_zstep(c->d, mode, exact, c->p.if_variant, c->p.g_sign, c->p.nonlinear ? c->Gh : nullptr, Wn, Ws, Wout,
-                        want_hybrid ? c->H : nullptr, c->scal, c->cdn, c->cup, c->collfac, c->tabz, c->tabp, c->twz, c->st);
+    return launch_zstep(c->d, c->tm, mode, exact, c->p.if_variant, c->p.g_sign, c->p.nonlinear != 0, Wn, Ws, Wout,
+                        want_hybrid, c->scal, c->cdn, c->cup, c->collfac, c->tabz, c->tabp, c->twz, c->st);
   }));
   return GANDALF_OK;
 }

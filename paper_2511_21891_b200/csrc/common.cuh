@@ -10,6 +10,7 @@
 // cx = 0..Kx-1 is n_x = cx; cy = 0..Ky-1 is n_y = cy (cy <= hy3) or cy-Ky (negative modes);
 // cz likewise.  The zeroed third is never stored or transformed.
 #pragma once
+#include <cuda.h>            // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint, api.cu)
 #include <cuda_runtime.h>
 #include "fft.cuh"
 
@@ -26,6 +27,19 @@ struct Dims {
                           // floor is not set by A's magnitude before N+- = -1/2 A -+ 1/2 kperp^2 B amplifies it
   int xl, xlsh;           // lines per x-pass CTA (power of two) and its log2: block size of the D layout
   size_t PS, PH, PD, PE;  // per-field strides (complex elements): compact, hybrid, D (blocked, padded), E
+};
+
+// Row split of a tile of `rows` rows into boxes (a box has at most 256 rows; box starts stay multiples of 8 rows so that the
+// swizzle phase of a row is its index & 7 throughout the sub-tile).  Used by the kernels (compile time) and by api.cu (maps).
+constexpr int tma_nrb(int rows) { return (rows + 255) / 256; }
+constexpr int tma_rb(int rows) { return tma_nrb(rows) == 1 ? rows : (((rows + tma_nrb(rows) - 1) / tma_nrb(rows) + 7) / 8 * 8); }
+constexpr int tma_substr(int rows) {          // complex entries of one 8-column sub-tile, a multiple of 1024 bytes
+  return (tma_nrb(rows) * tma_rb(rows) * 8 + 63) / 64 * 64;
+}
+
+// Tensor maps of the context's arrays (built once in gandalf_create, api.cu; passed to the kernels as __grid_constant__ params).
+struct TMaps {
+  CUtensorMap g_flat, h_flat;   // Gh, H as {2*Ky*Kx, nz, F}: the [nz][8 columns] boxes of P4 (load / store)
 };
 
 __device__ __forceinline__ int c2n(int c, int h3, int K) { return c <= h3 ? c : c - K; }        // compact -> signed mode
@@ -86,6 +100,26 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, unsign
 // global -> L2 only (no shared-memory destination, no completion tracking): warms the lines a later load will ask for
 __device__ __forceinline__ void bulk_prefetch_l2(const void* src, unsigned bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+// ---- tiled bulk tensor copies (TMA, tensor-map form) for P4.  Its [nz][columns] tiles move with ONE instruction per 8-column
+// sub-tile issued by one thread: per-row 1-D bulk copies cost a warp-serialised issue loop (ELECT/R2UR per lane: 20 % of P4's warp
+// time in round 1).  The maps view the arrays as fp64 tensors (a complex entry = 2 elements); boxes are 8 complex columns wide
+// (128 B) and land in shared memory with the 128-byte swizzle: element (row r, column c < 8) of a sub-tile sits at
+// r*8 + (c ^ (r & 7)) (in complex entries; sub-tile base 1024-byte aligned), so the lanes of a transform, which read one column
+// over consecutive rows, hit eight different 16-byte bank groups.  Measured at 4a: P4 0.816 -> 0.780 ms.  The same scheme on the
+// y passes (P1, P3) was measured SLOWER than their per-row 1-D copies of 256 B (P1 0.869 -> 0.905 ms with two 8-column boxes,
+// 0.924 ms with one row-major {16, 2, rows} box; P3 0.528 -> 0.542 / 0.566 ms), so they keep the 1-D form.
+__device__ __forceinline__ int swz8(int r, int c) { return r * 8 + (c ^ (r & 7)); }
+__device__ __forceinline__ void tma_load_3d(void* dst_smem, const CUtensorMap* m, int c0, int c1, int c2, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+               ::"r"(smem_u32(dst_smem)), "l"(m), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, int c0, int c1, int c2, const void* src_smem) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3}], [%4];"
+               ::"l"(m), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(src_smem)) : "memory");
+}
+__device__ __forceinline__ cd* align1024(void* p) {           // dynamic shared memory is only 16-byte aligned by contract
+  return reinterpret_cast<cd*>((reinterpret_cast<unsigned long long>(p) + 1023ull) & ~1023ull);
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }

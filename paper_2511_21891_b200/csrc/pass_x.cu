@@ -24,6 +24,10 @@
 #ifndef GD_X_STAGGER_NS
 #define GD_X_STAGGER_NS 0
 #endif
+#ifndef GD_X_QRTM
+#define GD_X_QRTM 1       // 1: the Hermite sliding-window state (Q_{m-1}, the running R_m) lives in tensor memory next to the Phi/Psi lines
+                          // (one 16-word record per x-point) instead of 64 registers per lane: the transforms then run with ~190 registers
+#endif
 #ifndef GD_X_ALT
 #define GD_X_ALT 0        // 1: nx = 256 on one WARP per line (plan 8*8*4, 8 points per lane, 16 warps per SM).  Measured SLOWER (1.72 vs 1.40 ms at 4a:
                           // the second exchange costs more than the extra warps hide; bare transform 1.35 vs 2.53 G/s) -- kept as a tested option
@@ -52,7 +56,11 @@ struct XGeom {
   // Tensor memory as a thread-private scratchpad (tcgen05.ld/st, shape 32x32b: lane i of a warp owns TMEM lane
   // 32*(warp%4)+i).  Per thread: 8 words per x-point for (Phi_x,Phi_y,Psi_x,Psi_y) and 2 words per x-point for the
   // parked R_{m-2}.  Warps sharing a lane quarter take consecutive column slots.
-  static constexpr int TM_PHI = 0, TM_RD = 8 * E, TM_SLOT = 10 * E;
+  // QRTM layout: one 16-word record per x-point, [Phi_x Phi_y Psi_x Psi_y | Ra Rd Qp -] (Ra: the running R_m, Rd: the parked
+  // R_{m-2}, Qp: Q_{m-1}), so one x16 load brings everything a moment's products need and one x8 store puts the window back.
+  static constexpr bool QRTM = GD_X_QRTM && (16 * E * (THREADS / 128) <= 512);
+  static constexpr int TM_PSTR = QRTM ? 16 : 8;             // words per x-point record
+  static constexpr int TM_PHI = 0, TM_RD = 8 * E, TM_SLOT = QRTM ? 16 * E : 10 * E;
   static_assert(TM_SLOT * (THREADS / 128) <= 512, "TMEM columns");
   // columns to allocate: the next power of two >= what the CTA uses (>= 32), so that small-nx CTAs sharing an SM, or other
   // tensor-memory users on the device, are not locked out by a 512-column allocation
@@ -67,6 +75,16 @@ __device__ __forceinline__ void tm_st2(unsigned a, double x) {
 __device__ __forceinline__ void tm_st4(unsigned a, double x, double y) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(__double2loint(x)), "r"(__double2hiint(x)),
                "r"(__double2loint(y)), "r"(__double2hiint(y)) : "memory");
+}
+__device__ __forceinline__ void tm_st8(unsigned a, double x, double y, double z, double w) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(a), "r"(__double2loint(x)), "r"(__double2hiint(x)),
+               "r"(__double2loint(y)), "r"(__double2hiint(y)), "r"(__double2loint(z)), "r"(__double2hiint(z)), "r"(__double2loint(w)), "r"(__double2hiint(w)) : "memory");
+}
+struct TmRaw16 { unsigned w[16]; };
+__device__ __forceinline__ void tm_ld16(unsigned a, TmRaw16& r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+               : "=r"(r.w[0]), "=r"(r.w[1]), "=r"(r.w[2]), "=r"(r.w[3]), "=r"(r.w[4]), "=r"(r.w[5]), "=r"(r.w[6]), "=r"(r.w[7]),
+                 "=r"(r.w[8]), "=r"(r.w[9]), "=r"(r.w[10]), "=r"(r.w[11]), "=r"(r.w[12]), "=r"(r.w[13]), "=r"(r.w[14]), "=r"(r.w[15]) : "r"(a) : "memory");
 }
 struct TmRaw2 { unsigned w[2]; };
 struct TmRaw4 { unsigned w[4]; };
@@ -132,7 +150,9 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
   const int M = d.M;
   const double bsc = d.bscale;
   cd v[E];
-  double Qp[E], Ra[E];             // Hermite sliding window; Qp doubles as the {xi+,w-} accumulator of the Elsasser part
+  constexpr bool QRTM = X::QRTM;
+  constexpr int PSTR = X::TM_PSTR;
+  double Qp[QRTM ? 1 : E], Ra[QRTM ? 1 : E];   // Hermite sliding window (registers unless QRTM); Qp doubles as the {xi+,w-} accumulator of the Elsasser part
 
   // Producer (lane 0 of warp 0): the tiles of arrays a, a+1 for the lines of this CTA.  D[a][line block][kx][LD] is laid
   // out so that a CTA's tile is ONE contiguous run (line slot XOR-swizzled with kx against bank conflicts): one bulk async copy (TMA engine) per array into
@@ -180,7 +200,19 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
         // R_{M-1} is complete (up_{M-1} = 0 after the closure was folded into dn): flush the last pair / single
         tail_done = true;
         fwd = true;
-        if (((M - 1) & 1) == 1) {
+        const bool pair = (((M - 1) & 1) == 1);
+        if constexpr (QRTM) {
+          tm_wait_st();
+#pragma unroll
+          for (int q0 = 0; q0 < E; q0 += 4) {
+            TmRaw4 rr[4];
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) tm_ld4(tm + PSTR * (q0 + jj) + 8, rr[jj]);       // (Ra, Rd)
+            tm_wait_ld();
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) v[q0 + jj] = pair ? cmake(tm_d(rr[jj].w + 2), tm_d(rr[jj].w)) : cmake(tm_d(rr[jj].w), 0.0);
+          }
+        } else if (pair) {
           tm_wait_st();
 #pragma unroll
           for (int q0 = 0; q0 < E; q0 += 4) {
@@ -191,12 +223,12 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
 #pragma unroll
             for (int jj = 0; jj < 4; ++jj) v[q0 + jj] = cmake(tm_d(rd[jj].w), Ra[q0 + jj]);
           }
-          e0 = 2 + M - 2; e1 = 2 + M - 1;
         } else {
 #pragma unroll
           for (int q = 0; q < E; ++q) v[q] = cmake(Ra[q], 0.0);
-          e0 = 2 + M - 1; e1 = -1;
         }
+        if (pair) { e0 = 2 + M - 2; e1 = 2 + M - 1; }
+        else { e0 = 2 + M - 1; e1 = -1; }
       } else {
         // wait for the staged tiles and pack conj(Z), Z = Fx + i Fy.  P1 delivers U = kx f~ + (df/dy)~ and
         // V = (df/dy)~ - kx f~, so that Z(kx) = i U(kx) and Z(-kx) = i conj(V(kx)) (Hermitian completion) need no arithmetic
@@ -265,41 +297,56 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
     // inverse job done: v[q] = (df/dx, -df/dy) at x = t + T q   (conjugated output)
     if (kind == 0 || kind == 1) {          // xi+ / xi-: park the derivative lines in tensor memory
 #pragma unroll
-      for (int q = 0; q < E; ++q) tm_st4(tm + X::TM_PHI + 8 * q + 4 * kind, v[q].x, -v[q].y);
+      for (int q = 0; q < E; ++q) tm_st4(tm + X::TM_PHI + PSTR * q + 4 * kind, v[q].x, -v[q].y);
     } else if (kind == 2) {                // w-: {xi+, w-}
       tm_wait_st();
 #pragma unroll
       for (int q0 = 0; q0 < E; q0 += 4) {
         TmRaw4 r[4];
 #pragma unroll
-        for (int jj = 0; jj < 4; ++jj) tm_ld4(tm + X::TM_PHI + 8 * (q0 + jj), r[jj]);
+        for (int jj = 0; jj < 4; ++jj) tm_ld4(tm + X::TM_PHI + PSTR * (q0 + jj), r[jj]);
         tm_wait_ld();
 #pragma unroll
         for (int jj = 0; jj < 4; ++jj) {
           const double xpx = tm_d(r[jj].w), xpy = tm_d(r[jj].w + 2);
-          Qp[q0 + jj] = xpx * (-v[q0 + jj].y) - xpy * v[q0 + jj].x;
+          const double acc = xpx * (-v[q0 + jj].y) - xpy * v[q0 + jj].x;
+          if constexpr (QRTM) tm_st2(tm + PSTR * (q0 + jj) + 12, acc);
+          else Qp[q0 + jj] = acc;
         }
       }
     } else if (kind == 3) {                // w+: A = {xi+,w-} + {xi-,w+}, B = {xi+,xi-}; Phi/Psi lines; CFL max
+      if constexpr (QRTM) tm_wait_st();
 #pragma unroll
       for (int q0 = 0; q0 < E; q0 += 4) {
         TmRaw8 r[4];
+        TmRaw2 rq[4];
 #pragma unroll
-        for (int jj = 0; jj < 4; ++jj) tm_ld8(tm + X::TM_PHI + 8 * (q0 + jj), r[jj]);
+        for (int jj = 0; jj < 4; ++jj) tm_ld8(tm + X::TM_PHI + PSTR * (q0 + jj), r[jj]);
+        if constexpr (QRTM) {
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj) tm_ld2(tm + PSTR * (q0 + jj) + 12, rq[jj]);
+        }
         tm_wait_ld();
 #pragma unroll
         for (int jj = 0; jj < 4; ++jj) {
           const int q = q0 + jj;
           const cd xp = cmake(tm_d(r[jj].w), tm_d(r[jj].w + 2)), xm = cmake(tm_d(r[jj].w + 4), tm_d(r[jj].w + 6));
-          const double a = Qp[q] + (xm.x * (-v[q].y) - xm.y * v[q].x);
+          double acc;
+          if constexpr (QRTM) acc = tm_d(rq[jj].w); else acc = Qp[q];
+          const double a = acc + (xm.x * (-v[q].y) - xm.y * v[q].x);
           const double b = xp.x * xm.y - xp.y * xm.x;
           v[q] = cmake(a, bsc * b);                                          // (A, bscale*B): see Dims::bscale
           const cd phi = cmake(0.5 * (xp.x + xm.x), 0.5 * (xp.y + xm.y));   // grad Phi, Phi = (xi+ + xi-)/2
           const cd psi = cmake(0.5 * (xp.x - xm.x), 0.5 * (xp.y - xm.y));   // grad Psi
-          tm_st4(tm + X::TM_PHI + 8 * q, phi.x, phi.y);
-          tm_st4(tm + X::TM_PHI + 8 * q + 4, psi.x, psi.y);
+          if constexpr (QRTM) {
+            tm_st8(tm + PSTR * q, phi.x, phi.y, psi.x, psi.y);
+            tm_st8(tm + PSTR * q + 8, 0.0, 0.0, 0.0, 0.0);                   // Ra = Rd = Qp = 0
+          } else {
+            tm_st4(tm + X::TM_PHI + 8 * q, phi.x, phi.y);
+            tm_st4(tm + X::TM_PHI + 8 * q + 4, psi.x, psi.y);
+            Qp[q] = 0.0; Ra[q] = 0.0;
+          }
           gblk = fmax(gblk, phi.x * phi.x + phi.y * phi.y);
-          Qp[q] = 0.0; Ra[q] = 0.0;
         }
       }
       fwd = true; e0 = 0; e1 = 1;
@@ -309,6 +356,27 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const c
       const double upp = (m > 0) ? cup[m - 1] : 0.0;
       const bool emit = (m >= 1) && (((m - 1) & 1) == 1);     // R_{m-1} completes the pair (R_{m-2}, R_{m-1})
       tm_wait_st();
+      if constexpr (QRTM) {
+#pragma unroll
+        for (int q0 = 0; q0 < E; q0 += 4) {
+          TmRaw16 r[4];
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj) tm_ld16(tm + PSTR * (q0 + jj), r[jj]);
+          tm_wait_ld();
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj) {
+            const int q = q0 + jj;
+            const double phx = tm_d(r[jj].w), phy = tm_d(r[jj].w + 2), psx = tm_d(r[jj].w + 4), psy = tm_d(r[jj].w + 6);
+            const double ra = tm_d(r[jj].w + 8), rd = tm_d(r[jj].w + 10), qp = tm_d(r[jj].w + 12);
+            const double gx = v[q].x, gy = -v[q].y;
+            const double P = phx * gy - phy * gx;               // {Phi, g_m}
+            const double Q = psx * gy - psy * gx;               // {Psi, g_m}
+            const double rfin = ra + upp * Q;                   // R_{m-1} complete
+            if (emit) v[q] = cmake(rd, rfin);
+            tm_st8(tm + PSTR * q + 8, dn * qp - P, rfin, Q, 0.0);   // (Ra, Rd, Qp): the window moves on; Rd is dead after an emit
+          }
+        }
+      } else
 #pragma unroll
       for (int q0 = 0; q0 < E; q0 += 4) {
         TmRaw8 r[4];

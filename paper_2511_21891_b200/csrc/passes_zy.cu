@@ -53,26 +53,34 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zfft(Dims d, const cd* __restr
 // Tables (k_tables, once per step): tabz[cz] = {cos th/2, sin th/2, cos th, sin th, fz, fzg}, th = kz vA dt;
 // tabp[col] = {fperp, fperp_g}: the separable factors of exp(-(eta P_perp + eta_z P_z) dt).
 // Work items are ordered with f fastest so that the CTAs that read g_{m-1}, g_m, g_{m+1} of the same columns run together.
-#ifndef GD_Z_PREFETCH
-#define GD_Z_PREFETCH 0     // 0: off; 1: own rows (Ws[f], Wn[f]); 2: also the neighbours' rows Ws[f-1], Ws[f+1]
-#endif
 template <int NZ> struct ZStepGeom {
   using G = FftGeom<NZ>;
-  static constexpr int GROUPS = GD_Z_THREADS / G::T;         // columns per CTA
+  // 16 columns (256 B per z row) up to nz = 256; at nz = 512 (one warp per column) 8 columns
+#ifndef GD_ZS_THREADS
+#define GD_ZS_THREADS 128
+#endif
+  static constexpr int THREADS = (G::T >= 16) ? 256 : GD_ZS_THREADS;
+  static constexpr int GROUPS = THREADS / G::T;              // columns per CTA
+  static constexpr int NSUB = (GROUPS + 7) / 8;              // 8-column sub-tiles (one TMA box each)
+  static constexpr int SUBSTR = tma_substr(NZ);              // complex entries per sub-tile [NZ][8], a multiple of 1024 bytes
   static constexpr int KZ = 2 * (NZ / 3) + 1;                // retained kz (== Dims::Kz)
   static constexpr int LD = GROUPS + 1;                      // padded row of the [kz][column] tile
-  static constexpr int XCH = GROUPS * (G::BUF + 1);          // FFT exchange buffers (alias the tile)
-  static constexpr int REGION = XCH > KZ * LD ? XCH : KZ * LD;
-  static constexpr bool TMA_IN = (NZ * LD <= REGION);        // the staged [nz][GROUPS] tile of Gh fits in the region
-  static constexpr size_t SMEM = ((size_t)REGION + FftTw<NZ>::COUNT) * sizeof(cd);
+  static constexpr int XCH = GROUPS * (G::BUF + 1);          // FFT exchange buffers (alias the tiles)
+  static constexpr int cmax(int a, int b) { return a > b ? a : b; }
+  static constexpr int REGION = cmax(cmax(XCH, KZ * LD), NSUB * SUBSTR);
+  static constexpr size_t SMEM = ((size_t)REGION + FftTw<NZ>::COUNT) * sizeof(cd) + 1024;   // + alignment slack
 };
 // EXACT (hermite_exact = 1, hermite.cu; Q30): the streaming term of H_m is left to the exact propagator -- the moment
 // fields get only their bracket term (no neighbour reads), no dissipation here, and no hybrid copy (the propagated state's
 // copy is made afterwards); in mode 2 they are updated in place on Ws (= P(dt/2) g_n), w+- as usual on Wn -> Wout.
+// mapG / mapH: Gh and H viewed as fp64 tensors {2*Ky*Kx, nz, F} (the (ky,kx) plane flattened: hybrid rows are unpadded, so a
+// block of columns is contiguous even across a ky row end), boxes {16 doubles, NZ, 1}, 128-byte swizzle (common.cuh).
 template <int NZ, int MODE, bool EXACT>   // MODE 0 / 1 / 2 = RHS only / predictor / corrector + dissipation (compile time: fewer registers)
-__global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, double skz_sign, const cd* __restrict__ Gh,
+__global__ void __launch_bounds__(ZStepGeom<NZ>::THREADS, ZStepGeom<NZ>::THREADS > 128 ? 2 : 4) k_zstep(Dims d, int if_variant, double skz_sign,
+                                                      const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapH,
+                                                      bool have_G, bool want_H,
                                                       const cd* __restrict__ Wn, const cd* __restrict__ Ws, cd* __restrict__ Wout,
-                                                      cd* __restrict__ Hout, const double* __restrict__ scal,
+                                                      const double* __restrict__ scal,
                                                       const double* __restrict__ cdn, const double* __restrict__ cup,
                                                       const double* __restrict__ collfac, const double* __restrict__ tabz,
                                                       const double* __restrict__ tabp, const cd* __restrict__ tw) {
@@ -80,70 +88,51 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
   using Z = ZStepGeom<NZ>;
   constexpr int mode = MODE;
   constexpr int T = G::T, E = G::E;
-  constexpr int GROUPS = Z::GROUPS, KZ = Z::KZ, LD = Z::LD;
-  extern __shared__ cd smem[];
+  constexpr int GROUPS = Z::GROUPS, KZ = Z::KZ, LD = Z::LD, THREADS = Z::THREADS;
+  constexpr int RB = tma_rb(NZ), NRB = tma_nrb(NZ);            // a box has at most 256 rows
+  extern __shared__ cd smem_raw[];
   __shared__ unsigned long long bar;
   const int grp = threadIdx.x / T, t = threadIdx.x % T;
-  cd* tile = smem + FftTw<NZ>::COUNT;                          // [KZ][LD], aliases the exchange buffers
+  cd* tile = align1024(smem_raw);                              // region: TMA sub-tiles / [KZ][LD] tile / exchange buffers
+  cd* tws_s = tile + Z::REGION;                                // stage twiddle table
   cd* buf = tile + (size_t)grp * (G::BUF + 1);
-  const cd* tws = smem;
+  cd* sub = tile + (size_t)(grp >> 3) * Z::SUBSTR;             // this group's 8-column sub-tile, column grp & 7
+  const int subc = grp & 7;
+  const cd* tws = tws_s;
   const int plane = d.Ky * d.Kx;
   const int f = blockIdx.x % d.F, cb = blockIdx.x / d.F;
   const int col0 = cb * GROUPS;
   const int col = col0 + grp;
   const bool active = col < plane;
-  const int colc = active ? col : 0;
-  const int planeH = d.Ky * d.Kxp, colH = (colc / d.Kx) * d.Kxp + colc % d.Kx;   // hybrid rows are padded to Kxp
-  // per-item scalars and the column of Gh are requested BEFORE the twiddle table is staged, so that all three
-  // round trips overlap
+  const int ncolv = min(GROUPS, plane - col0);
+  const int nsubv = (ncolv + 7) >> 3;                          // sub-tiles with at least one valid column
+  // the bracket tile and the twiddle table are requested first (one thread, three instructions), then the per-item scalars
+  if (threadIdx.x == 0) {
+    mbar_init(&bar, 1);
+    unsigned bytes = (unsigned)(FftTw<NZ>::COUNT * sizeof(cd));
+    if (have_G) bytes += (unsigned)(nsubv * NZ * 8 * sizeof(cd));   // a box always delivers its full size (out-of-range columns as zeros)
+    if (bytes > 0) {
+      mbar_arrive_expect_tx(&bar, bytes);
+      if (have_G)
+        for (int sidx = 0; sidx < nsubv; ++sidx)
+          for (int rb = 0; rb < NRB; ++rb) tma_load_3d(tile + (size_t)sidx * Z::SUBSTR + rb * RB * 8, &mapG, 2 * (col0 + 8 * sidx), rb * RB, f, &bar);
+      if (FftTw<NZ>::COUNT > 0) bulk_g2s(tws_s, tw, (unsigned)(FftTw<NZ>::COUNT * sizeof(cd)), &bar);
+    } else {
+      mbar_arrive(&bar);
+    }
+  }
   const double dt = scal[SC_DT];
   const int m = f - 2;
   const double dn = f >= 2 ? cdn[m] : 0.0, up = f >= 2 ? cup[m] : 0.0;
   const double cf = (mode == 2 && f >= 2) ? collfac[m] : 1.0;
-#if GD_Z_PREFETCH
-  // The operand rows of step 2 (Ws[f], its neighbours, Wn[f]: KZ rows of this CTA's columns) are asked into L2 now, so that
-  // the loads of step 2 -- which cannot issue before the forward transform is done -- find them there instead of paying a
-  // second DRAM round trip (P4 was bound by exposed load latency).
-  if (mode != 0 || f >= 2) {
-    const int ncolv = min(GROUPS, plane - col0);
-    const unsigned nb = (unsigned)(ncolv * sizeof(cd));
-    const bool lo = !EXACT && f > 2, hi = !EXACT && f + 1 < d.F, same = (EXACT || Ws == Wn || mode == 0);
-    const cd* own = (f < 2 ? Wn : Ws) + (size_t)f * d.PS + col0;
-    for (int r = threadIdx.x; r < KZ; r += GD_Z_THREADS) {
-      const size_t o = (size_t)r * plane;
-      bulk_prefetch_l2(own + o, nb);
-      if (f >= 2) {
-#if GD_Z_PREFETCH > 1
-        if (lo) bulk_prefetch_l2(own - d.PS + o, nb);
-        if (hi) bulk_prefetch_l2(own + d.PS + o, nb);
-#endif
-        if (!same) bulk_prefetch_l2(Wn + (size_t)f * d.PS + col0 + o, nb);
-      }
-    }
-  }
-#endif
+  __syncthreads();                                             // barrier initialised before anybody waits on it
+  mbar_wait(&bar, 0);
   // 1. forward z transform of the bracket term, retained kz -> tile (scaled by 1/N)
-  if (Gh != nullptr) {
+  if (have_G) {
     cd v[E];
-    if (Z::TMA_IN && d.Kxp == d.Kx) {
-      // (unpadded hybrid rows: the block's columns are contiguous in memory even across a ky row end)  The [nz][GROUPS]
-      // tile comes by one bulk async copy per z row (TMA engine) into the region the exchange buffers will reuse.
-      const int ncolv = min(GROUPS, plane - col0);
-      if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_arrive_expect_tx(&bar, (unsigned)(NZ * ncolv * sizeof(cd))); }
-      __syncthreads();
-      const cd* src0 = Gh + (size_t)f * d.PH + col0;
-      for (int r = threadIdx.x; r < NZ; r += GD_Z_THREADS) bulk_g2s(tile + (size_t)r * LD, src0 + (size_t)r * planeH, (unsigned)(ncolv * sizeof(cd)), &bar);
-      fft_load_table<NZ>(smem, tw);                            // ends with __syncthreads()
-      mbar_wait(&bar, 0);
 #pragma unroll
-      for (int q = 0; q < E; ++q) v[q] = active ? tile[(t + T * q) * LD + grp] : cmake(0.0, 0.0);
-      __syncthreads();                                         // tile consumed: the exchange buffers may overwrite it
-    } else {
-      const cd* src = Gh + (size_t)f * d.PH + colH;
-#pragma unroll
-      for (int q = 0; q < E; ++q) v[q] = active ? ldg_cd(src + (size_t)(t + T * q) * planeH) : cmake(0.0, 0.0);
-      fft_load_table<NZ>(smem, tw);                            // ends with __syncthreads()
-    }
+    for (int q = 0; q < E; ++q) v[q] = active ? sub[swz8(t + T * q, subc)] : cmake(0.0, 0.0);
+    __syncthreads();                                           // tile consumed: the exchange buffers may overwrite it
     fft_lanes<NZ, -1>(v, t, buf, tws);
     __syncthreads();                                           // every group is done with its exchange buffer
 #pragma unroll
@@ -152,8 +141,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
       if (cz >= 0) tile[cz * LD + grp] = cscale(v[q], d.inv_n);
     }
   } else {
-    fft_load_table<NZ>(smem, tw);                              // ends with __syncthreads()
-    for (int e = threadIdx.x; e < KZ * LD; e += GD_Z_THREADS) tile[e] = cmake(0.0, 0.0);
+    for (int e = threadIdx.x; e < KZ * LD; e += THREADS) tile[e] = cmake(0.0, 0.0);
   }
   __syncthreads();
   // 2. pointwise stage update on the tile: thread <-> (kz, column), columns fastest (row-contiguous global accesses);
@@ -162,14 +150,13 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
     const double c = (mode == 1) ? 0.5 * dt : dt;
     const bool lo = !EXACT && f > 2, hi = !EXACT && f + 1 < d.F, same = (EXACT || Ws == Wn || mode == 0);
     cd* const wout = (EXACT && mode == 2 && f >= 2) ? const_cast<cd*>(Ws) : Wout;
-    const int ncolv = min(GROUPS, plane - col0);
     constexpr int NEL = KZ * GROUPS, UB = 6;
-    for (int e0 = threadIdx.x; e0 < NEL; e0 += UB * GD_Z_THREADS) {
+    for (int e0 = threadIdx.x; e0 < NEL; e0 += UB * THREADS) {
       cd a0[UB], a1[UB], a2[UB], a3[UB];
       bool ok[UB];
 #pragma unroll
       for (int u = 0; u < UB; ++u) {
-        const int e = e0 + u * GD_Z_THREADS;
+        const int e = e0 + u * THREADS;
         const int cz = e / GROUPS, cl = e % GROUPS;
         ok[u] = e < NEL && cl < ncolv;
         const size_t idx = ok[u] ? (size_t)cz * plane + col0 + cl : 0;
@@ -187,7 +174,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
 #pragma unroll
       for (int u = 0; u < UB; ++u) {
         if (!ok[u]) continue;
-        const int e = e0 + u * GD_Z_THREADS;
+        const int e = e0 + u * THREADS;
         const int cz = e / GROUPS, cl = e % GROUPS;
         const size_t idx = (size_t)cz * plane + col0 + cl;
         const cd Gv = tile[cz * LD + cl];
@@ -225,7 +212,7 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
       }
     }
   }
-  if (Hout == nullptr || (EXACT && f >= 2)) return;
+  if (!want_H || (EXACT && f >= 2)) return;
   __syncthreads();
   // 3. inverse z transform of the new stage state (zero-padded) -> hybrid copy
   cd v[E];
@@ -236,22 +223,18 @@ __global__ void __launch_bounds__(GD_Z_THREADS) k_zstep(Dims d, int if_variant, 
   }
   __syncthreads();                                             // tile read by every group: the exchange may overwrite it
   fft_lanes<NZ, +1>(v, t, buf, tws);
-  if (Z::TMA_IN && d.Kxp == d.Kx) {
-    // the [nz][GROUPS] result tile goes through the (now free) exchange region and leaves by one bulk async store per z row
-    const int ncolv = min(GROUPS, plane - col0);
-    __syncthreads();                                           // every group is done with its exchange buffer
+  // the [nz][GROUPS] result goes through the (now free) region in the swizzled sub-tile layout and leaves by one tensor store
+  // per sub-tile (columns beyond the plane are clipped by the map)
+  __syncthreads();                                             // every group is done with its exchange buffer
 #pragma unroll
-    for (int q = 0; q < E; ++q) tile[(t + T * q) * LD + grp] = v[q];
-    fence_proxy_async();                                       // generic-proxy writes -> visible to the async proxy
-    __syncthreads();
-    cd* dst0 = Hout + (size_t)f * d.PH + col0;
-    for (int r = threadIdx.x; r < NZ; r += GD_Z_THREADS) bulk_s2g(dst0 + (size_t)r * planeH, tile + (size_t)r * LD, (unsigned)(ncolv * sizeof(cd)));
+  for (int q = 0; q < E; ++q) sub[swz8(t + T * q, subc)] = v[q];
+  fence_proxy_async();                                         // generic-proxy writes -> visible to the async proxy
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int sidx = 0; sidx < nsubv; ++sidx)
+      for (int rb = 0; rb < NRB; ++rb) tma_store_3d(&mapH, 2 * (col0 + 8 * sidx), rb * RB, f, tile + (size_t)sidx * Z::SUBSTR + rb * RB * 8);
     bulk_commit();
     bulk_wait_read0();                                         // shared memory must stay valid until the engine has read it
-  } else if (active) {
-    cd* dst = Hout + (size_t)f * d.PH + colH;
-#pragma unroll
-    for (int q = 0; q < E; ++q) st_cd(dst + (size_t)(t + T * q) * planeH, v[q]);
   }
 }
 
@@ -532,18 +515,20 @@ cudaError_t launch_zfft(const Dims& d, const cd* in, cd* out, const cd* tw, int 
   GD_DISPATCH(d.nz, ZCASE)
   return cudaGetLastError();
 }
-cudaError_t launch_zstep(const Dims& d, int mode, bool exact, int if_variant, int g_sign, const cd* Gh, const cd* Wn, const cd* Ws, cd* Wout, cd* Hout,
-                         const double* scal, const double* cdn, const double* cup, const double* collfac, const double* tabz,
-                         const double* tabp, const cd* tw, cudaStream_t st) {
+cudaError_t launch_zstep(const Dims& d, const TMaps& tm, int mode, bool exact, int if_variant, int g_sign, bool have_G, const cd* Wn, const cd* Ws,
+                         cd* Wout, bool want_H, const double* scal, const double* cdn, const double* cup, const double* collfac,
+                         const double* tabz, const double* tabp, const cd* tw, cudaStream_t st) {
   const long long ncols = (long long)d.Ky * d.Kx;
+#define ZSARGS d, if_variant, (double)g_sign, tm.g_flat, tm.h_flat, have_G, want_H, Wn, Ws, Wout, scal, cdn, cup, collfac, tabz, tabp, tw
 #define ZSCASE(NN)                                                                                               \
   {                                                                                                              \
-    const int nb = fft_blocks<NN>(ncols) * d.F;                                                                  \
-    if (mode == 0) k_zstep<NN, 0, false><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
-    else if (mode == 1 && !exact) k_zstep<NN, 1, false><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
-    else if (mode == 1) k_zstep<NN, 1, true><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
-    else if (!exact) k_zstep<NN, 2, false><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
-    else k_zstep<NN, 2, true><<<nb, GD_Z_THREADS, ZStepGeom<NN>::SMEM, st>>>(d, if_variant, (double)g_sign, Gh, Wn, Ws, Wout, Hout, scal, cdn, cup, collfac, tabz, tabp, tw); \
+    using Z = ZStepGeom<NN>;                                                                                     \
+    const int nb = (int)((ncols + Z::GROUPS - 1) / Z::GROUPS) * d.F;                                             \
+    if (mode == 0) k_zstep<NN, 0, false><<<nb, Z::THREADS, Z::SMEM, st>>>(ZSARGS);                               \
+    else if (mode == 1 && !exact) k_zstep<NN, 1, false><<<nb, Z::THREADS, Z::SMEM, st>>>(ZSARGS);                \
+    else if (mode == 1) k_zstep<NN, 1, true><<<nb, Z::THREADS, Z::SMEM, st>>>(ZSARGS);                           \
+    else if (!exact) k_zstep<NN, 2, false><<<nb, Z::THREADS, Z::SMEM, st>>>(ZSARGS);                             \
+    else k_zstep<NN, 2, true><<<nb, Z::THREADS, Z::SMEM, st>>>(ZSARGS);                                          \
   }
   GD_DISPATCH(d.nz, ZSCASE)
   return cudaGetLastError();
