@@ -331,6 +331,81 @@ def run_microbench(device=0, which=(0, 1, 2, 3)):
     return out
 
 
+def run_mshard(args, rank, world, local):
+    """ONE run of the workload sharded by Hermite moment over the ranks (strong scaling): xi+- replicated, one halo moment per
+    neighbour exchanged twice per step with NCCL point-to-point copies in place on the library's buffers (sharded.py)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2511_21891_b200 import sharded
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    prm, z, g, run = make_workload(args.workload)
+    shape, dt, M = run["shape"], run["dt"], prm.get("M", 0)
+    emu = args.emulate_ranks if world == 1 else 0
+    nranks = emu if emu else world
+    if M < nranks or prm.get("nspecies", 1) != 1:
+        raise SystemExit("mshard needs one species and at least one moment per rank")
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    stream = torch.cuda.current_stream()        # NCCL orders its copies against torch's current stream: the contexts run on it
+    lays = [sharded.ShardLayout.make(M, nranks, r) for r in range(nranks)]
+    mine = lays if emu else [lays[rank]]
+    shards = [sharded.GandalfShard(*shape, lay, device=local, stream=stream.cuda_stream, **prm) for lay in mine]
+    for sh in shards:
+        sh.set_state(z, g)
+    if emu or world == 1:
+        def advance(n):
+            sharded.step_all(shards, mine, dt, n)
+    else:
+        stepper = sharded.ShardedStepper(shards[0], mine[0], sharded.DistExchange())
+        advance = lambda n: stepper.step(dt, n)                   # noqa: E731
+    advance(args.warmup)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    n0 = sum(sh.g.launch_count() for sh in shards)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    advance(args.steps)
+    e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ms = max_over_ranks(e0.elapsed_time(e1), world)
+    clocks = sampler.stop()
+    launches = sum(sh.g.launch_count() for sh in shards) - n0
+    en = np.array([sh.energy() for sh in shards])
+    wg = float(en[:, 5].sum())
+    if world > 1:
+        t = torch.tensor([wg], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t)
+        wg = float(t.item())
+    if rank == 0:
+        steps_per_s = args.steps / (ms * 1e-3)                     # ONE run: the ranks share the work (strong scaling)
+        halo_bytes = 16 * (shape[0] // 3 + 1) * (2 * (shape[1] // 3) + 1) * (2 * (shape[2] // 3) + 1)
+        print(json.dumps({
+            "metric": "RHS evals/s", "value": 2 * steps_per_s, "unit": "RHS evals/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE config {args.workload}", "grid": list(shape), "M": M,
+                       "parallelism": f"m-shard, {nranks} ranks" + (" EMULATED in one process on one GPU (path check, not a scaling number)" if emu else ""),
+                       "moments_per_rank": [lay.hi - lay.lo for lay in lays], "halo_fields_per_rank": [lay.halo_lo + lay.halo_hi for lay in lays],
+                       "halo_bytes_per_neighbour_per_exchange": halo_bytes, "exchanges_per_step": 2},
+            "steps_per_s": steps_per_s, "grid_point_moments_per_s": shape[0] * shape[1] * shape[2] * (2 + M) * steps_per_s,
+            "gpu_launches": int(launches), "clocks": clocks,
+            "final_energy": {"E_A": float(en[0, 0]), "W_g": wg},
+        }), flush=True)
+    for sh in shards:
+        sh.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -343,6 +418,10 @@ def main():
     ap.add_argument("--no-cufft-compare", action="store_true")
     ap.add_argument("--oracle-full-rhs", action="store_true", help="also time one oracle RHS evaluation at the FULL grid (slow, ~20 GB host memory at 4a)")
     ap.add_argument("--microbench", action="store_true", help="print the measured unit ceilings (gandalf_microbench) and exit")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "mshard"],
+                    help="N > 1: independent replicas (default; north_star keeps the product on one GPU) or ONE run sharded by Hermite "
+                         "moment with halo exchange over NCCL (paper_2511_21891_b200/sharded.py, DESIGN.md Q31)")
+    ap.add_argument("--emulate-ranks", type=int, default=0, help="mshard on ONE GPU: emulate this many ranks in one process (checks the path; not a scaling number)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -356,6 +435,9 @@ def main():
         return
     if args.warmup < 3:
         args.warmup = 3
+    if args.parallelism == "mshard":
+        run_mshard(args, rank, world, local)
+        return
 
     import torch
     import torch.distributed as dist

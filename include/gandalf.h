@@ -74,6 +74,14 @@ typedef struct gandalf_params {
                              operator s i kz (I - T) of Eq. 6 is integrated exactly (matrix exponential in m per kz,
                              integrating-factor midpoint for the brackets) [future work of PAPER.md:657, 829; lifts the
                              dt < dz/v_th constraint of PAPER.md:214; Q30] */
+  int    m_offset;        /* Moment shard [SURVEY.md 8(e)(i); PAPER.md:832, 975 list multi-device runs as future work; Q31]: */
+  int    M_global;        /* this context holds the moments m_offset .. m_offset+M-1 of a hierarchy of M_global moments (0 = not
+                             sharded).  If m_offset > 0 its FIRST moment field is a halo copy of the lower neighbour's last owned
+                             moment, if m_offset+M < M_global its LAST one a halo copy of the upper neighbour's first: halos are
+                             inputs the caller refreshes after every stage (gandalf_step_stage, gandalf_field_ptr,
+                             gandalf_halo_refresh); they are left out of W_g.  Coefficients sqrt(m/2), sqrt((m+1)/2), the
+                             closure and (m/M)^(2p) use the global m and M_global; xi+- are replicated.  nspecies = 1,
+                             hermite_exact = 0 only.                                                   */
   int    device;          /* CUDA device ordinal                                                  */
   void*  stream;          /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
 } gandalf_params;
@@ -133,6 +141,20 @@ int gandalf_rhs(gandalf_ctx* ctx, double* dw_hat, double* dg_hat, int on_device)
  * asynchronous on the ctx's stream; errors detected on the device (non-finite energy) are
  * reported by gandalf_energy_history / gandalf_energy / gandalf_get_time, which synchronise. */
 int gandalf_step(gandalf_ctx* ctx, double dt, int nsteps);
+
+/* Moment-sharded stepping (Q31).  gandalf_step(dt, 1) == gandalf_step_stage(dt, 0) followed by
+ * gandalf_step_stage(dt, 1): stage 0 is the RHS at t_n, the dt of this step and the half-step predictor (Alg. 1 l.2-4), stage 1
+ * the midpoint RHS, corrector, dissipation, forcing and the energy record (Alg. 1 l.6-9, Alg. 2 l.12-14).  Between the stages
+ * (and after stage 1) a sharded run overwrites its halo moments with the neighbours' values:
+ *   gandalf_field_ptr(ctx, state, field, &p, &n)  device address and length (complex entries) of one field of the raw retained-
+ *       mode array (layout of gandalf_get_state_raw); state 0 = the state at t_n / t_{n+1}, 1 = the half-step (stage) state;
+ *       field 0, 1 = w+-, 2+j = local moment j.  The caller copies / sends / receives in place (stream-ordered on ctx's stream
+ *       or after synchronising it); the pointers stay valid for the life of the context.
+ *   gandalf_halo_refresh(ctx, state)  re-derives what the library keeps besides the raw array for the halo fields (their
+ *       z-real hybrid copy, the input of the next RHS evaluation) from the given state.  Call it after the halos were written. */
+int gandalf_step_stage(gandalf_ctx* ctx, double dt, int stage);
+int gandalf_field_ptr(gandalf_ctx* ctx, int state, int field, void** device_ptr, long long* ncomplex);
+int gandalf_halo_refresh(gandalf_ctx* ctx, int state);
 
 /* Energies of the current state (host output, synchronises):
  * out = { E_A, E_plus, E_minus, E_kin, E_mag, W_g } with E_+- = 1/4 sum_k kperp^2 |xi+-|^2,

@@ -45,13 +45,15 @@ class OracleParams(C.Structure):
         ("nspecies", C.c_int),
         ("dt_max", C.c_double),
         ("hermite_exact", C.c_int),
+        ("m_offset", C.c_int), ("M_global", C.c_int),
     ]
 
 
 _DEFAULTS = dict(M=0, Lx=2 * np.pi, Ly=2 * np.pi, Lz=2 * np.pi, vA=1.0, eta=0.0, r=1, eta_normalized=0,
                  eta_z=0.0, r_z=1, eta_g=0.0, nu_coll=0.0, p=1.0, closure=0, if_variant=0, g_sign=1,
                  nonlinear=1, hermite_coeff=0, force_eps=0.0, force_nperp_min=1, force_nperp_max=2,
-                 force_nz_max=1, seed=0, cfl=0.3, force_g_amp=0.0, force_g_nz=1, nspecies=1, dt_max=0.0, hermite_exact=0)
+                 force_nz_max=1, seed=0, cfl=0.3, force_g_amp=0.0, force_g_nz=1, nspecies=1, dt_max=0.0, hermite_exact=0,
+                 m_offset=0, M_global=0)
 
 _lib = None
 
@@ -83,6 +85,9 @@ def _load():
         lib.oracle_bracket_full.argtypes = [C.c_void_p, P, P, P, P]
         lib.oracle_get_full.argtypes = [C.c_void_p, C.c_int, P]
         lib.oracle_set_full.argtypes = [C.c_void_p, C.c_int, P]
+        lib.oracle_step_stage.argtypes = [C.c_void_p, C.c_double, C.c_int]
+        lib.oracle_get_stage_full.argtypes = [C.c_void_p, C.c_int, P]
+        lib.oracle_set_stage_full.argtypes = [C.c_void_p, C.c_int, P]
         lib.oracle_num_threads.restype = C.c_int
         lib.oracle_set_num_threads.argtypes = [C.c_int]
         lib.oracle_set_num_threads.restype = None
@@ -234,6 +239,21 @@ class Oracle:
         self._check(self._lib.oracle_bracket_full(self._h, _dp(f.view(np.float64)), _dp(g.view(np.float64)),
                                                   _dp(out.view(np.float64)), C.byref(mi)), "bracket")
         return out, mi.value
+
+    def step_stage(self, dt, stage):
+        """One stage of a step (0: RHS + predictor, 1: midpoint RHS + corrector + ...); a moment-sharded run refreshes its
+        halo moments in between (Q31)."""
+        self._check(self._lib.oracle_step_stage(self._h, float(dt), int(stage)), "step_stage")
+
+    def get_stage_full(self, field):
+        out = np.empty((self.nz, self.ny, self.nx), dtype=np.complex128)
+        self._check(self._lib.oracle_get_stage_full(self._h, field, _dp(out.view(np.float64))), "get_stage_full")
+        return out
+
+    def set_stage_full(self, field, a):
+        a = np.ascontiguousarray(a, dtype=np.complex128)
+        assert a.shape == (self.nz, self.ny, self.nx)
+        self._check(self._lib.oracle_set_stage_full(self._h, field, _dp(a.view(np.float64))), "set_stage_full")
 
     def get_full(self, field):
         out = np.empty((self.nz, self.ny, self.nx), dtype=np.complex128)

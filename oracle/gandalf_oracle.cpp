@@ -72,6 +72,11 @@ struct oracle_params {
   int nspecies;       // 1: g (sign g_sign);  2: g^+ (g_sign) then g^- (-g_sign), M moments each (Q27)
   double dt_max;      // > 0: upper bound of the CFL step of Eq. 16 (and the step taken when the flow vanishes); 0 = none (Q29)
   int hermite_exact;  // 1: exact propagator exp(s i kz (I - T) dt) for the streaming / phase-mixing terms of Eq. 6 (Q30)
+  // Moment shard (Q31): this instance holds the moments m_offset .. m_offset+M-1 of a hierarchy of
+  // M_global moments (0 = not sharded, M_global = M).  If m_offset > 0 its first field is a HALO copy of the neighbour's g_{m_offset}
+  // and if m_offset+M < M_global its last field is one: halos are inputs (set by the caller after every stage), their own update
+  // is meaningless, and they are left out of W_g.  The arithmetic of an owned moment is that of the unsharded run, operation by operation.
+  int m_offset, M_global;
 };
 
 }  // extern "C"
@@ -135,6 +140,11 @@ struct oracle_ctx {
   std::vector<cplx> w[2];                   // w^+ , w^-  
   std::vector<std::vector<cplx>> g;         // g_0 .. g_{M-1}
   std::vector<double> coef_dn, coef_up;     // Eq. 6 coupling coefficients to g_{m-1}, g_{m+1}
+  std::vector<cplx> hw[2];                  // half-step (stage) state of Alg. 1 l.3-4 between the two stages of a step
+  std::vector<std::vector<cplx>> hg;
+  double dt_cur;                            // the step's dt (fixed, or Eq. 16), set by the first stage
+  int moff, Mg;                             // shard: global index of local moment 0, global moment count (Q31)
+  int own_lo, own_hi;                       // owned local moments [own_lo, own_hi): the rest are halos
   double t; long long step; double last_dt;
   std::vector<double> hist;                 // 7 doubles per record: t, E_A, E+, E-, E_kin, E_mag, W_g
   std::string err;
@@ -265,7 +275,7 @@ static int neighbour_index(const oracle_ctx* c, int sp, int m) {   // field inde
   const int M = c->Msp;
   if (m < 0) return -1;
   if (m < M) return sp * M + m;
-  if (m == M && c->p.closure == 1 && M >= 2) return sp * M + M - 2;
+  if (m == M && c->moff + M == c->Mg && c->p.closure == 1 && M >= 2) return sp * M + M - 2;   // the closure sits at the GLOBAL end (Q31)
   return -1;
 }
 
@@ -327,13 +337,14 @@ static void rhs_eval(const oracle_ctx* c, const State& s, State& out, double* ma
           bracket_from_grads(c, gPhi, gg[fi], br);                    // {Phi, g_m}
           for (size_t i = 0; i < c->N; ++i) out.g[fi][i] -= br[i];
           int lo = neighbour_index(c, sp, m - 1), hi = neighbour_index(c, sp, m + 1);
-          if (lo >= 0 && c->coef_dn[m] != 0.0) {
+          const int gm = c->moff + m;                                 // global moment index (= m unless sharded, Q31)
+          if (lo >= 0 && c->coef_dn[gm] != 0.0) {
             bracket_from_grads(c, gPsi, gg[lo], br);                  // {Psi, g_{m-1}}
-            for (size_t i = 0; i < c->N; ++i) out.g[fi][i] += c->coef_dn[m] * br[i];
+            for (size_t i = 0; i < c->N; ++i) out.g[fi][i] += c->coef_dn[gm] * br[i];
           }
           if (hi >= 0) {
             bracket_from_grads(c, gPsi, gg[hi], br);                  // {Psi, g_{m+1}}
-            for (size_t i = 0; i < c->N; ++i) out.g[fi][i] += c->coef_up[m] * br[i];
+            for (size_t i = 0; i < c->N; ++i) out.g[fi][i] += c->coef_up[gm] * br[i];
           }
         }
     }
@@ -344,14 +355,15 @@ static void rhs_eval(const oracle_ctx* c, const State& s, State& out, double* ma
     const int sp = fi / c->Msp, m = fi % c->Msp;
     const double sgn = (sp == 0) ? (double)c->p.g_sign : -(double)c->p.g_sign;   // upper / lower signs of Eq. 6
     int lo = neighbour_index(c, sp, m - 1), hi = neighbour_index(c, sp, m + 1);
+    const int gm = c->moff + m;
 #pragma omp parallel for collapse(2) schedule(static)
     for (int iz = 0; iz < c->nz; ++iz)
       for (int iy = 0; iy < c->ny; ++iy)
         for (int ix = 0; ix < c->nx; ++ix) {
           size_t i = IDX(c, iz, iy, ix);
           cplx lin = s.g[fi][i];
-          if (lo >= 0) lin -= c->coef_dn[m] * s.g[lo][i];
-          if (hi >= 0) lin -= c->coef_up[m] * s.g[hi][i];
+          if (lo >= 0) lin -= c->coef_dn[gm] * s.g[lo][i];
+          if (hi >= 0) lin -= c->coef_up[gm] * s.g[hi][i];
           out.g[fi][i] += cplx(0.0, sgn * c->kz[iz]) * lin;
         }
   }
@@ -395,7 +407,7 @@ static void apply_dissipation(const oracle_ctx* c, State& s, double dt) {
         }
         for (int fi = 0; fi < c->M; ++fi) {
           const int m = fi % c->Msp;
-          double rate = rate_gk + p.nu_coll * std::pow((double)m / (double)c->Msp, 2.0 * p.p);   // Eq. 19
+          double rate = rate_gk + p.nu_coll * std::pow((double)(c->moff + m) / (double)c->Mg, 2.0 * p.p);   // Eq. 19 (global m and M, Q31)
           s.g[fi][i] *= std::exp(-rate * dt);
         }
       }
@@ -466,7 +478,7 @@ static void apply_forcing(oracle_ctx* c, State& s, double dt) {
 // RNG key seed ^ 0xA5A5A5A5A5A5A5A5, counters 2*step and 2*step+1; Box-Muller as in apply_forcing.
 static void apply_forcing_g(oracle_ctx* c, State& s, double dt) {
   const oracle_params& p = c->p;
-  if (!(p.force_g_amp > 0.0) || c->M < 1) return;
+  if (!(p.force_g_amp > 0.0) || c->M < 1 || c->moff != 0) return;   // g_0 lives on the shard with m_offset = 0
   unsigned long long key = p.seed ^ 0xA5A5A5A5A5A5A5A5ULL;
   double u1 = rng_uniform(key, 2ULL * (unsigned long long)c->step), u2 = rng_uniform(key, 2ULL * (unsigned long long)c->step + 1ULL);
   double rad = std::sqrt(-2.0 * std::log(1.0 - u1));
@@ -493,7 +505,7 @@ static void energies(const oracle_ctx* c, const State& s, double out[6]) {
         Ek += 0.5 * k2 * std::norm(phi);
         Eb += 0.5 * k2 * std::norm(psi);
       }
-  for (int m = 0; m < c->M; ++m)
+  for (int m = c->own_lo; m < c->own_hi; ++m)            // owned moments (all of them unless sharded)
     for (size_t i = 0; i < c->N; ++i) Wg += 0.5 * std::norm(s.g[m][i]);
   out[0] = Ep + Em; out[1] = Ep; out[2] = Em; out[3] = Ek; out[4] = Eb; out[5] = Wg;
 }
@@ -571,10 +583,13 @@ static void propagate(const oracle_ctx* c, std::vector<std::vector<cplx>>& g, do
 // ---------------------------------------------------------------------------------------------
 // One complete step (Alg. 2; Alg. 1).
 // ---------------------------------------------------------------------------------------------
-static int step_once(oracle_ctx* c, double dt_in) {
+// The step is written as two stages so that a moment-sharded run (Q31) can refresh its halo moments in between; step_once
+// runs them back to back.  Stage 1: RHS at state_n, dt, half-step predictor -> (hw, hg).  Stage 2: midpoint RHS, corrector,
+// dissipation, forcing, time and diagnostics.
+static int step_stage1(oracle_ctx* c, double dt_in) {
   const int M = c->M;
   State sn; sn.w[0] = c->w[0]; sn.w[1] = c->w[1]; sn.g = c->g;
-  State k1, sh, k2;
+  State k1, sh;
   double dt = dt_in;
   double maxg2 = 0.0;
   // Alg. 2 l.2: CFL step from state_n (only when the caller asks for it: dt <= 0)
@@ -607,6 +622,18 @@ static int step_once(oracle_ctx* c, double dt_in) {
   for (int m = 0; m < M; ++m)
     for (size_t i = 0; i < c->N; ++i) sh.g[m][i] = sn.g[m][i] + (0.5 * dt) * k1.g[m][i];
   if (exact) propagate(c, sh.g, 0.5 * dt);                  // g_{n+1/2} = P(dt/2) (g_n + dt/2 R_n),  P(tau) = exp(s i kz (I - T) tau)
+  c->hw[0].swap(sh.w[0]); c->hw[1].swap(sh.w[1]); c->hg.swap(sh.g);
+  c->dt_cur = dt;
+  return 0;
+}
+
+static int step_stage2(oracle_ctx* c) {
+  const int M = c->M;
+  const bool exact = (c->p.hermite_exact != 0) && M > 0;
+  const double dt = c->dt_cur;
+  State sn; sn.w[0] = c->w[0]; sn.w[1] = c->w[1]; sn.g = c->g;
+  State sh; sh.w[0] = c->hw[0]; sh.w[1] = c->hw[1]; sh.g = c->hg;
+  State k2;
   // Alg. 1 l.6: midpoint RHS
   rhs_eval(c, sh, k2, nullptr, !exact);
   // Alg. 1 l.8-9: full-step corrector
@@ -650,6 +677,12 @@ static int step_once(oracle_ctx* c, double dt_in) {
   for (int i = 0; i < 6; ++i) c->hist.push_back(e[i]);
   for (int i = 0; i < 6; ++i) if (!std::isfinite(e[i])) { c->err = "non-finite energy"; return -3; }
   return 0;
+}
+
+static int step_once(oracle_ctx* c, double dt_in) {
+  int rc = step_stage1(c, dt_in);
+  if (rc) return rc;
+  return step_stage2(c);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -703,9 +736,16 @@ int oracle_create(const oracle_params* p, oracle_ctx** out) {
   if (p->M > 0 && p->vA != 1.0) return -4;                 // Q12
   if (p->nspecies != 1 && p->nspecies != 2) return -1;
   if (p->hermite_exact != 0 && p->hermite_exact != 1) return -1;
+  if (p->M_global != 0) {                                  // moment shard (Q31): one species, plain RK2 streaming
+    if (p->M < 1 || p->m_offset < 0 || p->m_offset + p->M > p->M_global || p->nspecies != 1 || p->hermite_exact) return -1;
+  } else if (p->m_offset != 0) return -1;
   oracle_ctx* c = new oracle_ctx();
   c->p = *p; c->nx = p->nx; c->ny = p->ny; c->nz = p->nz;
   c->Msp = p->M; c->nsp = p->nspecies; c->M = p->M * p->nspecies;
+  c->moff = p->m_offset; c->Mg = p->M_global ? p->M_global : p->M;
+  c->own_lo = (c->moff > 0) ? 1 : 0;
+  c->own_hi = (p->M_global && c->moff + p->M < c->Mg) ? c->M - 1 : c->M;
+  c->dt_cur = 0.0;
   c->N = (size_t)p->nx * p->ny * p->nz;
   c->kx.resize(c->nx); c->ky.resize(c->ny); c->kz.resize(c->nz);
   c->mx.resize(c->nx); c->my.resize(c->ny); c->mz.resize(c->nz);
@@ -714,14 +754,14 @@ int oracle_create(const oracle_params* p, oracle_ctx** out) {
   for (int i = 0; i < c->nz; ++i) { c->mz[i] = signed_mode(i, c->nz); c->kz[i] = 2 * PI * c->mz[i] / p->Lz; }
   c->w[0].assign(c->N, cplx(0, 0)); c->w[1].assign(c->N, cplx(0, 0));
   c->g.assign(c->M, std::vector<cplx>(c->N, cplx(0, 0)));
-  c->coef_dn.resize(c->Msp + 1); c->coef_up.resize(c->Msp + 1);
-  for (int m = 0; m <= c->Msp; ++m) {
+  c->coef_dn.resize(c->Mg + 1); c->coef_up.resize(c->Mg + 1);   // indexed by the GLOBAL moment number
+  for (int m = 0; m <= c->Mg; ++m) {
     c->coef_dn[m] = std::sqrt(m / 2.0);                    // Eq. 6c
     c->coef_up[m] = std::sqrt((m + 1) / 2.0);
   }
   if (p->hermite_coeff == 1) {                             // literal Eq. 6a / 6b (Q24)
-    if (c->Msp > 0) c->coef_up[0] = std::sqrt(2.0);
-    if (c->Msp > 1) c->coef_up[1] = std::sqrt(1.5);
+    if (c->Mg > 0) c->coef_up[0] = std::sqrt(2.0);
+    if (c->Mg > 1) c->coef_up[1] = std::sqrt(1.5);
   }
   c->t = 0.0; c->step = 0; c->last_dt = 0.0;
   *out = c;
@@ -882,6 +922,25 @@ int oracle_bracket_full(oracle_ctx* c, const double* f_hat, const double* g_hat,
   bracket_from_grads(c, gf, gg, b);
   for (size_t i = 0; i < c->N; ++i) { out[2 * i] = b[i].real(); out[2 * i + 1] = b[i].imag(); }
   if (max_imag) *max_imag = mi;
+  return 0;
+}
+// One stage of a step (stage 0: RHS at state_n + predictor; stage 1: midpoint RHS + corrector + dissipation + forcing + record).
+// A moment-sharded run exchanges its halo moments between the stages (Q31); oracle_step(dt, 1) == stage 0 then stage 1.
+int oracle_step_stage(oracle_ctx* c, double dt, int stage) {
+  if (!c || (stage != 0 && stage != 1)) return -1;
+  return stage == 0 ? step_stage1(c, dt) : step_stage2(c);
+}
+// Full-spectrum access to the half-step (stage) state, same field numbering as oracle_get_full.
+int oracle_get_stage_full(const oracle_ctx* c, int field, double* out) {
+  if (!c || field < 0 || field >= 2 + c->M || c->hw[0].size() != c->N) return -1;
+  const std::vector<cplx>& a = (field < 2) ? c->hw[field] : c->hg[field - 2];
+  for (size_t i = 0; i < c->N; ++i) { out[2 * i] = a[i].real(); out[2 * i + 1] = a[i].imag(); }
+  return 0;
+}
+int oracle_set_stage_full(oracle_ctx* c, int field, const double* in) {
+  if (!c || field < 0 || field >= 2 + c->M || c->hw[0].size() != c->N) return -1;
+  std::vector<cplx>& a = (field < 2) ? c->hw[field] : c->hg[field - 2];
+  for (size_t i = 0; i < c->N; ++i) a[i] = cplx(in[2 * i], in[2 * i + 1]);
   return 0;
 }
 // Full-spectrum access to the evolved vorticities / moments (field 0,1 = w+-, 2+m = g_m).

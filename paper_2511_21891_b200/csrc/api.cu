@@ -68,6 +68,7 @@ struct gandalf_ctx {
   long long hist_cap;
   // host bookkeeping
   long long step, hist_base; bool H_valid;   // history record i belongs to step hist_base + i
+  bool stage_pending, need_h;                // between gandalf_step_stage(.., 0) and (.., 1); whether this step keeps the hybrid copy
   int num_sms;
   long long launches;
   bool timing;
@@ -204,6 +205,7 @@ int gandalf_default_params(gandalf_params* p) {
   p->force_g_nz = 1;
   p->nspecies = 1;
   p->dt_max = 0.0; p->hermite_exact = 0;
+  p->m_offset = 0; p->M_global = 0;
   return GANDALF_OK;
 }
 
@@ -222,6 +224,12 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (p->hermite_exact != 0 && p->hermite_exact != 1) return GANDALF_ERR_INVALID;
   if (p->force_eps > 0.0 && (p->force_nperp_min < 0 || p->force_nperp_max > p->nx / 3 || p->force_nperp_max > p->ny / 3 ||
                              p->force_nz_max > p->nz / 3 || count_forced_pairs(p) == 0)) return GANDALF_ERR_INVALID;   // empty / unresolved shell
+  if (p->M_global != 0) {   // moment shard (Q31)
+    if (p->M < 1 || p->m_offset < 0 || p->m_offset + p->M > p->M_global) return GANDALF_ERR_INVALID;
+    if (p->nspecies != 1 || p->hermite_exact) return GANDALF_ERR_UNSUPPORTED;
+    if (p->m_offset > 0 && p->M < 2) return GANDALF_ERR_INVALID;               // a halo and at least one owned moment
+    if (p->m_offset + p->M < p->M_global && p->M < 2 + (p->m_offset > 0)) return GANDALF_ERR_INVALID;
+  } else if (p->m_offset != 0) return GANDALF_ERR_INVALID;
   if (p->M > 0 && p->vA != 1.0) return GANDALF_ERR_UNSUPPORTED;
   if (p->hermite_exact && p->M > 0 && (p->closure != 0 || p->hermite_coeff != 0)) return GANDALF_ERR_UNSUPPORTED;   // symmetric coupling matrix only (Q30)
   if (cudaSetDevice(p->device) != cudaSuccess) { cudaGetLastError(); return GANDALF_ERR_CUDA; }
@@ -233,6 +241,9 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   Dims& d = c->d;
   d.nx = p->nx; d.ny = p->ny; d.nz = p->nz;
   d.Msp = p->M; d.M = p->M * p->nspecies; d.F = 2 + d.M;     // d.M = number of moment FIELDS (species-major)
+  const int moff = p->m_offset, Mg = p->M_global ? p->M_global : p->M;   // global numbering of the moments (Q31)
+  const bool halo_lo = moff > 0, halo_hi = p->M_global != 0 && moff + p->M < Mg;
+  d.own_lo = halo_lo ? 1 : 0; d.own_hi = d.M - (halo_hi ? 1 : 0);
   d.hx = p->nx / 2 + 1;
   d.hx3 = p->nx / 3; d.hy3 = p->ny / 3; d.hz3 = p->nz / 3;
   d.Kx = d.hx3 + 1; d.Ky = 2 * d.hy3 + 1; d.Kz = 2 * d.hz3 + 1;
@@ -289,13 +300,16 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   const int Ms = d.Msp;
   for (int sp = 0; sp < p->nspecies; ++sp) {
     double* dns = dn.data() + sp * Ms; double* ups = up.data() + sp * Ms; double* crs = cr.data() + sp * Ms;
-    for (int m = 0; m < Ms; ++m) { dns[m] = std::sqrt(m / 2.0); ups[m] = std::sqrt((m + 1) / 2.0); }
-    if (p->hermite_coeff == 1) { if (Ms > 0) ups[0] = std::sqrt(2.0); if (Ms > 1) ups[1] = std::sqrt(1.5); }
-    if (Ms > 0) {
-      if (p->closure == 1 && Ms >= 2) dns[Ms - 1] += ups[Ms - 1];   // g_M := g_{M-2}
-      ups[Ms - 1] = 0.0;                                            // g_M := 0 otherwise
+    for (int m = 0; m < Ms; ++m) { const int gm = moff + m; dns[m] = std::sqrt(gm / 2.0); ups[m] = std::sqrt((gm + 1) / 2.0); }
+    if (p->hermite_coeff == 1) {
+      for (int m = 0; m < Ms; ++m) { if (moff + m == 0) ups[m] = std::sqrt(2.0); if (moff + m == 1) ups[m] = std::sqrt(1.5); }
     }
-    for (int m = 0; m < Ms; ++m) crs[m] = p->nu_coll * std::pow((double)m / (double)Ms, 2.0 * p->p);   // Eq. 19
+    if (Ms > 0) {
+      if (!halo_hi && p->closure == 1 && Ms >= 2) dns[Ms - 1] += ups[Ms - 1];   // g_M := g_{M-2}: the closure sits at the GLOBAL end
+      ups[Ms - 1] = 0.0;                                            // g_M := 0 otherwise; a shard's upper halo has no neighbour here
+      if (halo_lo) dns[0] = 0.0;                                    // the lower halo has none either (its own update is discarded)
+    }
+    for (int m = 0; m < Ms; ++m) crs[m] = p->nu_coll * std::pow((double)(moff + m) / (double)Mg, 2.0 * p->p);   // Eq. 19
   }
   // hermite_exact: T = V diag(lambda) V^T of the Msp x Msp coupling matrix (absorbing closure: symmetric tridiagonal)
   if (p->hermite_exact && Ms > 0) {
@@ -344,6 +358,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   }
   if (e != cudaSuccess) { cudaGetLastError(); free_all(c); delete c; return GANDALF_ERR_CUDA; }
   c->step = 0; c->hist_base = 0; c->H_valid = true; c->launches = 0; c->timing = false;
+  c->stage_pending = false; c->need_h = true;
   for (int i = 0; i < KC_N; ++i) { c->t_ms[i] = 0; c->t_n[i] = 0; }
   *out = c;
   return GANDALF_OK;
@@ -448,6 +463,7 @@ int gandalf_set_state_raw(gandalf_ctx* c, const double* in, int on_device) {
   GD_CUDA(c, cudaSetDevice(c->p.device));
   const size_t bytes = (size_t)c->d.F * c->d.PS * sizeof(cd);
   GD_CUDA(c, cudaMemcpyAsync(c->S0, in, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->st));
+  c->stage_pending = false;
   int rc = make_hybrid(c, c->S0);
   if (rc) return rc;
   c->H_valid = true;
@@ -483,7 +499,7 @@ int gandalf_set_state(gandalf_ctx* c, const double* zeta_hat, const double* g_ha
   GD_CUDA(c, timed(c, -1, 1, [&] { return launch_pack(d, zin, c->S0, 2, 2, c->st); }));
   if (d.M > 0) GD_CUDA(c, timed(c, -1, 1, [&] { return launch_pack(d, gin, c->S0 + 2 * d.PS, d.M, 0, c->st); }));
   GD_CUDA(c, cudaMemsetAsync(c->scal, 0, SC_COUNT * sizeof(double), c->st));
-  c->step = 0; c->hist_base = 0;
+  c->step = 0; c->hist_base = 0; c->stage_pending = false;
   int rc = make_hybrid(c, c->S0);
   if (rc) return rc;
   c->H_valid = true;
@@ -521,6 +537,7 @@ int gandalf_get_state(gandalf_ctx* c, double* zeta_hat, double* g_hat, int on_de
 int gandalf_rhs(gandalf_ctx* c, double* dw_hat, double* dg_hat, int on_device) {
   if (!c) return GANDALF_ERR_INVALID;
   if (!dw_hat || (c->d.M > 0 && !dg_hat)) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_rhs: NULL array");
+  if (c->stage_pending) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_rhs: a step is half done (the stage state would be overwritten)");
   GD_CUDA(c, cudaSetDevice(c->p.device));
   int rc;
   if (!c->H_valid) { rc = make_hybrid(c, c->S0); if (rc) return rc; c->H_valid = true; }
@@ -531,72 +548,129 @@ int gandalf_rhs(gandalf_ctx* c, double* dw_hat, double* dg_hat, int on_device) {
   return export_fields(c, c->S1, dw_hat, dg_hat, 0, on_device);
 }
 
+}  // extern "C"
+
+// One step = two stages (a moment-sharded run refreshes its halo moments in between, Q31).
+// Stage 0 (Alg. 2 l.2-6): RHS at t_n (its x-pass also yields max|grad Phi| for Eq. 16), dt, tables, half-step predictor.
+static int step_stage0(gandalf_ctx* c, double dt) {
+  const Dims& d = c->d;
+  const bool adaptive = !(dt > 0.0);
+  const double cfl_dxy = c->p.cfl * std::fmin(c->p.Lx / d.nx, c->p.Ly / d.ny);
+  const bool exact = c->p.hermite_exact && d.M > 0;
+  int rc = rhs_pipeline(c, adaptive);
+  if (rc) return rc;
+  GD_CUDA(c, timed(c, -1, 1, [&] {
+    return launch_prepare_dt(adaptive ? 0.0 : dt, cfl_dxy, c->p.dt_max, c->maxbits, c->scal, c->crate, c->collfac, d.M, c->st);
+  }));
+  GD_CUDA(c, timed(c, -1, 1, [&] { return launch_tables(d, c->ph, c->scal, c->tabz, c->tabp, c->st); }));
+  if (!exact) {
+    rc = stage_update(c, 1, c->S0, c->S0, c->S1, c->p.nonlinear);
+    if (rc) return rc;
+  } else {
+    // hermite_exact (Q30): with P = P(dt/2) = exp(s i kz (I - T) dt/2) per kz,
+    //   g_{n+1/2} = P (g_n + dt/2 R_n),   g_{n+1} = P (P g_n + dt R_{n+1/2}),   R = the bracket terms of Eq. 6;
+    // w+- exactly as above.  D is free between two RHS pipelines and serves as scratch for the propagated half-step state.
+    GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_propagator(d, c->p.g_sign, 0.5, c->scal, c->hxV, c->hxLam, c->hxP, c->st); }));
+    rc = stage_update(c, 1, c->S0, c->S0, c->S1, c->p.nonlinear, true);          // S1 = w_{n+1/2} | g_n + dt/2 R_n ; H(w+-)
+    if (rc) return rc;
+    GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_apply(d, c->S1, c->D, c->hxP, 0, c->collfac, c->tabz, c->tabp, c->st); }));
+    if (c->p.nonlinear) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->D + 2 * d.PS, c->H + 2 * d.PH, c->twz, d.M, c->st); }));
+  }
+  c->need_h = c->p.nonlinear || adaptive;
+  c->stage_pending = true;
+  return GANDALF_OK;
+}
+// Stage 1 (Alg. 2 l.7-14): midpoint RHS, full-step corrector + dissipation (in place on S0: each mode reads only its own S0
+// entry), forcing, energy record.
+static int step_stage1(gandalf_ctx* c) {
+  const Dims& d = c->d;
+  const bool exact = c->p.hermite_exact && d.M > 0;
+  const bool need_h = c->need_h;
+  int rc = rhs_pipeline(c, false);
+  if (rc) return rc;
+  if (!exact) {
+    rc = stage_update(c, 2, c->S0, c->S1, c->S0, need_h);
+    if (rc) return rc;
+  } else {
+    GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_apply(d, c->S0, c->S1, c->hxP, 0, c->collfac, c->tabz, c->tabp, c->st); }));   // S1(g) = P g_n
+    rc = stage_update(c, 2, c->S0, c->S1, c->S0, need_h, true);                   // S0(w) = w_{n+1};  S1(g) += dt R_{n+1/2}
+    if (rc) return rc;
+    GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_apply(d, c->S1, c->S0, c->hxP, 1, c->collfac, c->tabz, c->tabp, c->st); }));   // S0(g) = diss . P S1(g)
+    if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0 + 2 * d.PS, c->H + 2 * d.PH, c->twz, d.M, c->st); }));
+  }
+  if (c->npairs) {
+    GD_CUDA(c, timed(c, -1, 1, [&] {
+      return launch_forcing(d, c->S0, c->pairs, c->npairs, c->force_amp, c->p.seed, c->step, c->scal, c->st);
+    }));
+    // the forcing touches w+- only: refresh the hybrid copy of those two fields
+    if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0, c->H, c->twz, 2, c->st); }));
+  }
+  if (c->p.force_g_amp > 0.0 && c->p.m_offset == 0) {     // g_0 lives on the shard with m_offset = 0
+    GD_CUDA(c, timed(c, -1, 1, [&] {
+      return launch_forcing_g(d, c->S0, c->p.force_g_nz, c->p.force_g_amp, c->p.seed, c->step, c->scal, c->st);
+    }));
+    // the forcing touches g_0 only: refresh the hybrid copy of that field
+    if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0 + 2 * d.PS, c->H + 2 * d.PH, c->twz, 1, c->st); }));
+  }
+  GD_CUDA(c, timed(c, -1, 2, [&] {
+    return launch_energy(d, c->S0, c->partial, kEnergyBlocks, c->hist + (size_t)(c->step - c->hist_base) * 7, c->scal, 1, c->st);
+  }));
+  c->step += 1;
+  c->H_valid = need_h;
+  c->stage_pending = false;
+  return GANDALF_OK;
+}
+
+extern "C" {
+
 int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
   if (!c) return GANDALF_ERR_INVALID;
   if (nsteps < 0 || !std::isfinite(dt)) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_step: bad dt or nsteps");
+  if (c->stage_pending) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_step: a step is half done (gandalf_step_stage(.., 0) without stage 1)");
   GD_CUDA(c, cudaSetDevice(c->p.device));
-  const Dims& d = c->d;
   int rc = ensure_hist(c, c->step - c->hist_base + nsteps);
   if (rc) return rc;
-  const bool adaptive = !(dt > 0.0);
-  const double cfl_dxy = c->p.cfl * std::fmin(c->p.Lx / d.nx, c->p.Ly / d.ny);
   if (!c->H_valid) { rc = make_hybrid(c, c->S0); if (rc) return rc; c->H_valid = true; }
-  const bool need_h = c->p.nonlinear || adaptive;
-  const bool exact = c->p.hermite_exact && d.M > 0;
   for (int i = 0; i < nsteps; ++i) {
-    // Alg. 2 l.3-6: RHS at t_n (its x-pass also yields max|grad Phi| for Eq. 16), half-step predictor
-    rc = rhs_pipeline(c, adaptive);
+    rc = step_stage0(c, dt);
     if (rc) return rc;
-    GD_CUDA(c, timed(c, -1, 1, [&] {
-      return launch_prepare_dt(adaptive ? 0.0 : dt, cfl_dxy, c->p.dt_max, c->maxbits, c->scal, c->crate, c->collfac, d.M, c->st);
-    }));
-    GD_CUDA(c, timed(c, -1, 1, [&] { return launch_tables(d, c->ph, c->scal, c->tabz, c->tabp, c->st); }));
-    if (!exact) {
-      rc = stage_update(c, 1, c->S0, c->S0, c->S1, c->p.nonlinear);
-      if (rc) return rc;
-      // Alg. 2 l.7-9: midpoint RHS
-      rc = rhs_pipeline(c, false);
-      if (rc) return rc;
-      // Alg. 2 l.10-14: full step + dissipation (in place on S0: each mode reads only its own S0 entry)
-      rc = stage_update(c, 2, c->S0, c->S1, c->S0, need_h);
-      if (rc) return rc;
-    } else {
-      // hermite_exact (Q30): with P = P(dt/2) = exp(s i kz (I - T) dt/2) per kz,
-      //   g_{n+1/2} = P (g_n + dt/2 R_n),   g_{n+1} = P (P g_n + dt R_{n+1/2}),   R = the bracket terms of Eq. 6;
-      // w+- exactly as above.  D is free between two RHS pipelines and serves as scratch for the propagated half-step state.
-      GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_propagator(d, c->p.g_sign, 0.5, c->scal, c->hxV, c->hxLam, c->hxP, c->st); }));
-      rc = stage_update(c, 1, c->S0, c->S0, c->S1, c->p.nonlinear, true);          // S1 = w_{n+1/2} | g_n + dt/2 R_n ; H(w+-)
-      if (rc) return rc;
-      GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_apply(d, c->S1, c->D, c->hxP, 0, c->collfac, c->tabz, c->tabp, c->st); }));
-      if (c->p.nonlinear) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->D + 2 * d.PS, c->H + 2 * d.PH, c->twz, d.M, c->st); }));
-      rc = rhs_pipeline(c, false);                                                  // brackets at the midpoint state
-      if (rc) return rc;
-      GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_apply(d, c->S0, c->S1, c->hxP, 0, c->collfac, c->tabz, c->tabp, c->st); }));   // S1(g) = P g_n
-      rc = stage_update(c, 2, c->S0, c->S1, c->S0, need_h, true);                   // S0(w) = w_{n+1};  S1(g) += dt R_{n+1/2}
-      if (rc) return rc;
-      GD_CUDA(c, timed(c, -1, 1, [&] { return launch_hermite_apply(d, c->S1, c->S0, c->hxP, 1, c->collfac, c->tabz, c->tabp, c->st); }));   // S0(g) = diss . P S1(g)
-      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0 + 2 * d.PS, c->H + 2 * d.PH, c->twz, d.M, c->st); }));
-    }
-    if (c->npairs) {
-      GD_CUDA(c, timed(c, -1, 1, [&] {
-        return launch_forcing(d, c->S0, c->pairs, c->npairs, c->force_amp, c->p.seed, c->step, c->scal, c->st);
-      }));
-      // the forcing touches w+- only: refresh the hybrid copy of those two fields
-      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0, c->H, c->twz, 2, c->st); }));
-    }
-    if (c->p.force_g_amp > 0.0) {
-      GD_CUDA(c, timed(c, -1, 1, [&] {
-        return launch_forcing_g(d, c->S0, c->p.force_g_nz, c->p.force_g_amp, c->p.seed, c->step, c->scal, c->st);
-      }));
-      // the forcing touches g_0 only: refresh the hybrid copy of that field
-      if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0 + 2 * d.PS, c->H + 2 * d.PH, c->twz, 1, c->st); }));
-    }
-    GD_CUDA(c, timed(c, -1, 2, [&] {
-      return launch_energy(d, c->S0, c->partial, kEnergyBlocks, c->hist + (size_t)(c->step - c->hist_base) * 7, c->scal, 1, c->st);
-    }));
-    c->step += 1;
+    rc = step_stage1(c);
+    if (rc) return rc;
   }
-  c->H_valid = need_h;
+  return GANDALF_OK;
+}
+
+int gandalf_step_stage(gandalf_ctx* c, double dt, int stage) {
+  if (!c) return GANDALF_ERR_INVALID;
+  if ((stage != 0 && stage != 1) || !std::isfinite(dt)) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_step_stage: bad dt or stage");
+  if ((stage == 1) != c->stage_pending) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_step_stage: stages must alternate 0, 1");
+  GD_CUDA(c, cudaSetDevice(c->p.device));
+  if (stage == 1) return step_stage1(c);
+  int rc = ensure_hist(c, c->step - c->hist_base + 1);
+  if (rc) return rc;
+  if (!c->H_valid) { rc = make_hybrid(c, c->S0); if (rc) return rc; c->H_valid = true; }
+  return step_stage0(c, dt);
+}
+
+int gandalf_field_ptr(gandalf_ctx* c, int state, int field, void** device_ptr, long long* ncomplex) {
+  if (!c || !device_ptr) return GANDALF_ERR_INVALID;
+  if ((state != 0 && state != 1) || field < 0 || field >= c->d.F) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_field_ptr: bad state or field");
+  *device_ptr = (state == 0 ? c->S0 : c->S1) + (size_t)field * c->d.PS;
+  if (ncomplex) *ncomplex = (long long)c->d.PS;
+  return GANDALF_OK;
+}
+
+int gandalf_halo_refresh(gandalf_ctx* c, int state) {
+  if (!c) return GANDALF_ERR_INVALID;
+  if (state != 0 && state != 1) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_halo_refresh: bad state");
+  GD_CUDA(c, cudaSetDevice(c->p.device));
+  const Dims& d = c->d;
+  const cd* S = state == 0 ? c->S0 : c->S1;
+  if (d.own_lo > 0) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, S + 2 * d.PS, c->H + 2 * d.PH, c->twz, 1, c->st); }));
+  if (d.own_hi < d.M) {
+    const size_t f = (size_t)(2 + d.M - 1);
+    GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, S + f * d.PS, c->H + f * d.PH, c->twz, 1, c->st); }));
+  }
   return GANDALF_OK;
 }
 

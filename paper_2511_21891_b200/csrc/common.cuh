@@ -17,6 +17,7 @@
 struct Dims {
   int nx, ny, nz, M, F;   // M = number of moment FIELDS (nspecies * Msp), F = 2 + M
   int Msp;                // moments per species
+  int own_lo, own_hi;     // owned moment fields [own_lo, own_hi) (all of them unless the context is a moment shard with halos, Q31)
   int hx;                 // nx/2+1 (boundary layout)
   int Kx, Ky, Kz;         // retained counts
   int Kxp, Kxe;           // row strides (>= Kx) of the hybrid arrays H, Gh and of E

@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(256) k_energy_partial(Dims d, const cd* __rest
       acc[3] += wgt * 0.5 * (sm.x * sm.x + sm.y * sm.y) * ik2;
     }
     double g2 = 0.0;
-    for (int m = 0; m < d.M; ++m) {
+    for (int m = d.own_lo; m < d.own_hi; ++m) {          // owned moments (a shard's halo copies belong to its neighbours)
       const cd g = S[(size_t)(2 + m) * d.PS + idx];
       g2 += g.x * g.x + g.y * g.y;
     }

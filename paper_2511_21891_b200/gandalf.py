@@ -35,6 +35,7 @@ class GandalfParams(C.Structure):
         ("force_g_amp", C.c_double), ("force_g_nz", C.c_int),
         ("nspecies", C.c_int),
         ("dt_max", C.c_double), ("hermite_exact", C.c_int),
+        ("m_offset", C.c_int), ("M_global", C.c_int),
         ("device", C.c_int),
         ("stream", C.c_void_p),
     ]
@@ -75,6 +76,9 @@ def load_library():
     lib.gandalf_kperp_spectrum.argtypes = [V, I, I, PD]
     lib.gandalf_hermite_spectrum.argtypes = [V, PD]
     lib.gandalf_kpar_spectrum.argtypes = [V, I, PD]
+    lib.gandalf_step_stage.argtypes = [V, D, I]
+    lib.gandalf_field_ptr.argtypes = [V, I, I, C.POINTER(V), C.POINTER(C.c_longlong)]
+    lib.gandalf_halo_refresh.argtypes = [V, I]
     lib.gandalf_energy_history.argtypes = [V, I, PD, C.POINTER(I)]
     lib.gandalf_get_time.argtypes = [V, PD, C.POINTER(C.c_longlong), PD]
     lib.gandalf_launch_count.argtypes = [V]
@@ -223,6 +227,25 @@ class Gandalf:
 
     def step(self, dt, nsteps=1):
         self._ck(self._lib.gandalf_step(self._h, float(dt), int(nsteps)))
+
+    def step_stage(self, dt, stage):
+        """gandalf_step_stage: stage 0 = RHS + predictor, stage 1 = midpoint RHS + corrector + ... (moment-sharded runs
+        refresh their halo moments in between)."""
+        self._ck(self._lib.gandalf_step_stage(self._h, float(dt), int(stage)))
+
+    def field_tensor(self, state, field):
+        """Zero-copy torch view (float64, 2 * ncomplex entries) of one field of the raw retained-mode array
+        (gandalf_field_ptr): state 0 = the state, 1 = the half-step stage state; field 0, 1 = w+-, 2+j = local moment j."""
+        import torch
+        ptr, n = C.c_void_p(), C.c_longlong()
+        self._ck(self._lib.gandalf_field_ptr(self._h, int(state), int(field), C.byref(ptr), C.byref(n)))
+
+        class _View:       # the CUDA array interface lets torch wrap a raw device pointer without copying
+            __cuda_array_interface__ = {"shape": (2 * n.value,), "typestr": "<f8", "data": (ptr.value, False), "version": 2}
+        return torch.as_tensor(_View(), device=f"cuda:{self.params.device}")
+
+    def halo_refresh(self, state):
+        self._ck(self._lib.gandalf_halo_refresh(self._h, int(state)))
 
     def energy(self):
         out = np.zeros(6)
