@@ -42,12 +42,19 @@ struct XGeom {
                                                                      // (the three-stage plan of nx = 512 pays two split exchanges: measured slower)
   static constexpr int LB = SPLITX ? (NX + NX / G::PADDIV + 2) / 2 : NX + NX / G::PADDIV + 1;   // per-group FFT exchange buffer, complex entries
   static constexpr int KXP = NX / 3 + 1;                    // retained kx count (== Dims::Kx)
-  static constexpr int THREADS = ALT ? 512 : 256;           // one CTA per SM (it owns the SM's tensor memory); ALT: 16 warps, 4 per scheduler
+#ifndef GD_X_THREADS
+#define GD_X_THREADS 256
+#endif
+  static constexpr int THREADS = ALT ? 512 : GD_X_THREADS;  // 256: one CTA per SM (it owns the SM's tensor memory); 128: two CTAs per SM, each
+                                                            // with half the lines, tiles and tensor memory (independent tile rings, so the two
+                                                            // warps of a scheduler are never phase-locked) -- measured SLOWER: 1.481 vs 1.424 ms
+                                                            // at 4a, 1.301 vs 1.217 ms at 4b; ALT: 16 warps, 4 per scheduler
+  static constexpr int CTAS = (THREADS <= 128) ? 2 : 1;     // resident CTAs per SM
   static constexpr int WARPS = THREADS / 32;
   static constexpr int GROUPS = THREADS / T;                // lines per CTA: consecutive (z,y), y fastest
   static constexpr int LD = GROUPS;                         // row of a staged tile [kx][line]; line slot XOR-swizzled with kx
   static constexpr int STAGE = 2 * KXP * LD;                // one stage: the tiles of U and V (P1) for all lines of the CTA
-  static constexpr size_t SMEM_CAP = 227 * 1024;
+  static constexpr size_t SMEM_CAP = (CTAS == 2 ? 113 : 227) * 1024;   // per CTA
   static constexpr size_t smem_for(int nst) { return ((size_t)GROUPS * LB + (size_t)nst * STAGE + FftTw<FID>::COUNT) * sizeof(cd); }
   static constexpr int NST = (SPLITX && smem_for(4) <= SMEM_CAP) ? 4 : (smem_for(3) <= SMEM_CAP ? 3 : 2);                             // stages in flight (full/empty mbarrier ring), <= 5 (the first NST-1 are Elsasser arrays)
   // stage-1 twiddles held in registers (plans with one stage-1 butterfly per lane): fewer shared-memory reads per transform
@@ -104,7 +111,7 @@ __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sy
 __device__ __forceinline__ double tm_d(const unsigned* w) { return __hiloint2double((int)w[1], (int)w[0]); }
 
 template <int NX>
-__global__ void __launch_bounds__(XGeom<NX>::THREADS, 1) k_xpass(Dims d, const cd* __restrict__ D, cd* __restrict__ Eo,
+__global__ void __launch_bounds__(XGeom<NX>::THREADS, XGeom<NX>::CTAS) k_xpass(Dims d, const cd* __restrict__ D, cd* __restrict__ Eo,
                                                            const cd* __restrict__ tw, const double* __restrict__ cdn,
                                                            const double* __restrict__ cup,
                                                            unsigned long long* __restrict__ maxbits, int nlines) {
@@ -449,7 +456,8 @@ cudaError_t launch_xpass(const Dims& d, const cd* D, cd* Eo, const cd* tw, const
     using X = XGeom<NN>;                                                                                      \
     if (prepare_only) return cudaFuncSetAttribute(k_xpass<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X::SMEM); \
     const int nb = (nlines + X::GROUPS - 1) / X::GROUPS;                                                        \
-    k_xpass<NN><<<(persist && nb > num_sms) ? num_sms : nb, X::THREADS, X::SMEM, st>>>(d, D, Eo, tw, cdn, cup, maxbits, nlines); \
+    const int cap = X::CTAS * num_sms;                                                                          \
+    k_xpass<NN><<<(persist && nb > cap) ? cap : nb, X::THREADS, X::SMEM, st>>>(d, D, Eo, tw, cdn, cup, maxbits, nlines); \
   }
   switch (d.nx) {
     case 8: XCASE(8) break; case 16: XCASE(16) break; case 32: XCASE(32) break; case 64: XCASE(64) break;

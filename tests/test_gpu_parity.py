@@ -268,10 +268,11 @@ def test_velocity_space_benchmark_forced_g0_large_M():
 
 
 def test_velocity_space_benchmark_linear_cascade_slope_reported():
-    """The linear phase-mixing run itself (brackets off, 5000 steps to t = 50): the time-averaged C_m is reported with its
-    fitted slope over m in [2, 20] (paper: -0.50 +- 0.02, PAPER.md:617 -- a statistical result of the paper's own forcing
-    normalisation and averaging window: PARITY UNPINNED); gated only on the GPU/oracle agreement of
-    the first 200 steps and on a decaying, finite spectrum."""
+    """The linear phase-mixing run itself (brackets off, 20 000 steps to t = 200): the time-averaged C_m is reported with its
+    fitted slope over m in [2, 20] and [8, 64] (paper: -0.50 +- 0.02, PAPER.md:617 -- a statistical result: PARITY UNPINNED,
+    DESIGN.md section 7).  Round 1 reported -0.38 from 24 samples in t in [25, 50]; the white-noise forcing needs a longer
+    average: over [25, 200] two seeds and both closures give -0.47 .. -0.49 on [2, 20] and -0.50 .. -0.51 on [8, 64]
+    (BASELINE.md section 5).  Gated on the GPU/oracle agreement of the first 200 steps and on a loose band around -1/2."""
     from paper_2511_21891_b200.gandalf import Gandalf
     shape, M = (32, 32, 32), 128
     prm = dict(M=M, nu_coll=0.25, p=6.0, force_g_amp=0.0035, force_g_nz=1, seed=2024, nonlinear=0)
@@ -281,15 +282,17 @@ def test_velocity_space_benchmark_linear_cascade_slope_reported():
     o.step(0.01, 200); g.step(0.01, 200)
     assert np.abs(g.hermite_spectrum() - o.hermite_spectrum()).max() <= 1e-10 * o.hermite_spectrum().max()
     acc, n = np.zeros(M), 0
-    for _ in range(48):
+    for _ in range(198):
         g.step(0.01, 100)
-        if g.time()[1] >= 2500:
+        if g.time()[0] >= 25.0:
             acc += g.hermite_spectrum(); n += 1
     cm = acc / n
-    ms = np.arange(2, 21)
-    slope = np.polyfit(np.log(ms), np.log(cm[2:21]), 1)[0]
-    print(f"velocity-space benchmark: time-averaged C_m slope over m in [2,20] = {slope:.3f} (paper: -0.50 +- 0.02)")
-    assert np.isfinite(cm).all() and cm[2] > cm[20] > cm[100] and slope < 0
+    s1 = np.polyfit(np.log(np.arange(2, 21)), np.log(cm[2:21]), 1)[0]
+    s2 = np.polyfit(np.log(np.arange(8, 65)), np.log(cm[8:65]), 1)[0]
+    print(f"velocity-space benchmark: time-averaged C_m slope, t in [25,200]: {s1:.3f} over m in [2,20], {s2:.3f} over [8,64] "
+          f"(paper: -0.50 +- 0.02)")
+    assert np.isfinite(cm).all() and cm[2] > cm[20] > cm[100]
+    assert -0.58 < s1 < -0.40 and -0.58 < s2 < -0.42
 
 
 def test_repeated_runs_are_bit_identical():
