@@ -573,6 +573,18 @@ def main():
         alu = {"measured_fp64_fma_tflops": mb[0], "measured_fp64_t_instr_per_s": mb[1], "how": "gandalf_microbench(0): dependency-free DFMA chains, all SMs, best of 5",
                "kernels": {k: {"transform_gflop_per_launch": nfft[k] / 1e9, "achieved_tflops": nfft[k] / 1e12 / (kern[k]["avg_ms"] * 1e-3),
                                "frac_of_measured_fp64_peak": nfft[k] / 1e12 / (kern[k]["avg_ms"] * 1e-3) / mb[0]} for k in nfft if k in kern}}
+        # instruction side: executed fp64 warp instructions per launch from the committed ncu capture (profiles/), against
+        # the issue rate measured above -- the roofline that actually bounds the x-pass's transforms
+        try:
+            for ln in open(os.path.join(ROOT, "profiles", "r02_fp64_instr.csv")).read().splitlines()[1:]:
+                w, k, n_ = ln.split(",")
+                if w == args.workload and k == dom and k in kern:
+                    rate = float(n_) * 32 / (kern[k]["avg_ms"] * 1e-3)
+                    alu["instr"] = {"kernel": k, "fp64_warp_instructions_per_launch": float(n_), "achieved_t_instr_per_s": rate / 1e12,
+                                    "frac_of_measured_issue_rate": rate / 1e12 / mb[1],
+                                    "source": "profiles/r02_fp64_instr.csv (ncu source page, committed; not counted in this run)"}
+        except Exception:
+            pass
     except Exception as exc:
         alu = {"error": repr(exc)[:200]}
     step_ms = ms / args.steps

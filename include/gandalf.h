@@ -172,6 +172,12 @@ int gandalf_kperp_spectrum(gandalf_ctx* ctx, int nbins, int literal_eq26, double
  * (nothing is written when M = 0).  SURVEY.md 8(f) rank 1. */
 int gandalf_hermite_spectrum(gandalf_ctx* ctx, double* out);
 
+/* Truncation monitor of the Hermite expansion [PAPER.md:269, section 3.5: "GANDALF monitors convergence via the energy ratio
+ * E_M/E_total (energy in the single highest retained moment m = M relative to total energy), typically requiring this to fall
+ * below 1e-3"; Q32]: *out = E_M / (E_A + W_g) with E_M = 1/2 sum_k |g_{M-1}(k)|^2 (summed over the species).
+ * Host output, synchronises.  INVALID when M = 0; UNSUPPORTED on a moment shard (the driver combines the shards' spectra). */
+int gandalf_truncation_ratio(gandalf_ctx* ctx, double* out);
+
 /* Parallel spectrum E(k_par) [PAPER.md:385; Q25]: bin j = |n_z|, j = 0..nbins-1, of the Alfvenic mode
  * energy 1/4 kperp^2 (|xi+|^2 + |xi-|^2) summed over (kx, ky) (bins sum to E_A; bins above nz/3 are zero).
  * out: nbins doubles on the HOST. */

@@ -73,6 +73,7 @@ def _load():
         lib.oracle_kperp_spectrum.argtypes = [C.c_void_p, C.c_int, C.c_int, P]
         lib.oracle_hermite_spectrum.argtypes = [C.c_void_p, P]
         lib.oracle_kpar_spectrum.argtypes = [C.c_void_p, C.c_int, P]
+        lib.oracle_truncation_ratio.argtypes = [C.c_void_p, P]
         lib.oracle_energy_history.argtypes = [C.c_void_p, C.c_int, P, C.POINTER(C.c_int)]
         lib.oracle_get_time.argtypes = [C.c_void_p, P, C.POINTER(C.c_longlong), P]
         lib.oracle_set_time.argtypes = [C.c_void_p, C.c_double, C.c_longlong]
@@ -205,6 +206,11 @@ class Oracle:
         out = np.zeros(max(self.M, 1))
         self._check(self._lib.oracle_hermite_spectrum(self._h, _dp(out)), "hermite spectrum")
         return out[: self.M]
+
+    def truncation_ratio(self):
+        out = np.zeros(1)
+        self._check(self._lib.oracle_truncation_ratio(self._h, _dp(out)), "truncation ratio")
+        return float(out[0])
 
     def kpar_spectrum(self, nbins):
         out = np.zeros(nbins)

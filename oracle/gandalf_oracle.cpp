@@ -855,6 +855,21 @@ int oracle_hermite_spectrum(oracle_ctx* c, double* out) {
   return 0;
 }
 
+// Truncation monitor (section 3.5: "the energy ratio E_M/E_total (energy in the single highest retained moment
+// m = M relative to total energy)"; reading Q32): E_M = 1/2 sum_k |g_{M-1}|^2 summed over the species, E_total = E_A + W_g.
+int oracle_truncation_ratio(oracle_ctx* c, double* out) {
+  if (!c || !out || c->M < 1 || c->p.M_global != 0) return -1;
+  double eM = 0.0;
+  for (int sp = 0; sp < c->nsp; ++sp) {
+    const std::vector<cplx>& g = c->g[sp * c->Msp + c->Msp - 1];
+    for (size_t i = 0; i < c->N; ++i) eM += 0.5 * std::norm(g[i]);
+  }
+  State cur; cur.w[0] = c->w[0]; cur.w[1] = c->w[1]; cur.g = c->g;
+  double e[6]; energies(c, cur, e);
+  *out = eM / (e[0] + e[5]);
+  return 0;
+}
+
 // Parallel spectrum (Q25): bin j = |n_z| of the Alfvenic mode energy 1/4 kperp^2 (|xi+|^2+|xi-|^2).
 int oracle_kpar_spectrum(oracle_ctx* c, int nbins, double* out) {
   if (!c || !out || nbins <= 0) return -1;

@@ -722,6 +722,22 @@ int gandalf_hermite_spectrum(gandalf_ctx* c, double* out) {
   return GANDALF_OK;
 }
 
+int gandalf_truncation_ratio(gandalf_ctx* c, double* out) {
+  if (!c || !out) return GANDALF_ERR_INVALID;
+  if (c->d.M < 1) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_truncation_ratio: no moments");
+  if (c->p.M_global != 0) GD_FAIL(c, GANDALF_ERR_UNSUPPORTED, "gandalf_truncation_ratio: moment shard");
+  std::vector<double> cm((size_t)c->d.M);
+  int rc = gandalf_hermite_spectrum(c, cm.data());
+  if (rc) return rc;
+  double e[6];
+  rc = gandalf_energy(c, e);
+  if (rc) return rc;
+  double eM = 0.0;
+  for (int sp = 0; sp < c->p.nspecies; ++sp) eM += 0.5 * cm[(size_t)sp * c->d.Msp + c->d.Msp - 1];
+  *out = eM / (e[0] + e[5]);
+  return GANDALF_OK;
+}
+
 int gandalf_kpar_spectrum(gandalf_ctx* c, int nbins, double* out) {
   if (!c || !out || nbins <= 0 || nbins > 65535) return GANDALF_ERR_INVALID;
   GD_CUDA(c, cudaSetDevice(c->p.device));

@@ -76,6 +76,7 @@ def load_library():
     lib.gandalf_kperp_spectrum.argtypes = [V, I, I, PD]
     lib.gandalf_hermite_spectrum.argtypes = [V, PD]
     lib.gandalf_kpar_spectrum.argtypes = [V, I, PD]
+    lib.gandalf_truncation_ratio.argtypes = [V, PD]
     lib.gandalf_step_stage.argtypes = [V, D, I]
     lib.gandalf_field_ptr.argtypes = [V, I, I, C.POINTER(V), C.POINTER(C.c_longlong)]
     lib.gandalf_halo_refresh.argtypes = [V, I]
@@ -261,6 +262,12 @@ class Gandalf:
         out = np.zeros(max(self.M, 1))
         self._ck(self._lib.gandalf_hermite_spectrum(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
         return out[: self.M]
+
+    def truncation_ratio(self):
+        """E_M / E_total of PAPER.md:269 (gandalf_truncation_ratio)."""
+        out = C.c_double()
+        self._ck(self._lib.gandalf_truncation_ratio(self._h, C.byref(out)))
+        return out.value
 
     def kpar_spectrum(self, nbins):
         out = np.zeros(nbins)

@@ -42,7 +42,9 @@ def test_default_params_layout_matches_binding(lib):
                                  dict(r=0), dict(g_sign=0), dict(eta=-1.0), dict(closure=2), dict(dt_max=-1.0), dict(cfl=0.0),
                                  dict(hermite_exact=2), dict(nspecies=3),
                                  dict(force_eps=1.0, force_nz_max=-1), dict(force_eps=1.0, force_nperp_min=3, force_nperp_max=2),
-                                 dict(force_eps=1.0, force_nperp_max=20)])
+                                 dict(force_eps=1.0, force_nperp_max=20),
+                                 dict(M=4, m_offset=2, M_global=5), dict(M=4, m_offset=1), dict(M=0, M_global=8), dict(M=4, m_offset=-1, M_global=8),
+                                 dict(M=1, m_offset=3, M_global=8), dict(M=2, m_offset=3, M_global=8)])
 def test_create_rejects_bad_parameters_before_touching_cuda(lib, bad):
     from paper_2511_21891_b200.gandalf import GandalfParams
     p = GandalfParams()
@@ -63,7 +65,24 @@ def test_unsupported_combination(lib):
     assert lib.gandalf_create(C.byref(p), C.byref(h)) == -4
 
 
+@pytest.mark.parametrize("combo", [dict(M=4, M_global=8, nspecies=2), dict(M=4, M_global=8, hermite_exact=1),
+                                   dict(M=4, hermite_exact=1, closure=1), dict(M=4, hermite_exact=1, hermite_coeff=1)])
+def test_unsupported_shard_and_exact_combinations(lib, combo):
+    """Moment shards (Q31) take one species and the RK2 streaming step; the exact propagator (Q30) a symmetric
+    coupling matrix."""
+    from paper_2511_21891_b200.gandalf import GandalfParams
+    p = GandalfParams()
+    lib.gandalf_default_params(C.byref(p))
+    for k, v in combo.items():
+        setattr(p, k, v)
+    h = C.c_void_p()
+    assert lib.gandalf_create(C.byref(p), C.byref(h)) == -4
+    assert not h.value
+
+
 def test_null_handles(lib):
+    assert lib.gandalf_step_stage(None, 0.1, 0) == -1 and lib.gandalf_halo_refresh(None, 0) == -1
+    assert lib.gandalf_field_ptr(None, 0, 0, None, None) == -1
     assert lib.gandalf_step(None, 0.1, 1) == -1
     assert lib.gandalf_destroy(None) == -1
     assert lib.gandalf_set_time(None, 0.0, 0) == -1 and lib.gandalf_set_state_raw(None, None, 0) == -1

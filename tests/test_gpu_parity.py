@@ -295,6 +295,20 @@ def test_velocity_space_benchmark_linear_cascade_slope_reported():
     assert -0.58 < s1 < -0.40 and -0.58 < s2 < -0.42
 
 
+def test_truncation_ratio_matches_oracle():
+    """E_M / E_total (Q32) after a few steps, one and two species."""
+    for extra in (dict(), dict(nspecies=2)):
+        prm, z, gm, run = config2(32, 32, 16, 6)
+        prm = dict(prm, **extra)
+        if extra:
+            gm = np.concatenate([gm, 0.5 * gm])
+        o, g = _pair(run["shape"], prm)
+        o.set_state(z, gm); g.set_state(z, gm)
+        o.step(run["dt"], 5); g.step(run["dt"], 5)
+        ro, rg = o.truncation_ratio(), g.truncation_ratio()
+        assert ro > 0 and abs(rg - ro) <= 1e-9 * ro
+
+
 def test_repeated_runs_are_bit_identical():
     """No result depends on CTA scheduling: fixed-order reductions, no floating-point atomics (the CFL maximum is an
     order-independent atomicMax), persistent kernels that assign work by index.  Two runs of config 3 (forcing + CFL dt)

@@ -420,3 +420,23 @@ def test_p21_exact_streaming_with_brackets_is_second_order_and_consistent():
     for o in (both, op, om):
         o.step(1e-2, 3)
     assert np.array_equal(both.get_state()[1][:2], op.get_state()[1]) and np.array_equal(both.get_state()[1][2:], om.get_state()[1])
+
+
+# ---- P22: truncation monitor E_M / E_total (section 3.5; Q32) -------------------------------------
+def test_p22_truncation_ratio_closed_form():
+    """g_m = a_m cos(x + z) for every m, xi+ = cos(x), xi- = 0: |g_hat| = a_m/2 at two modes => 1/2 sum_k |g_m|^2 = a_m^2/4;
+    E_A = 1/4 k^2 |xi+|^2 summed over the two modes (+-1,0,0) with |xi_hat| = 1/2 => 1/8."""
+    nx, ny, nz, M = 8, 8, 8, 4
+    a = np.array([1.0, 0.5, 0.25, 0.03])
+    Z, Y, X = _grid(nx, ny, nz)
+    zeta = np.stack([_half(np.cos(X)), _half(0 * X)])
+    g = np.stack([_half(am * np.cos(X + Z)) for am in a])
+    o = Oracle(nx, ny, nz, M=M)
+    o.set_state(zeta, g)
+    want = (a[-1] ** 2 / 4) / (1.0 / 8 + (a ** 2).sum() / 4)
+    assert abs(o.truncation_ratio() - want) <= 1e-15
+    # two species: the last moment of EACH species counts
+    o2 = Oracle(nx, ny, nz, M=2, nspecies=2)
+    o2.set_state(zeta, g)                      # g+ = (a0, a1), g- = (a2, a3)
+    want2 = ((a[1] ** 2 + a[3] ** 2) / 4) / (1.0 / 8 + (a ** 2).sum() / 4)
+    assert abs(o2.truncation_ratio() - want2) <= 1e-15
