@@ -76,6 +76,13 @@ __device__ __forceinline__ bool mbar_try_wait(unsigned long long* bar, unsigned 
                : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
   return ok != 0;
 }
+// non-blocking probe of a phase: the result can be consumed much later, so its shared-memory round trip hides behind other work
+__device__ __forceinline__ bool mbar_test_wait(unsigned long long* bar, unsigned parity) {
+  unsigned ok;
+  asm volatile("{\n .reg .pred p;\n mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+               : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  return ok != 0;
+}
 // try_wait is the suspending form: the hardware parks the thread for a bounded time before it returns false, so the
 // retry loop does not burn issue slots.  -DGD_DEBUG_MBAR builds trap after ~2^26 retries (a faulted bulk copy then
 // surfaces as a launch error instead of hanging the stream).

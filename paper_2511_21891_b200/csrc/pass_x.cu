@@ -28,6 +28,11 @@
 #define GD_X_QRTM 1       // 1: the Hermite sliding-window state (Q_{m-1}, the running R_m) lives in tensor memory next to the Phi/Psi lines
                           // (one 16-word record per x-point) instead of 64 registers per lane: the transforms then run with ~190 registers
 #endif
+#ifndef GD_X_PROBE
+#define GD_X_PROBE 0      // 1: the full barrier of the NEXT inverse job's tile is probed (mbarrier.test_wait) right after the current tile was
+                          // packed and the answer consumed a whole transform later, to take the barrier round trip (6 % of the warp
+                          // samples) off the critical path.  Measured SLOWER (1.403 vs 1.389 ms at 4a, 1.228 vs 1.217 at 4b): kept as an option
+#endif
 #ifndef GD_X_ALT
 #define GD_X_ALT 0        // 1: nx = 256 on one WARP per line (plan 8*8*4, 8 points per lane, 16 warps per SM).  Measured SLOWER (1.72 vs 1.40 ms at 4a:
                           // the second exchange costs more than the extra warps hide; bare transform 1.35 vs 2.53 G/s) -- kept as a tested option
@@ -183,6 +188,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, XGeom<NX>::CTAS) k_xpass(D
   auto src_array = [&](int kind) { return kind == 0 ? 0 : kind == 1 ? 2 : kind == 2 ? 6 : kind == 3 ? 4 : 8 + 2 * (kind - 4); };
   const int nkinds = 4 + M;
   double gmax = 0.0;
+  bool tile_ready = false;         // the next inverse job's tile was already seen complete (GD_X_PROBE)
   cd twr[X::NTWR > 0 ? X::NTWR : 1];
   if constexpr (X::NTWR > 0) fft_load_stage1_twiddles<FID, X::NTWR>(twr, t, tws);
 #if GD_X_STAGGER_NS > 0
@@ -241,7 +247,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, XGeom<NX>::CTAS) k_xpass(D
         // V = (df/dy)~ - kx f~, so that Z(kx) = i U(kx) and Z(-kx) = i conj(V(kx)) (Hermitian completion) need no arithmetic
         const int g = g0 + kind;
         const int sc = g % X::NST;
-        mbar_wait(&s_full[sc], (unsigned)((g / X::NST) & 1));
+        if (!tile_ready) mbar_wait(&s_full[sc], (unsigned)((g / X::NST) & 1));
         const cd* pU = stages + (size_t)sc * X::STAGE;            // element n of this line: pU[n * LD + (grp ^ (n & (LD-1)))]
         const cd* pV = pU + (size_t)KX * X::LD;
 #pragma unroll
@@ -260,6 +266,10 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, XGeom<NX>::CTAS) k_xpass(D
         }
         __syncwarp();                   // every lane of the warp has consumed the stage
         if ((threadIdx.x & 31) == 0) mbar_arrive(&s_empty[sc]);
+#if GD_X_PROBE
+        // (this warp has seen the previous use of that stage complete, so the parity test cannot alias)
+        tile_ready = mbar_test_wait(&s_full[(g + 1) % X::NST], (unsigned)(((g + 1) / X::NST) & 1));
+#endif
         if (warp == 0) {
           const int kn = kind + X::NST - 1;                     // job NST-1 ahead: of this block, or of the CTA's next one
           if (kn < nkinds) produce(g0 + kn, src_array(kn), blk);
