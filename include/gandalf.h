@@ -102,7 +102,9 @@ int gandalf_destroy(gandalf_ctx* ctx);
  * kept iff 3|n| <= N on every axis), zeroes kperp = 0 for zeta, and replaces
  * the kx = 0 plane by (a(0,ky,kz) + conj a(0,-ky,-kz))/2 so the real-space field is real.
  * It also resets time, step counter and energy history.  gandalf_get_state returns the current
- * (projected) state with zeros at removed modes. */
+ * (projected) state with zeros at removed modes.
+ * With HOST pointers only the retained modes of large inputs cross PCIe (30 % of the array: four pitched sub-block copies per
+ * field; the entries Eq. 20 removes are never read). */
 int gandalf_set_state(gandalf_ctx* ctx, const double* zeta_hat, const double* g_hat, int on_device);
 int gandalf_get_state(gandalf_ctx* ctx, double* zeta_hat, double* g_hat, int on_device);
 
@@ -190,6 +192,10 @@ int gandalf_energy_history(gandalf_ctx* ctx, int max_records, double* t_and_E, i
 
 /* Simulation time, number of completed steps and the last dt used (host output, synchronises). */
 int gandalf_get_time(gandalf_ctx* ctx, double* t, long long* step, double* last_dt);
+
+/* Bytes the host-pointer entry points of this context have copied host -> device and device -> host so far (state, RHS, energy
+ * and history transfers); bench.py's e2e.h2d_bytes_per_step / d2h_bytes_per_step are differences of these counters. */
+int gandalf_transfer_bytes(const gandalf_ctx* ctx, long long* h2d, long long* d2h);
 
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 long long gandalf_launch_count(const gandalf_ctx* ctx);

@@ -71,6 +71,7 @@ struct gandalf_ctx {
   bool stage_pending, need_h;                // between gandalf_step_stage(.., 0) and (.., 1); whether this step keeps the hybrid copy
   int num_sms;
   long long launches;
+  long long h2d_bytes, d2h_bytes;            // bytes the host-pointer entry points moved over PCIe so far (gandalf_transfer_bytes)
   bool timing;
   struct Ev { cudaEvent_t a, b; int cls; };
   std::vector<Ev> evs;
@@ -359,6 +360,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   if (e != cudaSuccess) { cudaGetLastError(); free_all(c); delete c; return GANDALF_ERR_CUDA; }
   c->step = 0; c->hist_base = 0; c->H_valid = true; c->launches = 0; c->timing = false;
   c->stage_pending = false; c->need_h = true;
+  c->h2d_bytes = 0; c->d2h_bytes = 0;
   for (int i = 0; i < KC_N; ++i) { c->t_ms[i] = 0; c->t_n[i] = 0; }
   *out = c;
   return GANDALF_OK;
@@ -384,6 +386,37 @@ static int ensure_io(gandalf_ctx* c, size_t bytes) {
   if (c->io) { GD_CUDA(c, cudaStreamSynchronize(c->st)); cudaFree(c->io); c->io = nullptr; c->io_bytes = 0; }
   GD_CUDA(c, cudaMalloc((void**)&c->io, bytes));
   c->io_bytes = bytes;
+  return GANDALF_OK;
+}
+
+// Host -> device copy of `nfields` boundary-layout fields.  gandalf_set_state reads only the RETAINED modes of its input (Eq. 20:
+// kx <= nx/3 and the two retained ranges of ky and of kz: 30 % of the half-plane array), so for large arrays only those
+// sub-blocks cross PCIe: four pitched 3-D copies per field into the same layout on the device (the rest of the staging buffer is
+// never read).  Small arrays go in one piece (fewer calls).
+static int copy_boundary_h2d(gandalf_ctx* c, cd* dst, const cd* src, int nfields) {
+  const Dims& d = c->d;
+  const size_t hp = (size_t)d.nz * d.ny * d.hx;
+  if ((size_t)nfields * hp * sizeof(cd) < ((size_t)64 << 20)) {
+    GD_CUDA(c, cudaMemcpyAsync(dst, src, (size_t)nfields * hp * sizeof(cd), cudaMemcpyHostToDevice, c->st));
+    c->h2d_bytes += (long long)((size_t)nfields * hp * sizeof(cd));
+    return GANDALF_OK;
+  }
+  const int zr[2][2] = {{0, d.hz3 + 1}, {d.nz - d.hz3, d.hz3}}, yr[2][2] = {{0, d.hy3 + 1}, {d.ny - d.hy3, d.hy3}};   // {start, count}
+  for (int f = 0; f < nfields; ++f)
+    for (int a = 0; a < 2; ++a)
+      for (int b = 0; b < 2; ++b) {
+        if (zr[a][1] <= 0 || yr[b][1] <= 0) continue;
+        cudaMemcpy3DParms p3;
+        std::memset(&p3, 0, sizeof(p3));
+        p3.srcPtr = make_cudaPitchedPtr(const_cast<cd*>(src), (size_t)d.hx * sizeof(cd), (size_t)d.hx * sizeof(cd), (size_t)d.ny);
+        p3.dstPtr = make_cudaPitchedPtr(dst, (size_t)d.hx * sizeof(cd), (size_t)d.hx * sizeof(cd), (size_t)d.ny);
+        p3.srcPos = make_cudaPos(0, (size_t)yr[b][0], (size_t)f * d.nz + zr[a][0]);
+        p3.dstPos = p3.srcPos;
+        p3.extent = make_cudaExtent((size_t)d.Kx * sizeof(cd), (size_t)yr[b][1], (size_t)zr[a][1]);
+        p3.kind = cudaMemcpyHostToDevice;
+        GD_CUDA(c, cudaMemcpy3DAsync(&p3, c->st));
+        c->h2d_bytes += (long long)((size_t)d.Kx * sizeof(cd) * yr[b][1] * zr[a][1]);
+      }
   return GANDALF_OK;
 }
 
@@ -453,7 +486,7 @@ int gandalf_get_state_raw(gandalf_ctx* c, double* out, int on_device) {
   GD_CUDA(c, cudaSetDevice(c->p.device));
   const size_t bytes = (size_t)c->d.F * c->d.PS * sizeof(cd);
   GD_CUDA(c, cudaMemcpyAsync(out, c->S0, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->st));
-  if (!on_device) GD_CUDA(c, cudaStreamSynchronize(c->st));
+  if (!on_device) { c->d2h_bytes += (long long)bytes; GD_CUDA(c, cudaStreamSynchronize(c->st)); }
   return GANDALF_OK;
 }
 
@@ -463,6 +496,7 @@ int gandalf_set_state_raw(gandalf_ctx* c, const double* in, int on_device) {
   GD_CUDA(c, cudaSetDevice(c->p.device));
   const size_t bytes = (size_t)c->d.F * c->d.PS * sizeof(cd);
   GD_CUDA(c, cudaMemcpyAsync(c->S0, in, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->st));
+  if (!on_device) c->h2d_bytes += (long long)bytes;
   c->stage_pending = false;
   int rc = make_hybrid(c, c->S0);
   if (rc) return rc;
@@ -492,8 +526,9 @@ int gandalf_set_state(gandalf_ctx* c, const double* zeta_hat, const double* g_ha
   if (!on_device) {
     int rc = ensure_io(c, (size_t)d.F * hp * sizeof(cd));
     if (rc) return rc;
-    GD_CUDA(c, cudaMemcpyAsync(c->io, zeta_hat, 2 * hp * sizeof(cd), cudaMemcpyHostToDevice, c->st));
-    if (d.M > 0) GD_CUDA(c, cudaMemcpyAsync(c->io + 2 * hp, g_hat, (size_t)d.M * hp * sizeof(cd), cudaMemcpyHostToDevice, c->st));
+    rc = copy_boundary_h2d(c, c->io, zin, 2);
+    if (rc) return rc;
+    if (d.M > 0) { rc = copy_boundary_h2d(c, c->io + 2 * hp, gin, d.M); if (rc) return rc; }
     zin = c->io; gin = c->io + 2 * hp;
   }
   GD_CUDA(c, timed(c, -1, 1, [&] { return launch_pack(d, zin, c->S0, 2, 2, c->st); }));
@@ -522,6 +557,7 @@ static int export_fields(gandalf_ctx* c, const cd* S, double* a2, double* aM, in
   if (!on_device) {
     GD_CUDA(c, cudaMemcpyAsync(a2, o2, 2 * hp * sizeof(cd), cudaMemcpyDeviceToHost, c->st));
     if (d.M > 0) GD_CUDA(c, cudaMemcpyAsync(aM, oM, (size_t)d.M * hp * sizeof(cd), cudaMemcpyDeviceToHost, c->st));
+    c->d2h_bytes += (long long)((size_t)d.F * hp * sizeof(cd));
     GD_CUDA(c, cudaStreamSynchronize(c->st));
   }
   return GANDALF_OK;
@@ -680,6 +716,7 @@ int gandalf_energy(gandalf_ctx* c, double out[6]) {
   GD_CUDA(c, timed(c, -1, 2, [&] { return launch_energy(c->d, c->S0, c->partial, kEnergyBlocks, c->rec_scratch, c->scal, 0, c->st); }));
   double rec[7];
   GD_CUDA(c, cudaMemcpyAsync(rec, c->rec_scratch, sizeof(rec), cudaMemcpyDeviceToHost, c->st));
+  c->d2h_bytes += (long long)sizeof(rec);
   GD_CUDA(c, cudaStreamSynchronize(c->st));
   bool ok = true;
   for (int i = 0; i < 6; ++i) { out[i] = rec[i + 1]; ok = ok && std::isfinite(out[i]); }
@@ -757,6 +794,7 @@ int gandalf_energy_history(gandalf_ctx* c, int max_records, double* t_and_E, int
   const long long have = c->step - c->hist_base;
   const long long k = have < max_records ? have : max_records;
   if (k > 0) GD_CUDA(c, cudaMemcpyAsync(t_and_E, c->hist, (size_t)k * 7 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+  c->d2h_bytes += (long long)(k * 7 * sizeof(double));
   GD_CUDA(c, cudaStreamSynchronize(c->st));
   *n = (int)k;
   for (long long i = 0; i < k * 7; ++i)
@@ -775,6 +813,13 @@ int gandalf_get_time(gandalf_ctx* c, double* t, long long* step, double* last_dt
   if (last_dt) *last_dt = s[SC_LASTDT];
   if (!std::isfinite(s[SC_T])) GD_FAIL(c, GANDALF_ERR_NONFINITE, "non-finite time (CFL dt)");
   if (s[SC_ERR] != 0.0) GD_FAIL(c, GANDALF_ERR_CFL, "CFL step (Eq. 16): max|grad Phi| is zero and dt_max is not set; the state was left untouched");
+  return GANDALF_OK;
+}
+
+int gandalf_transfer_bytes(const gandalf_ctx* c, long long* h2d, long long* d2h) {
+  if (!c) return GANDALF_ERR_INVALID;
+  if (h2d) *h2d = c->h2d_bytes;
+  if (d2h) *d2h = c->d2h_bytes;
   return GANDALF_OK;
 }
 

@@ -82,6 +82,7 @@ def load_library():
     lib.gandalf_halo_refresh.argtypes = [V, I]
     lib.gandalf_energy_history.argtypes = [V, I, PD, C.POINTER(I)]
     lib.gandalf_get_time.argtypes = [V, PD, C.POINTER(C.c_longlong), PD]
+    lib.gandalf_transfer_bytes.argtypes = [V, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     lib.gandalf_launch_count.argtypes = [V]
     lib.gandalf_launch_count.restype = C.c_longlong
     lib.gandalf_kernel_timing.argtypes = [V, I]
@@ -247,6 +248,12 @@ class Gandalf:
 
     def halo_refresh(self, state):
         self._ck(self._lib.gandalf_halo_refresh(self._h, int(state)))
+
+    def transfer_bytes(self):
+        """(host -> device, device -> host) bytes moved by the host-pointer entry points so far."""
+        a, b = C.c_longlong(), C.c_longlong()
+        self._ck(self._lib.gandalf_transfer_bytes(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def energy(self):
         out = np.zeros(6)
