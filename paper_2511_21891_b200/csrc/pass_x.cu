@@ -33,6 +33,14 @@
                           // packed and the answer consumed a whole transform later, to take the barrier round trip (6 % of the warp
                           // samples) off the critical path.  Measured SLOWER (1.403 vs 1.389 ms at 4a, 1.228 vs 1.217 at 4b): kept as an option
 #endif
+#ifndef GD_X_TMPIPE
+#define GD_X_TMPIPE 0     // moment products (QRTM): 0 = batches of four records, load - wait - compute; B > 0 = batches of B records software-
+                          // pipelined (the next batch's tcgen05.ld is issued before the current batch is computed), 1 also with the first
+                          // batch requested BEFORE the transform of g_m (the records do not depend on it)
+#endif
+#ifndef GD_X_TMHOIST
+#define GD_X_TMHOIST 0
+#endif
 #ifndef GD_X_ALT
 #define GD_X_ALT 0        // 1: nx = 256 on one WARP per line (plan 8*8*4, 8 points per lane, 16 warps per SM).  Measured SLOWER (1.72 vs 1.40 ms at 4a:
                           // the second exchange costs more than the extra warps hide; bare transform 1.35 vs 2.53 G/s) -- kept as a tested option
@@ -189,6 +197,8 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, XGeom<NX>::CTAS) k_xpass(D
   const int nkinds = 4 + M;
   double gmax = 0.0;
   bool tile_ready = false;         // the next inverse job's tile was already seen complete (GD_X_PROBE)
+  TmRaw16 pre[GD_X_TMPIPE > 0 ? GD_X_TMPIPE : 1];   // prefetched records of the moment products (GD_X_TMPIPE)
+  bool hoisted = false;
   cd twr[X::NTWR > 0 ? X::NTWR : 1];
   if constexpr (X::NTWR > 0) fft_load_stage1_twiddles<FID, X::NTWR>(twr, t, tws);
 #if GD_X_STAGGER_NS > 0
@@ -278,6 +288,14 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, XGeom<NX>::CTAS) k_xpass(D
       }
     }
 
+#if GD_X_TMPIPE > 0 && GD_X_TMHOIST
+    if (QRTM && !fwd && kind >= 4) {       // the first records of this moment's products: requested now, they arrive during the transform
+      tm_wait_st();
+#pragma unroll
+      for (int jj = 0; jj < GD_X_TMPIPE; ++jj) tm_ld16(tm + PSTR * jj, pre[jj]);
+      hoisted = true;
+    }
+#endif
     if constexpr (X::SPLITX && X::NTWR > 0) fft_lanes_fwd_rt_split<FID, X::NTWR>(v, t, reinterpret_cast<double*>(buf), tws, twr);
     else if constexpr (X::SPLITX) fft_lanes_split<FID, -1>(v, t, reinterpret_cast<double*>(buf), tws);
     else if constexpr (X::NTWR > 0) fft_lanes_fwd_rt<FID, X::NTWR>(v, t, buf, tws, twr);
@@ -373,7 +391,37 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, XGeom<NX>::CTAS) k_xpass(D
       const double upp = (m > 0) ? cup[m - 1] : 0.0;
       const bool emit = (m >= 1) && (((m - 1) & 1) == 1);     // R_{m-1} completes the pair (R_{m-2}, R_{m-1})
       tm_wait_st();
-      if constexpr (QRTM) {
+      if constexpr (QRTM && GD_X_TMPIPE > 0) {
+        constexpr int B = GD_X_TMPIPE;
+        if (!(GD_X_TMHOIST && hoisted)) {
+#pragma unroll
+          for (int jj = 0; jj < B; ++jj) tm_ld16(tm + PSTR * jj, pre[jj]);
+        }
+        hoisted = false;
+#pragma unroll
+        for (int q0 = 0; q0 < E; q0 += B) {
+          TmRaw16 r[B];
+          tm_wait_ld();
+#pragma unroll
+          for (int jj = 0; jj < B; ++jj) r[jj] = pre[jj];
+          if (q0 + B < E) {
+#pragma unroll
+            for (int jj = 0; jj < B; ++jj) tm_ld16(tm + PSTR * (q0 + B + jj), pre[jj]);
+          }
+#pragma unroll
+          for (int jj = 0; jj < B; ++jj) {
+            const int q = q0 + jj;
+            const double phx = tm_d(r[jj].w), phy = tm_d(r[jj].w + 2), psx = tm_d(r[jj].w + 4), psy = tm_d(r[jj].w + 6);
+            const double ra = tm_d(r[jj].w + 8), rd = tm_d(r[jj].w + 10), qp = tm_d(r[jj].w + 12);
+            const double gx = v[q].x, gy = -v[q].y;
+            const double P = phx * gy - phy * gx;               // {Phi, g_m}
+            const double Q = psx * gy - psy * gx;               // {Psi, g_m}
+            const double rfin = ra + upp * Q;                   // R_{m-1} complete
+            if (emit) v[q] = cmake(rd, rfin);
+            tm_st8(tm + PSTR * q + 8, dn * qp - P, rfin, Q, 0.0);
+          }
+        }
+      } else if constexpr (QRTM) {
 #pragma unroll
         for (int q0 = 0; q0 < E; q0 += 4) {
           TmRaw16 r[4];
