@@ -193,12 +193,13 @@ def cpu_baseline_sample(name, full_shape, full_rhs=False):
     nthreads = oracle.num_threads()
     nz_s = min(ORACLE_SLAB_NZ, full_shape[2])
     o, prm, run = _oracle_slab(name, nz_s)
+    o.step(run["dt"], 1)                  # one untimed step first, as the reference arm does (page faults, thread start-up)
     t0 = time.perf_counter()
     o.step(run["dt"], 1)
     el = time.perf_counter() - t0
     frac = nz_s / full_shape[2]
     out = {"value": 2.0 / el * frac, "unit": "RHS evals/s", "cores": nthreads, "kind": "oracle", "seconds": el,
-           "sample": f"one full Algorithm-2 step (2 RHS) on a {run['shape'][0]}x{run['shape'][1]}x{nz_s} z-slab of the "
+           "sample": f"one full Algorithm-2 step (2 RHS; after one untimed step) on a {run['shape'][0]}x{run['shape'][1]}x{nz_s} z-slab of the "
                      f"workload, all moments; rate scaled by {nz_s}/{full_shape[2]} to the full grid"}
     del o
     nz_1 = min(2, full_shape[2])

@@ -83,6 +83,36 @@ def test_config2_krmhd_hermite():
     _check_history(o, g)
 
 
+def test_config2_all_200_steps_against_the_oracle_written_golden():
+    """BASELINE config 2 AS SPECIFIED (64x64x32, M = 16, dt = 5e-4, all 200 steps): energy record every 10th step (1e-9) and 48
+    sampled coefficients of the final state against tests/golden/config2_history_oracle.txt, which
+    tests/golden/make_config2_history.py wrote from the oracle alone (six minutes of CPU: too slow to repeat in the test)."""
+    import os
+    from paper_2511_21891_b200.gandalf import Gandalf
+    prm, z, gm, run = config2()
+    g = Gandalf(*run["shape"], **prm)
+    g.set_state(z, gm)
+    g.step(run["dt"], run["steps"])
+    hist = g.energy_history()
+    zeta, gg = g.get_state()
+    allf = np.concatenate([zeta, gg])
+    nH = nS = 0
+    for ln in open(os.path.join(os.path.dirname(__file__), "golden", "config2_history_oracle.txt")):
+        if ln.startswith("H "):
+            t = ln.split()
+            step, want = int(t[1]), np.array([float(x) for x in t[2:]])
+            got = hist[step - 1]
+            assert abs(got[0] - want[0]) <= 1e-12 and np.abs(got[1:] - want[1:]).max() <= 1e-9 * max(1.0, np.abs(want[1:]).max()), step
+            nH += 1
+        elif ln.startswith("S "):
+            t = ln.split()
+            f, iz, iy, ix = (int(x) for x in t[1:5])
+            want = complex(float(t[5]), float(t[6]))
+            assert abs(allf[f, iz, iy, ix] - want) <= 1e-9 * np.abs(allf[f]).max(), (f, iz, iy, ix)
+            nS += 1
+    assert nH == 20 and nS == 48 and hist.shape[0] == 200
+
+
 @pytest.mark.parametrize("shape,M", [((8, 8, 2), 0), ((16, 8, 4), 1), ((8, 16, 8), 2), ((32, 64, 16), 3),
                                      ((64, 32, 8), 5), ((128, 16, 4), 2), ((16, 128, 4), 2), ((256, 8, 2), 1),
                                      ((8, 256, 2), 1), ((512, 8, 2), 1), ((8, 512, 2), 2), ((8, 8, 64), 2),
