@@ -245,7 +245,10 @@ template <int NY> struct YGeom {
   using G = FftGeom<NY>;
   static constexpr int T = G::T, E = G::E;
   // ny = 512 (one warp per transform): 12 warps = 12 columns with 170 registers per lane (no spills)
-  static constexpr int THREADS = (T >= 32) ? 384 : 256;
+#ifndef GD_Y512_THREADS
+#define GD_Y512_THREADS 384
+#endif
+  static constexpr int THREADS = (T >= 32) ? GD_Y512_THREADS : 256;
   static constexpr int CTAS = (THREADS > 256) ? 1 : 2;       // resident CTAs per SM
   static constexpr int GROUPS = THREADS / T;                 // columns per CTA
 };
