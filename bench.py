@@ -332,6 +332,31 @@ def run_microbench(device=0, which=(0, 1, 2, 3)):
     return out
 
 
+def run_planes_sweep(device=0, planes=(2, 4, 8, 16, 32, 128)):
+    """What z-batching the P1 -> P2 -> P3 chain to keep its intermediates in L2 would have to beat: the same
+    kernels on 256x256xnz grids with all 34 fields.  D + E are 37.6 MB per plane, so nz = 2 is L2-resident and nz >= 8 is not."""
+    import torch
+    from paper_2511_21891_b200.gandalf import Gandalf, KERNEL_CLASSES
+    from paper_2511_21891_b200 import workloads
+    out = {"what": "ms per launch of each pass kernel at 256x256xnz, M = 32, scaled by 128/nz", "D_plus_E_MB_per_plane": 37.6, "rows": {}}
+    for nz in planes:
+        prm, z, g, run = workloads.config4a(nz=nz)
+        stream = torch.cuda.Stream(device=device)
+        sim = Gandalf(*run["shape"], device=device, stream=stream.cuda_stream, **prm)
+        with torch.cuda.stream(stream):
+            sim.set_state(torch.from_numpy(z).cuda(device), torch.from_numpy(g).cuda(device))
+            sim.step(run["dt"], 5)
+        torch.cuda.synchronize()
+        sim.kernel_timing(True)
+        with torch.cuda.stream(stream):
+            sim.step(run["dt"], 20)
+        torch.cuda.synchronize()
+        kt = sim.kernel_times()
+        out["rows"][str(nz)] = {k: round(kt[k][0] / nz * 128, 4) for k in KERNEL_CLASSES if kt[k][1]}
+        sim.close()
+    return out
+
+
 def run_mshard(args, rank, world, local):
     """ONE run of the workload sharded by Hermite moment over the ranks (strong scaling): xi+- replicated, one halo moment per
     neighbour exchanged twice per step with NCCL point-to-point copies in place on the library's buffers (sharded.py)."""
@@ -422,6 +447,9 @@ def main():
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "mshard"],
                     help="N > 1: independent replicas (default; north_star keeps the product on one GPU) or ONE run sharded by Hermite "
                          "moment with halo exchange over NCCL (paper_2511_21891_b200/sharded.py, DESIGN.md Q31)")
+    ap.add_argument("--planes-sweep", action="store_true",
+                    help="time the four pass kernels of config 4(a) restricted to nz = 2, 4, ... planes (working set of the P1->P2->P3 "
+                         "intermediates from inside the 126 MB L2 to far outside it) and print ms per launch scaled to 128 planes")
     ap.add_argument("--emulate-ranks", type=int, default=0, help="mshard on ONE GPU: emulate this many ranks in one process (checks the path; not a scaling number)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -433,6 +461,10 @@ def main():
     if args.microbench:
         if rank == 0:
             print(json.dumps(run_microbench(local)), flush=True)
+        return
+    if args.planes_sweep:
+        if rank == 0:
+            print(json.dumps(run_planes_sweep(local)), flush=True)
         return
     if args.warmup < 3:
         args.warmup = 3
