@@ -161,7 +161,10 @@ int gandalf_halo_refresh(gandalf_ctx* ctx, int state);
 /* Energies of the current state (host output, synchronises):
  * out = { E_A, E_plus, E_minus, E_kin, E_mag, W_g } with E_+- = 1/4 sum_k kperp^2 |xi+-|^2,
  * E_A = E_plus + E_minus, E_kin = 1/2 sum kperp^2 |Phi|^2, E_mag = 1/2 sum kperp^2 |Psi|^2,
- * W_g = 1/2 sum_m sum_k |g_m|^2, sums over the full spectrum [PAPER.md:115, 383, 442; Q14]. */
+ * W_g = 1/2 sum_m sum_k |g_m|^2, sums over the full spectrum [PAPER.md:115, 383, 442; Q14].
+ * The other two diagnostics PAPER.md:383 names follow from these without another pass over the state: cross-helicity
+ * H_c = E_plus - E_minus, residual energy E_r = E_kin - E_mag (the paper gives no formulas; these are the standard Elsasser
+ * definitions, Schekochihin et al. 2009, which PAPER.md:115 refers to). */
 int gandalf_energy(gandalf_ctx* ctx, double out[6]);
 
 /* Perpendicular shell spectrum [Eq. 26; Q15]: bin j = floor(kperp/dk + 1/2),
