@@ -141,3 +141,29 @@ def test_config4b_full_size_rhs_and_step_vs_small_grid_oracle():
     assert _full_rel_l2(z_in, zo, z_rn) <= 1e-10, _full_rel_l2(z_in, zo, z_rn)
     hg, ho = g.energy_history(), o.energy_history()
     assert np.abs(hg[:, 1:] - ho[:, 1:]).max() <= 1e-9 * np.abs(ho[:, 1:]).max()
+
+
+@pytest.mark.parametrize("workload", ["4a", "4b"])
+def test_full_size_runs_are_bit_reproducible(workload):
+    """Race check at the bench sizes (compute-sanitizer is closed on this pool): two runs of 60 steps of BASELINE config 4(a) /
+    4(b), dense state, in the launch configuration bench.py times, must agree bit for bit on the raw state and on the energy
+    history -- every TMA / mbarrier / tensor-memory pipeline, persistent item loop and fixed-order reduction included."""
+    import torch
+    from paper_2511_21891_b200.gandalf import Gandalf
+    from paper_2511_21891_b200.workloads import config4b
+    if workload == "4a":
+        prm, z, g, run = config4a()
+        g = synth.dense_random(*run["shape"], 32, seed=77, decay=3.0) * 1e-2
+    else:
+        prm, z, g, run = config4b()
+        g = None
+    z = synth.dense_random(*run["shape"], 2, seed=78, decay=3.0)
+    outs = []
+    for _ in range(2):
+        sim = Gandalf(*run["shape"], **prm)
+        sim.set_state(z, g)
+        sim.step(run["dt"], 60)
+        outs.append((sim.get_state_raw(device=True).clone(), sim.energy_history().copy()))
+        sim.close()
+    assert np.isfinite(outs[0][1]).all()
+    assert torch.equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
