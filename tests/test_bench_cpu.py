@@ -54,3 +54,22 @@ def test_reference_arm_under_torchrun_two_ranks():
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_algorithmic_bytes_match_the_survey_table():
+    """bench.py's roofline numerators are SURVEY.md 8(d)'s formulas: 30.6 GB per step at config 4(a), 19.1 GB at 4(b), and the
+    per-pass figures P1 8.5, P2 9.6, P3 5.1, P4 7.4 GB per step (two launches each)."""
+    import bench
+    per, step = bench.algorithmic_bytes((256, 256, 128), 32)
+    assert abs(step / 1e9 - 30.63) < 0.01
+    assert abs(2 * per["y_inverse_P1"] / 1e9 - 8.54) < 0.01 and abs(2 * per["x_pass_P2"] / 1e9 - 9.56) < 0.01
+    assert abs(2 * per["y_forward_P3"] / 1e9 - 5.11) < 0.01 and abs(2 * per["z_step_P4"] / 1e9 - 7.42) < 0.01
+    _, step_b = bench.algorithmic_bytes((512, 512, 256), 0)
+    assert abs(step_b / 1e9 - 19.12) < 0.01
+
+
+def test_moment_shard_layouts_used_by_the_bench():
+    from paper_2511_21891_b200 import sharded
+    lays = [sharded.ShardLayout.make(32, 4, r) for r in range(4)]
+    assert [lay.hi - lay.lo for lay in lays] == [8, 8, 8, 8] and [lay.M_local for lay in lays] == [9, 10, 10, 9]
+    assert lays[1].params() == dict(M=10, m_offset=7, M_global=32) and sharded.ShardLayout.make(32, 1, 0).params() == dict(M=32)
