@@ -8,8 +8,9 @@
 //   k_yfwd(_pair): P3.  E -> Gh: forward c2c along y, ky part of Eq. 20; the Elsasser pair is assembled as
 //                 N+- = -1/2 A -+ 1/2 kperp^2 B  (Eq. 1 with Eq. 11)
 // Every FFT is the lane-group transform of fft.cuh: T lanes of one warp per column, data in registers, one
-// shared-memory exchange per stage boundary.  The y passes stage their input tiles with bulk async copies (TMA engine,
-// mbarrier completion) so that global memory sees whole row segments; see DESIGN.md section 5.
+// shared-memory exchange per stage boundary.  The y passes stage their input tiles with per-row bulk async copies (TMA engine,
+// mbarrier completion) so that global memory sees whole 256-byte row segments; P4 moves its tiles with tensor-map TMA
+// (cp.async.bulk.tensor, one instruction per 8-column sub-tile, 128-byte swizzle; common.cuh); see DESIGN.md section 5.
 #include <vector>
 #include "common.cuh"
 
