@@ -30,6 +30,8 @@ WORKLOADS = {
     "4a": ("config4a", dict(nx=256, ny=256, nz=128, M=32)),
     "4a2": ("config4a", dict(nx=256, ny=256, nz=128, M=32, nspecies=2)),     # both species: 2 + 64 fields
     "4b": ("config4b", dict(nx=512, ny=512, nz=256)),
+    "0": ("config0", dict(nx=32, ny=32, nz=16)),          # the small configurations are launch-bound: they time the step's launch path
+    "1": ("config1", dict(n=128)),
     "2": ("config2", dict(nx=64, ny=64, nz=32, M=16)),
     # driven turbulence; e.g. --steps 79990 --warmup 10 reaches the statistically steady state (t ~ 17).  cfl = 0.03, not
     # BASELINE's 0.3: with C = 0.3 on max|grad Phi| alone (Eq. 16) the explicit RK2 of the Hermite couplings
@@ -44,6 +46,8 @@ def make_workload(name, **override):
     fn, kw = WORKLOADS[name]
     kw = dict(kw)
     kw.update(override)
+    if name == "1":
+        kw.pop("nz", None)      # Orszag-Tang is z-uniform on two planes: the oracle's sample is the whole workload
     prm, z, g, run = getattr(cases, fn)(**kw)
     if name == "3":
         prm = dict(prm, cfl=0.03)
@@ -154,7 +158,7 @@ def run_reference(args, rank, world):
     import oracle
     name = args.workload
     fn, kw = WORKLOADS[name]
-    full = (kw["nx"], kw["ny"], kw["nz"])
+    full = (kw["nx"], kw["ny"], kw["nz"]) if "nx" in kw else (kw["n"], kw["n"], 2)
     nz_s = min(ORACLE_SLAB_NZ, full[2])
     o, prm, run = _oracle_slab(name, nz_s)
     for _ in range(args.warmup):
@@ -442,6 +446,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cufft-compare", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="plain stream launches instead of the replayed CUDA graph of one step")
     ap.add_argument("--oracle-full-rhs", action="store_true", help="also time one oracle RHS evaluation at the FULL grid (slow, ~20 GB host memory at 4a)")
     ap.add_argument("--microbench", action="store_true", help="print the measured unit ceilings (gandalf_microbench) and exit")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "mshard"],
@@ -486,6 +491,8 @@ def main():
     F = 2 + M
     stream = torch.cuda.Stream()
     sim = Gandalf(*shape, device=local, stream=stream.cuda_stream, **prm)
+    if args.no_graph:
+        sim.graph_mode(False)
     # device-resident inputs for the device-timed number
     zd = torch.from_numpy(z).cuda()
     gd = torch.from_numpy(g).cuda() if M else None
@@ -510,6 +517,7 @@ def main():
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
     launches = sim.launch_count() - n0
+    graph_replays = sim.graph_mode()    # steps of the timed region replayed from the captured CUDA graph of one step (gandalf_graph_mode)
     ms = max_over_ranks(ms, world)
     # per-kernel CUDA-event times in a SECOND, untimed-for-the-headline pass (the events cost a little per launch)
     ksteps = min(args.steps, 10)
@@ -661,7 +669,8 @@ def main():
             "config": {"workload": wl, "grid": list(shape), "M": M, "dt": dt, "fields": F, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "no flush needed: every kernel streams inputs far larger than the 126 MB L2 (working set per step > 9 GB at 4a)"},
             "steps_per_s": steps_per_s, "grid_point_moments_per_s": steps_per_s * shape[0] * shape[1] * shape[2] * F,
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cufft_comparison": cufft, "kperp_spectrum": spectrum,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+            "launch_path": ("cuda graph of one step, replayed" if graph_replays else "plain stream launches"), "graph_replays": graph_replays, "roofline": roofline, "cpu_baseline": cpu, "cufft_comparison": cufft, "kperp_spectrum": spectrum,
             "final_energy": {"E_A": float(hist[-1, 1]), "W_g": float(hist[-1, 6])},
         }
         print(json.dumps(line), flush=True)

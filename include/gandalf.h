@@ -200,8 +200,17 @@ int gandalf_get_time(gandalf_ctx* ctx, double* t, long long* step, double* last_
  * and history transfers); bench.py's e2e.h2d_bytes_per_step / d2h_bytes_per_step are differences of these counters. */
 int gandalf_transfer_bytes(const gandalf_ctx* ctx, long long* h2d, long long* d2h);
 
-/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+/* Number of kernels this context has launched so far (bench.py's gpu_launches); kernels of a replayed graph count as launched. */
 long long gandalf_launch_count(const gandalf_ctx* ctx);
+
+/* Launch path of gandalf_step [Algorithm 2, is the same kernel sequence every step].  enable = 1 (the default):
+ * one step is captured into a CUDA graph the first time gandalf_step runs two or more steps (or is called a second time with the
+ * same dt) and replayed afterwards -- the launch-bound small grids (BASELINE configs 0-2) step faster, the results are bit for bit
+ * those of plain launches (same kernels, same arguments; dt, time and the step number live in device memory).  The graph is rebuilt
+ * when dt or the history buffer changes.  Plain launches are used on the legacy default stream (stream = NULL: capture is not allowed
+ * there), while per-kernel timing is on, and for gandalf_step_stage.  enable = 0: plain launches; enable = -1: query only.
+ * *replays (may be NULL) receives the number of graph launches made so far.  Returns GANDALF_ERR_INVALID for another enable. */
+int gandalf_graph_mode(gandalf_ctx* ctx, int enable, long long* replays);
 
 /* Event-timed average duration (ms) of one named kernel class since the last reset; used by
  * bench.py for the roofline line.  which: 0 z-inverse (set_state / after forcing only), 1 y-inverse (P1),

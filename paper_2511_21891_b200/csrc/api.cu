@@ -37,10 +37,10 @@ cudaError_t launch_zero_u64(unsigned long long* p, cudaStream_t st);
 cudaError_t launch_pack(const Dims& d, const cd* in, cd* S, int nfields, int nzeta, cudaStream_t st);
 cudaError_t launch_unpack(const Dims& d, const cd* S, cd* out, int nfields, int nzeta, cudaStream_t st);
 cudaError_t launch_forcing(const Dims& d, cd* S, const int* pairs, int npairs, double amp, unsigned long long seed,
-                           long long step, const double* scal, cudaStream_t st);
-cudaError_t launch_forcing_g(const Dims& d, cd* S, int nzf, double amp, unsigned long long seed, long long step,
+                           const double* scal, cudaStream_t st);
+cudaError_t launch_forcing_g(const Dims& d, cd* S, int nzf, double amp, unsigned long long seed,
                              const double* scal, cudaStream_t st);
-cudaError_t launch_energy(const Dims& d, const cd* S, double* partial, int nblocks, double* rec, double* scal, int advance,
+cudaError_t launch_energy(const Dims& d, const cd* S, double* partial, int nblocks, double* rec, long long hist_base, double* scal, int advance,
                           cudaStream_t st);
 cudaError_t launch_spectrum(const Dims& d, const cd* S, double* col, int nbins, int literal, double dk, double* out, cudaStream_t st);
 cudaError_t launch_hermite_spectrum(const Dims& d, const cd* S, double* out, cudaStream_t st);
@@ -73,6 +73,10 @@ struct gandalf_ctx {
   long long launches;
   long long h2d_bytes, d2h_bytes;            // bytes the host-pointer entry points moved over PCIe so far (gandalf_transfer_bytes)
   bool timing;
+  // CUDA graph of ONE step (gandalf_step with a fixed dt or the CFL dt; DESIGN.md section 5 "launch path"): captured from the very
+  // launches a plain step makes, replayed nsteps times.  Valid while the by-value launch arguments stay the same (key below).
+  int graph_mode;                            // 1 (default): replay a graph when the stream allows capture; 0: plain launches
+  cudaGraphExec_t gexec; double g_dt, g_last_dt; double* g_hist; long long g_hist_base; long long g_launches; long long graph_replays;
   struct Ev { cudaEvent_t a, b; int cls; };
   std::vector<Ev> evs;
   double t_ms[KC_N]; long long t_n[KC_N];
@@ -165,6 +169,7 @@ static void free_all(gandalf_ctx* c) {
                   c->collfac, c->scal, c->partial, c->hist, c->rec_scratch, c->spec_col, c->spec_out, c->maxbits,
                   c->pairs, c->io, c->hxV, c->hxLam, c->hxP};
   for (void* q : ptrs) if (q) cudaFree(q);
+  if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
   for (auto& e : c->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
 }
 
@@ -359,6 +364,7 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   }
   if (e != cudaSuccess) { cudaGetLastError(); free_all(c); delete c; return GANDALF_ERR_CUDA; }
   c->step = 0; c->hist_base = 0; c->H_valid = true; c->launches = 0; c->timing = false;
+  c->graph_mode = 1; c->gexec = nullptr; c->g_launches = 0; c->graph_replays = 0; c->g_last_dt = -1.0;
   c->stage_pending = false; c->need_h = true;
   c->h2d_bytes = 0; c->d2h_bytes = 0;
   for (int i = 0; i < KC_N; ++i) { c->t_ms[i] = 0; c->t_n[i] = 0; }
@@ -507,10 +513,12 @@ int gandalf_set_state_raw(gandalf_ctx* c, const double* in, int on_device) {
 
 int gandalf_set_time(gandalf_ctx* c, double t, long long step) {
   if (!c) return GANDALF_ERR_INVALID;
-  if (step < 0 || !std::isfinite(t)) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_set_time: bad time or step");
+  if (step < 0 || step > (1LL << 52) || !std::isfinite(t)) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_set_time: bad time or step");
   GD_CUDA(c, cudaSetDevice(c->p.device));
+  const double dstep = (double)step;
   GD_CUDA(c, cudaMemcpyAsync(c->scal + SC_T, &t, sizeof(double), cudaMemcpyHostToDevice, c->st));
-  GD_CUDA(c, cudaStreamSynchronize(c->st));     // t lives on this stack frame
+  GD_CUDA(c, cudaMemcpyAsync(c->scal + SC_STEP, &dstep, sizeof(double), cudaMemcpyHostToDevice, c->st));
+  GD_CUDA(c, cudaStreamSynchronize(c->st));     // t, dstep live on this stack frame
   c->step = step; c->hist_base = step;          // the history restarts at the resumed step
   return GANDALF_OK;
 }
@@ -636,20 +644,20 @@ static int step_stage1(gandalf_ctx* c) {
   }
   if (c->npairs) {
     GD_CUDA(c, timed(c, -1, 1, [&] {
-      return launch_forcing(d, c->S0, c->pairs, c->npairs, c->force_amp, c->p.seed, c->step, c->scal, c->st);
+      return launch_forcing(d, c->S0, c->pairs, c->npairs, c->force_amp, c->p.seed, c->scal, c->st);
     }));
     // the forcing touches w+- only: refresh the hybrid copy of those two fields
     if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0, c->H, c->twz, 2, c->st); }));
   }
   if (c->p.force_g_amp > 0.0 && c->p.m_offset == 0) {     // g_0 lives on the shard with m_offset = 0
     GD_CUDA(c, timed(c, -1, 1, [&] {
-      return launch_forcing_g(d, c->S0, c->p.force_g_nz, c->p.force_g_amp, c->p.seed, c->step, c->scal, c->st);
+      return launch_forcing_g(d, c->S0, c->p.force_g_nz, c->p.force_g_amp, c->p.seed, c->scal, c->st);
     }));
     // the forcing touches g_0 only: refresh the hybrid copy of that field
     if (need_h) GD_CUDA(c, timed(c, KC_ZINV, 1, [&] { return launch_zfft(d, c->S0 + 2 * d.PS, c->H + 2 * d.PH, c->twz, 1, c->st); }));
   }
   GD_CUDA(c, timed(c, -1, 2, [&] {
-    return launch_energy(d, c->S0, c->partial, kEnergyBlocks, c->hist + (size_t)(c->step - c->hist_base) * 7, c->scal, 1, c->st);
+    return launch_energy(d, c->S0, c->partial, kEnergyBlocks, c->hist, c->hist_base, c->scal, 1, c->st);   // slot (step - hist_base), step on the device
   }));
   c->step += 1;
   c->H_valid = need_h;
@@ -667,12 +675,56 @@ int gandalf_step(gandalf_ctx* c, double dt, int nsteps) {
   int rc = ensure_hist(c, c->step - c->hist_base + nsteps);
   if (rc) return rc;
   if (!c->H_valid) { rc = make_hybrid(c, c->S0); if (rc) return rc; c->H_valid = true; }
-  for (int i = 0; i < nsteps; ++i) {
+  int done = 0;
+  // Graph path: one step is the same launch sequence with the same arguments every time (dt and the step number are read from
+  // device memory), so it is captured once and replayed.  Not with per-kernel event timing, not on the legacy default stream
+  // (capture is not allowed there), not inside somebody else's capture.
+  if (c->graph_mode && !c->timing && c->st != nullptr && nsteps > 0) {
+    const double key_dt = dt > 0.0 ? dt : 0.0;
+    const bool cached = c->gexec && c->g_dt == key_dt && c->g_hist == c->hist && c->g_hist_base == c->hist_base;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    const bool want = !cached && (nsteps >= 2 || c->g_last_dt == key_dt) && cudaStreamIsCapturing(c->st, &cs) == cudaSuccess &&
+                      cs == cudaStreamCaptureStatusNone;
+    if (want && c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }   // before the capture begins (deferred until its replays end)
+    if (want && cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      const long long l0 = c->launches, s0 = c->step;
+      int rcc = step_stage0(c, dt);
+      if (!rcc) rcc = step_stage1(c);
+      cudaGraph_t g = nullptr;
+      cudaError_t e = cudaStreamEndCapture(c->st, &g);
+      const long long per_step = c->launches - l0;
+      c->launches = l0; c->step = s0; c->stage_pending = false; c->H_valid = true;   // nothing ran: the capture only recorded
+      if (!rcc && e == cudaSuccess && g && cudaGraphInstantiate(&c->gexec, g, 0) == cudaSuccess) {
+        c->g_dt = key_dt; c->g_hist = c->hist; c->g_hist_base = c->hist_base; c->g_launches = per_step;
+      } else {
+        c->gexec = nullptr;
+        cudaGetLastError();                        // a failed capture is not an error of the step: plain launches follow
+      }
+      if (g) cudaGraphDestroy(g);
+    }
+    if (c->gexec && c->g_dt == key_dt && c->g_hist == c->hist && c->g_hist_base == c->hist_base) {
+      for (; done < nsteps; ++done) {
+        GD_CUDA(c, cudaGraphLaunch(c->gexec, c->st));
+        c->step += 1; c->launches += c->g_launches; c->graph_replays += 1;
+      }
+      c->H_valid = c->p.nonlinear || !(dt > 0.0);   // what step_stage1 leaves (need_h)
+    }
+    c->g_last_dt = key_dt;                          // a second call with the same dt is worth a capture even with nsteps = 1
+  }
+  for (int i = done; i < nsteps; ++i) {
     rc = step_stage0(c, dt);
     if (rc) return rc;
     rc = step_stage1(c);
     if (rc) return rc;
   }
+  return GANDALF_OK;
+}
+
+int gandalf_graph_mode(gandalf_ctx* c, int enable, long long* replays) {
+  if (!c) return GANDALF_ERR_INVALID;
+  if (enable == 0 || enable == 1) c->graph_mode = enable;
+  else if (enable != -1) GD_FAIL(c, GANDALF_ERR_INVALID, "gandalf_graph_mode: enable must be 0, 1 or -1 (query)");
+  if (replays) *replays = c->graph_replays;
   return GANDALF_OK;
 }
 
@@ -713,7 +765,7 @@ int gandalf_halo_refresh(gandalf_ctx* c, int state) {
 int gandalf_energy(gandalf_ctx* c, double out[6]) {
   if (!c || !out) return GANDALF_ERR_INVALID;
   GD_CUDA(c, cudaSetDevice(c->p.device));
-  GD_CUDA(c, timed(c, -1, 2, [&] { return launch_energy(c->d, c->S0, c->partial, kEnergyBlocks, c->rec_scratch, c->scal, 0, c->st); }));
+  GD_CUDA(c, timed(c, -1, 2, [&] { return launch_energy(c->d, c->S0, c->partial, kEnergyBlocks, c->rec_scratch, 0, c->scal, 0, c->st); }));
   double rec[7];
   GD_CUDA(c, cudaMemcpyAsync(rec, c->rec_scratch, sizeof(rec), cudaMemcpyDeviceToHost, c->st));
   c->d2h_bytes += (long long)sizeof(rec);

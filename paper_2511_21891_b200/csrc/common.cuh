@@ -143,7 +143,9 @@ struct PhysParams {
 };
 
 // device scalars owned by the context
-enum { SC_DT = 0, SC_T = 1, SC_LASTDT = 2, SC_ERR = 3, SC_COUNT = 8 };   // SC_ERR != 0: Eq. 16 had no flow to bound dt (sticky)
+enum { SC_DT = 0, SC_T = 1, SC_LASTDT = 2, SC_ERR = 3, SC_STEP = 4, SC_COUNT = 8 };   // SC_ERR != 0: Eq. 16 had no flow to bound dt (sticky)
+// SC_STEP: the step number (an exact integer in a double), advanced on the device with the time so that a captured CUDA graph of
+// one step replays correctly: the forcing counters (Q17, Q26) and the slot of the energy record derive from it
 
 // Launch geometry of the z transforms: GD_Z_THREADS lanes per CTA = GD_Z_THREADS/T adjacent (cy,cx) columns.
 #define GD_Z_THREADS 128

@@ -123,9 +123,10 @@ __device__ __forceinline__ double rng_u01(unsigned long long seed, unsigned long
 }
 // pairs: int3 (nx >= 0, ny, nz) canonical members.  One thread per (field, pair).
 __global__ void k_forcing(Dims d, cd* __restrict__ S, const int* __restrict__ pairs, int npairs, double amp,
-                          unsigned long long seed, long long step, const double* __restrict__ scal) {
+                          unsigned long long seed, const double* __restrict__ scal) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= 2 * npairs) return;
+  const long long step = (long long)scal[SC_STEP];
   const int f = i / npairs, ip = i % npairs;
   const int nx_ = pairs[3 * ip], ny_ = pairs[3 * ip + 1], nz_ = pairs[3 * ip + 2];
   const unsigned long long base = (((unsigned long long)step * 2ULL + (unsigned long long)f) * (unsigned long long)npairs + (unsigned long long)ip) * 2ULL;
@@ -149,8 +150,9 @@ __global__ void k_forcing(Dims d, cd* __restrict__ S, const int* __restrict__ pa
 }
 
 // g_0 forcing of the velocity-space benchmark (Q26): one thread.
-__global__ void k_forcing_g(Dims d, cd* __restrict__ S, int nzf, double amp, unsigned long long seed, long long step,
+__global__ void k_forcing_g(Dims d, cd* __restrict__ S, int nzf, double amp, unsigned long long seed,
                             const double* __restrict__ scal) {
+  const long long step = (long long)scal[SC_STEP];
   const unsigned long long key = seed ^ 0xA5A5A5A5A5A5A5A5ULL;
   const double u1 = rng_u01(key, 2ULL * (unsigned long long)step), u2 = rng_u01(key, 2ULL * (unsigned long long)step + 1ULL);
   const double rad = sqrt(-2.0 * log(1.0 - u1));
@@ -208,8 +210,11 @@ __global__ void __launch_bounds__(256) k_energy_partial(Dims d, const cd* __rest
   }
 }
 // Final sum in a fixed order (deterministic): warp k sums quantity k, lane l takes blocks l, l+32, ... then a shuffle tree.
-// advance != 0: t += dt, and the record {t, E_A, E+, E-, Ekin, Emag, Wg} goes to rec.
-__global__ void __launch_bounds__(160) k_energy_final(const double* __restrict__ partial, int nblocks, double* __restrict__ rec, double* scal, int advance) {
+// advance == 0: the record {t, E_A, E+, E-, Ekin, Emag, Wg} goes to rec.  advance != 0: t += dt, rec is the energy HISTORY and the
+// record goes to its slot (step - hist_base), then the step number moves on -- all on the device, so that the launch has the same
+// arguments every step (CUDA graph replay).
+__global__ void __launch_bounds__(160) k_energy_final(const double* __restrict__ partial, int nblocks, double* __restrict__ rec, long long hist_base,
+                                                      double* scal, int advance) {
   __shared__ double sh[5];
   const int k = threadIdx.x >> 5, l = threadIdx.x & 31;
   double v = 0.0;
@@ -219,7 +224,11 @@ __global__ void __launch_bounds__(160) k_energy_final(const double* __restrict__
   if (l == 0) sh[k] = v;
   __syncthreads();
   if (threadIdx.x == 0) {
-    if (advance) { scal[SC_T] += scal[SC_DT]; scal[SC_LASTDT] = scal[SC_DT]; }
+    if (advance) {
+      scal[SC_T] += scal[SC_DT]; scal[SC_LASTDT] = scal[SC_DT];
+      rec += ((long long)scal[SC_STEP] - hist_base) * 7;
+      scal[SC_STEP] += 1.0;
+    }
     rec[0] = scal[SC_T];
     rec[1] = sh[0] + sh[1]; rec[2] = sh[0]; rec[3] = sh[1]; rec[4] = sh[2]; rec[5] = sh[3]; rec[6] = sh[4];
   }
@@ -337,14 +346,14 @@ cudaError_t launch_unpack(const Dims& d, const cd* S, cd* out, int nfields, int 
   return cudaGetLastError();
 }
 cudaError_t launch_forcing(const Dims& d, cd* S, const int* pairs, int npairs, double amp, unsigned long long seed,
-                           long long step, const double* scal, cudaStream_t st) {
-  k_forcing<<<nblk(2 * (size_t)npairs, 64), 64, 0, st>>>(d, S, pairs, npairs, amp, seed, step, scal);
+                           const double* scal, cudaStream_t st) {
+  k_forcing<<<nblk(2 * (size_t)npairs, 64), 64, 0, st>>>(d, S, pairs, npairs, amp, seed, scal);
   return cudaGetLastError();
 }
-cudaError_t launch_energy(const Dims& d, const cd* S, double* partial, int nblocks, double* rec, double* scal, int advance,
+cudaError_t launch_energy(const Dims& d, const cd* S, double* partial, int nblocks, double* rec, long long hist_base, double* scal, int advance,
                           cudaStream_t st) {
   k_energy_partial<<<nblocks, 256, 0, st>>>(d, S, partial);
-  k_energy_final<<<1, 160, 0, st>>>(partial, nblocks, rec, scal, advance);
+  k_energy_final<<<1, 160, 0, st>>>(partial, nblocks, rec, hist_base, scal, advance);
   return cudaGetLastError();
 }
 cudaError_t launch_spectrum(const Dims& d, const cd* S, double* col, int nbins, int literal, double dk, double* out, cudaStream_t st) {
@@ -361,8 +370,8 @@ cudaError_t launch_kpar_spectrum(const Dims& d, const cd* S, double* rows, int n
   k_kpar_bins<<<nblk((size_t)nbins, 128), 128, 0, st>>>(d, rows, nbins, out);
   return cudaGetLastError();
 }
-cudaError_t launch_forcing_g(const Dims& d, cd* S, int nzf, double amp, unsigned long long seed, long long step,
+cudaError_t launch_forcing_g(const Dims& d, cd* S, int nzf, double amp, unsigned long long seed,
                              const double* scal, cudaStream_t st) {
-  k_forcing_g<<<1, 1, 0, st>>>(d, S, nzf, amp, seed, step, scal);
+  k_forcing_g<<<1, 1, 0, st>>>(d, S, nzf, amp, seed, scal);
   return cudaGetLastError();
 }

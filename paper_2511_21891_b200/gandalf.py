@@ -85,6 +85,7 @@ def load_library():
     lib.gandalf_transfer_bytes.argtypes = [V, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     lib.gandalf_launch_count.argtypes = [V]
     lib.gandalf_launch_count.restype = C.c_longlong
+    lib.gandalf_graph_mode.argtypes = [V, I, C.POINTER(C.c_longlong)]
     lib.gandalf_kernel_timing.argtypes = [V, I]
     lib.gandalf_kernel_time_ms.argtypes = [V, I, PD, C.POINTER(C.c_longlong)]
     lib.gandalf_microbench.argtypes = [I, I, PD, I]
@@ -296,6 +297,12 @@ class Gandalf:
 
     def launch_count(self):
         return int(self._lib.gandalf_launch_count(self._h))
+
+    def graph_mode(self, enable=None):
+        """gandalf_graph_mode: switch the CUDA-graph launch path of step() on/off (None: query); returns the graph replays so far."""
+        n = C.c_longlong(0)
+        self._ck(self._lib.gandalf_graph_mode(self._h, -1 if enable is None else int(bool(enable)), C.byref(n)))
+        return n.value
 
     def kernel_timing(self, enable=True):
         self._ck(self._lib.gandalf_kernel_timing(self._h, int(bool(enable))))
