@@ -249,8 +249,15 @@ template <int NY> struct YGeom {
 #ifndef GD_Y512_THREADS
 #define GD_Y512_THREADS 384
 #endif
-  static constexpr int THREADS = (T >= 32) ? GD_Y512_THREADS : 256;
-  static constexpr int CTAS = (THREADS > 256) ? 1 : 2;       // resident CTAs per SM
+  // ny = 64, 128 (8 lanes per transform): 128-thread CTAs = 16 columns (256-byte rows, as at ny = 256), four per SM.  With 256 threads
+  // a CTA spans 32 columns and Kx = 43 (nx = 128) leaves the second block two thirds empty: measured at BASELINE config 3
+  // (128x128x64, M = 32) P1 0.163 -> 0.125 ms, P3 0.091 -> 0.080 ms, step 1.170 -> 1.067 ms; config 2 0.1637 -> 0.1597 ms
+#ifndef GD_Y8_THREADS
+#define GD_Y8_THREADS 128
+#endif
+  static constexpr int THREADS = (T >= 32) ? GD_Y512_THREADS : (T == 8 ? GD_Y8_THREADS : 256);
+  static constexpr int CTAS = (THREADS > 256) ? 1 : (THREADS <= 128 ? 4 : 2);       // resident CTAs per SM
+  static constexpr int PAIR_CTAS = (THREADS <= 128) ? 2 : 1;                        // of the register-heavy pair kernel
   static constexpr int GROUPS = THREADS / T;                 // columns per CTA
 };
 
@@ -371,7 +378,7 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Di
 // during B's transform.  (Geometry and shared-memory layout of k_yfwd below.)
 template <int NY> struct YFwdGeom;
 template <int NY>
-__global__ void __launch_bounds__(YGeom<NY>::THREADS, 1) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
+__global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::PAIR_CTAS) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
                                                                      const cd* __restrict__ tw, int ncb, int nitems);
 
 // k_yfwd: persistent CTAs over the work items (array a >= 2, z, block of GROUPS columns).  The exchange uses its
@@ -436,7 +443,7 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yfwd(Di
 }
 
 template <int NY>
-__global__ void __launch_bounds__(YGeom<NY>::THREADS, 1) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
+__global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::PAIR_CTAS) k_yfwd_pair(Dims d, const cd* __restrict__ Ein, cd* __restrict__ Gh,
                                                                      const cd* __restrict__ tw, int ncb, int nitems) {
   using Y = YGeom<NY>;
   using G = FftGeom<NY>;
@@ -554,7 +561,7 @@ cudaError_t launch_yfwd(const Dims& d, const cd* E, cd* Gh, const cd* tw, int nu
   {                                                                                                        \
     const int ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;                                    \
     const int np = d.nz * ncb;                                                                             \
-    k_yfwd_pair<NN><<<np < num_sms ? np : num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, np);   \
+    k_yfwd_pair<NN><<<np < YGeom<NN>::PAIR_CTAS * num_sms ? np : YGeom<NN>::PAIR_CTAS * num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, np);   \
     const int nitems = d.M * d.nz * ncb;                                                                   \
     if (d.M > 0) k_yfwd<NN><<<nitems < YGeom<NN>::CTAS * num_sms ? nitems : YGeom<NN>::CTAS * num_sms, YGeom<NN>::THREADS, YFwdGeom<NN>::SMEM, st>>>(d, E, Gh, tw, ncb, nitems); \
   }
