@@ -268,6 +268,38 @@ template <int NY> struct YGeom {
 // shared-memory tile; every lane group then reads its column once per output array (U, then V, Eq. 10; the
 // Elsasser sources first give xi = -w/kperp^2, then w) -- no second copy of the column in registers.
 // The next item's tile is requested as soon as the last read of the current one is done.
+#ifndef GD_Y_PAIR_RAGGED
+#define GD_Y_PAIR_RAGGED 1
+#endif
+// Work items of the persistent P1.  Classic enumeration: (array, z, column block), column block fastest; the last block of
+// a plane is ragged when GROUPS does not divide Kx (6 of 16 columns at nx = 256) and costs a full item's time.  Paired
+// enumeration (npf >= 0, the number of FULL blocks per plane; needs nz even and a remainder of at most GROUPS/2 columns): per
+// (array, pair of planes z0, z0+1) the 2*npf full blocks, then ONE item that takes the remainder columns of BOTH planes -- lane
+// groups [0, GROUPS/2) work on plane z0, [GROUPS/2, GROUPS) on plane z0+1, each on its own half of the tile.  At nx = 256 that is
+// 5.5 instead of 6 items per plane (lane use 86/88 instead of 86/96).  Measured at 4a, same box: P1 0.842 -> 0.800 ms, step 6.96 ->
+// 6.88 ms.  P3 keeps the classic enumeration: there the paired item doubles the per-row copy issue loop, which is what P3 waits
+// on (0.505 -> 0.513 ms).
+struct YItem { int arr, z0, cb; bool rag; };
+__device__ __forceinline__ YItem y_item(int item, int ncb, int nz, int npf) {
+  YItem it;
+  if (npf < 0) { it.cb = item % ncb; const int az = item / ncb; it.z0 = az % nz; it.arr = az / nz; it.rag = false; }
+  else {
+    const int ipp = 2 * npf + 1, j = item % ipp, ap = item / ipp, nzp = nz >> 1;
+    it.rag = (j == 2 * npf);
+    it.arr = ap / nzp;
+    it.z0 = 2 * (ap % nzp) + (it.rag ? 0 : j / (npf > 0 ? npf : 1));
+    it.cb = it.rag ? npf : j % (npf > 0 ? npf : 1);
+  }
+  return it;
+}
+// host: full blocks per plane if the paired enumeration applies, else -1; and the item count per array
+static inline int y_pair_mode(int Kx, int groups, int nz) {
+  const int rem = Kx % groups;
+  return (rem > 0 && 2 * rem <= groups && (nz & 1) == 0) ? Kx / groups : -1;
+}
+static inline int y_items_per_array(int Kx, int groups, int nz, int npf) {
+  return npf < 0 ? nz * ((Kx + groups - 1) / groups) : (nz / 2) * (2 * npf + 1);
+}
 template <int NY> struct YInvGeom {
   using Y = YGeom<NY>;
   static constexpr int LD = Y::GROUPS + 1;
@@ -277,10 +309,11 @@ template <int NY> struct YInvGeom {
 };
 template <int NY, bool ELS>   // ELS: the Elsasser sources s = 0, 1 (four outputs each, potentials first); else s = 2 + m
 __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Dims d, const cd* __restrict__ H, cd* __restrict__ D,
-                                                        const cd* __restrict__ tw, int ncb, int nitems) {
+                                                        const cd* __restrict__ tw, int ncb, int nitems, int npf) {
   using Y = YGeom<NY>;
   using G = FftGeom<NY>;
   using YI = YInvGeom<NY>;
+  constexpr int HALF = Y::GROUPS / 2;
   constexpr int T = G::T, E = G::E, LD = YI::LD;
   extern __shared__ cd smem[];
   __shared__ unsigned long long bar;
@@ -291,13 +324,16 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Di
   fft_load_table<NY>(smem, tw);                  // ends with __syncthreads()
   const cd* tws = smem;
   auto issue = [&](int item) {                   // all threads: one bulk copy per tile row (row = retained ky)
-    const int cb = item % ncb, sz = item / ncb;
-    const int z = sz % d.nz, s = sz / d.nz + (ELS ? 0 : 2);
-    const int cx0 = cb * Y::GROUPS;
+    const YItem it = y_item(item, ncb, d.nz, npf);
+    const int s = it.arr + (ELS ? 0 : 2);
+    const int cx0 = it.cb * Y::GROUPS;
     const int ncol = min(Y::GROUPS, d.Kx - cx0);
-    if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)(d.Ky * ncol * sizeof(cd)));
-    for (int r = threadIdx.x; r < d.Ky; r += Y::THREADS)
-      bulk_g2s(tile + (size_t)r * LD, H + (size_t)s * d.PH + ((size_t)z * d.Ky + r) * d.Kxp + cx0, (unsigned)(ncol * sizeof(cd)), &bar);
+    const cd* src = H + (size_t)s * d.PH + (size_t)it.z0 * d.Ky * d.Kxp + cx0;
+    if (threadIdx.x == 0) mbar_arrive_expect_tx(&bar, (unsigned)((it.rag ? 2 : 1) * d.Ky * ncol * sizeof(cd)));
+    for (int r = threadIdx.x; r < d.Ky; r += Y::THREADS) {
+      bulk_g2s(tile + (size_t)r * LD, src + (size_t)r * d.Kxp, (unsigned)(ncol * sizeof(cd)), &bar);
+      if (it.rag) bulk_g2s(tile + (size_t)r * LD + HALF, src + ((size_t)d.Ky + r) * d.Kxp, (unsigned)(ncol * sizeof(cd)), &bar);   // plane z0 + 1
+    }
   };
   constexpr int HY3 = NY / 3, KY = 2 * HY3 + 1;   // == d.hy3, d.Ky: compile-time so that the per-q mode tests fold
   int item = blockIdx.x;
@@ -305,10 +341,12 @@ __global__ void __launch_bounds__(YGeom<NY>::THREADS, YGeom<NY>::CTAS) k_yinv(Di
   unsigned phase = 0;
   const double kyt = d.ky0 * t, kyT = d.ky0 * T;
   while (item < nitems) {
-    const int cb = item % ncb, sz = item / ncb;
-    const int z = sz % d.nz, s = sz / d.nz + (ELS ? 0 : 2);
-    const int cx = cb * Y::GROUPS + grp;
-    const bool active = cx < d.Kx;
+    const YItem it = y_item(item, ncb, d.nz, npf);
+    const int s = it.arr + (ELS ? 0 : 2);
+    const int gz = (it.rag && grp >= HALF) ? 1 : 0;          // ragged pair item: the upper half of the groups takes plane z0 + 1
+    const int z = it.z0 + gz;
+    const int cx = it.cb * Y::GROUPS + grp - gz * HALF;
+    const bool active = cx < d.Kx;                           // (ragged: the remainder is at most HALF columns wide)
     const double kx = d.kx0 * cx;
     const int cxa = active ? cx : 0;
     constexpr int rounds = ELS ? 4 : 2;
@@ -549,9 +587,11 @@ cudaError_t launch_yinv(const Dims& d, const cd* H, cd* D, const cd* tw, int num
   {                                                                                                        \
     const int ncb = (d.Kx + YGeom<NN>::GROUPS - 1) / YGeom<NN>::GROUPS;                                    \
     const int cap = YGeom<NN>::CTAS * num_sms;                                                           \
-    const int ne = 2 * d.nz * ncb, nm = d.M * d.nz * ncb;                                                  \
-    k_yinv<NN, true><<<ne < cap ? ne : cap, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, ne);                 \
-    if (nm > 0) k_yinv<NN, false><<<nm < cap ? nm : cap, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, nm);    \
+    const int npf = GD_Y_PAIR_RAGGED ? y_pair_mode(d.Kx, YGeom<NN>::GROUPS, d.nz) : -1;                    \
+    const int ipa = y_items_per_array(d.Kx, YGeom<NN>::GROUPS, d.nz, npf);                                 \
+    const int ne = 2 * ipa, nm = d.M * ipa;                                                                \
+    k_yinv<NN, true><<<ne < cap ? ne : cap, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, ne, npf);                 \
+    if (nm > 0) k_yinv<NN, false><<<nm < cap ? nm : cap, YGeom<NN>::THREADS, YInvGeom<NN>::SMEM, st>>>(d, H, D, tw, ncb, nm, npf);    \
   }
   GD_DISPATCH(d.ny, YICASE)
   return cudaGetLastError();
