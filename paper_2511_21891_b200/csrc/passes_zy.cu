@@ -77,7 +77,7 @@ template <int NZ> struct ZStepGeom {
 // mapG / mapH: Gh and H viewed as fp64 tensors {2*Ky*Kx, nz, F} (the (ky,kx) plane flattened: hybrid rows are unpadded, so a
 // block of columns is contiguous even across a ky row end), boxes {16 doubles, NZ, 1}, 128-byte swizzle (common.cuh).
 template <int NZ, int MODE, bool EXACT>   // MODE 0 / 1 / 2 = RHS only / predictor / corrector + dissipation (compile time: fewer registers)
-__global__ void __launch_bounds__(ZStepGeom<NZ>::THREADS, ZStepGeom<NZ>::THREADS > 128 ? 2 : 4) k_zstep(Dims d, int if_variant, double skz_sign,
+__global__ void __launch_bounds__(ZStepGeom<NZ>::THREADS, ZStepGeom<NZ>::THREADS > 128 ? 2 : (ZStepGeom<NZ>::THREADS > 64 ? 4 : 8)) k_zstep(Dims d, int if_variant, double skz_sign,
                                                       const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapH,
                                                       bool have_G, bool want_H,
                                                       const cd* __restrict__ Wn, const cd* __restrict__ Ws, cd* __restrict__ Wout,
