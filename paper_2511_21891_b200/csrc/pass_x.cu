@@ -41,6 +41,11 @@
 #ifndef GD_X_TMHOIST
 #define GD_X_TMHOIST 0
 #endif
+#ifndef GD_X_ROTATE
+#define GD_X_ROTATE 1     // 1: the tile request of job g (wait for the stage to be released, two bulk copies) is made by warp g % WARPS instead of
+                          // always warp 0, so no warp runs systematically behind the others (they meet at every stage's empty barrier).
+                          // Measured, same box: x-pass 1.354 -> 1.288 ms at 4a, 1.215 -> 1.124 ms at 4b
+#endif
 #ifndef GD_X_ALT
 #define GD_X_ALT 0        // 1: nx = 256 on one WARP per line (plan 8*8*4, 8 points per lane, 16 warps per SM).  Measured SLOWER (1.72 vs 1.40 ms at 4a:
                           // the second exchange costs more than the extra warps hide; bare transform 1.35 vs 2.53 G/s) -- kept as a tested option
@@ -70,6 +75,8 @@ struct XGeom {
   static constexpr size_t SMEM_CAP = (CTAS == 2 ? 113 : 227) * 1024;   // per CTA
   static constexpr size_t smem_for(int nst) { return ((size_t)GROUPS * LB + (size_t)nst * STAGE + FftTw<FID>::COUNT) * sizeof(cd); }
   static constexpr int NST = (SPLITX && smem_for(4) <= SMEM_CAP) ? 4 : (smem_for(3) <= SMEM_CAP ? 3 : 2);                             // stages in flight (full/empty mbarrier ring), <= 5 (the first NST-1 are Elsasser arrays)
+  static constexpr int AHEAD = NST - 1;                      // tiles are requested this many jobs ahead (one stage less -- so that the stage being refilled was
+                                                            // released two jobs ago -- measured: no gain at 4a, 1.12 -> 1.18 ms at 4b)
   // stage-1 twiddles held in registers (plans with one stage-1 butterfly per lane): fewer shared-memory reads per transform
   static constexpr int NTWR = (G::S == 2 && E / FftPlan<FID>::R1 == 1) ? GD_X_NTWR : 0;
   static constexpr size_t SMEM = ((size_t)GROUPS * LB + (size_t)NST * STAGE + FftTw<FID>::COUNT) * sizeof(cd);
@@ -148,7 +155,7 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, XGeom<NX>::CTAS) k_xpass(D
     // the barriers, so that they travel while tensor memory is allocated and the twiddle table is staged
     constexpr unsigned TILE_BYTES0 = (unsigned)(X::KXP * X::LD * sizeof(cd));
 #pragma unroll
-    for (int kn = 0; kn < X::NST - 1; ++kn) {
+    for (int kn = 0; kn < X::AHEAD; ++kn) {
       const int a = kn == 0 ? 0 : kn == 1 ? 2 : kn == 2 ? 6 : 4;
       mbar_arrive_expect_tx(&s_full[kn], 2u * TILE_BYTES0);
       cd* st = stages + (size_t)kn * X::STAGE;
@@ -280,8 +287,8 @@ __global__ void __launch_bounds__(XGeom<NX>::THREADS, XGeom<NX>::CTAS) k_xpass(D
         // (this warp has seen the previous use of that stage complete, so the parity test cannot alias)
         tile_ready = mbar_test_wait(&s_full[(g + 1) % X::NST], (unsigned)(((g + 1) / X::NST) & 1));
 #endif
-        if (warp == 0) {
-          const int kn = kind + X::NST - 1;                     // job NST-1 ahead: of this block, or of the CTA's next one
+        if (warp == (GD_X_ROTATE ? (g & (X::WARPS - 1)) : 0)) {   // the producer role rotates over the warps: no warp lags the others by the request's cost
+          const int kn = kind + X::AHEAD;                       // job AHEAD ahead: of this block, or of the CTA's next one
           if (kn < nkinds) produce(g0 + kn, src_array(kn), blk);
           else if (blk + (int)gridDim.x < nblocks) produce(g0 + kn, src_array(kn - nkinds), blk + (int)gridDim.x);
         }
