@@ -172,6 +172,36 @@ int gandalf_energy(gandalf_ctx* ctx, double out[6]);
  * |xi-|^2) (bins sum to E_A); 1: |xi+|^2 + |xi-|^2 as printed.  out: nbins doubles on the HOST. */
 int gandalf_kperp_spectrum(gandalf_ctx* ctx, int nbins, int literal_eq26, double* out);
 
+/* The same shell spectrum for callers that must not allocate device memory [Eq. 26; Q15].
+ * Everything else in this header needs a gandalf_ctx, and a context (like gandalf_kperp_spectrum itself) gets its buffers from
+ * cudaMalloc.  That rules the library out for two kinds of caller: an application that gave all of the GPU's memory to its own
+ * pool when it started (a new cudaMalloc fails there, or makes the pool hand memory back), and a diagnostics hook that runs while
+ * other streams are busy and must not trigger the device-wide synchronisation cudaMalloc / cudaFree imply.  This one entry point
+ * takes no context, allocates nothing and frees nothing: the caller passes the state and the output as DEVICE pointers, and the
+ * per-column partial sums go to a fixed array of GANDALF_NOALLOC_MAX_COLUMNS doubles (256 KB) that is part of the library image.
+ *   device, stream   where to run; stream = NULL is the legacy default stream.  Two kernels are enqueued; the call does not
+ *                    synchronise.  The caller's current device is restored before returning.
+ *   nx, ny, nz       grid, as for gandalf_create (powers of two, 8 <= nx, ny <= 512, 2 <= nz <= 512), with
+ *                    (nx/3 + 1) * (2 (ny/3) + 1) <= GANDALF_NOALLOC_MAX_COLUMNS: 256 x 256 and 512 x 256 fit, 512 x 512 does not
+ *                    and is refused (GANDALF_ERR_INVALID, nothing launched) -- use gandalf_kperp_spectrum there.
+ *   Lx, Ly           box lengths (> 0); dk = 2 pi / max(Lx, Ly)
+ *   w_raw            device pointer, read only: the vorticities w^+ then w^- on the retained modes, i.e. the first two fields of
+ *                    the gandalf_get_state_raw layout (2 * 2 * Kz * Ky * Kx doubles; gandalf_field_ptr(ctx, 0, 0, ..) of a
+ *                    context the caller created earlier points at exactly this)
+ *   nbins, literal_eq26   as for gandalf_kperp_spectrum (1 <= nbins <= 65535)
+ *   out              device pointer, nbins doubles, overwritten; same values as gandalf_kperp_spectrum (same arithmetic and
+ *                    summation order)
+ *   err, errlen      optional caller buffer for a NUL-terminated message when the return value is not GANDALF_OK (may be NULL, 0)
+ * The fixed array is shared: every GPU that loads this library holds its 256 KB until the process exits; all calls on a device
+ * use it and it keeps the previous call's contents (harmless: each call writes every entry it later reads); calls that can
+ * overlap on the GPU -- two streams with no ordering between them, two host threads -- corrupt each other's sums, so order them.
+ * The FIRST call on a device also looks up the array's device address (cudaGetSymbolAddress; the driver may load the library's
+ * code on that device then): make it once at start-up, before any stream capture begins.
+ * Errors: INVALID (NULL array, bad grid / box / nbins / device, grid beyond the fixed array), CUDA (launch failed). */
+#define GANDALF_NOALLOC_MAX_COLUMNS 32768
+int gandalf_kperp_spectrum_noalloc(int device, void* stream, int nx, int ny, int nz, double Lx, double Ly,
+                                   const double* w_raw, int nbins, int literal_eq26, double* out, char* err, int errlen);
+
 /* Hermite spectrum [Eq. 27: C_m = <|g_m|^2>], instantaneous and volume averaged:
  * C_m = sum_k |g_m(k)|^2 over the full spectrum (so that sum_m C_m = 2 W_g).  out: M doubles on the HOST
  * (nothing is written when M = 0).  SURVEY.md 8(f) rank 1. */

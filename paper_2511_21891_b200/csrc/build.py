@@ -12,7 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 PKG = os.path.dirname(HERE)
 LIB = os.path.join(PKG, "libgandalf.so")
-SOURCES = ["api.cu", "passes_zy.cu", "pass_x.cu", "pointwise.cu", "microbench.cu", "hermite.cu"]
+SOURCES = ["api.cu", "passes_zy.cu", "pass_x.cu", "pointwise.cu", "microbench.cu", "hermite.cu", "noalloc.cu"]
 HEADERS = ["fft.cuh", "common.cuh", os.path.join("..", "..", "include", "gandalf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

@@ -74,6 +74,7 @@ def load_library():
     lib.gandalf_step.argtypes = [V, D, I]
     lib.gandalf_energy.argtypes = [V, PD]
     lib.gandalf_kperp_spectrum.argtypes = [V, I, I, PD]
+    lib.gandalf_kperp_spectrum_noalloc.argtypes = [I, V, I, I, I, D, D, V, I, I, V, C.c_char_p, I]
     lib.gandalf_hermite_spectrum.argtypes = [V, PD]
     lib.gandalf_kpar_spectrum.argtypes = [V, I, PD]
     lib.gandalf_truncation_ratio.argtypes = [V, PD]
@@ -105,6 +106,32 @@ def microbench(which, device=0):
     rc = lib.gandalf_microbench(int(which), int(device), out.ctypes.data_as(C.POINTER(C.c_double)), 4)
     if rc != OK:
         raise GandalfError(rc, "gandalf_microbench failed")
+    return out
+
+
+NOALLOC_MAX_COLUMNS = 32768      # GANDALF_NOALLOC_MAX_COLUMNS of include/gandalf.h
+
+
+def kperp_spectrum_noalloc(nx, ny, nz, w_raw, out, literal_eq26=False, Lx=2.0 * np.pi, Ly=2.0 * np.pi, device=0, stream=None):
+    """gandalf_kperp_spectrum_noalloc: the shell spectrum of Eq. 26 without a context and without any device allocation, for
+    callers that cannot allocate (all GPU memory already in their own pool, or no device-wide synchronisation allowed).
+    `w_raw` (float64 CUDA tensor: w+ then w- in the get_state_raw layout; more fields may follow) and `out` (float64 CUDA
+    tensor, one entry per bin, overwritten) are the caller's; the partial sums use a fixed 256 KB array inside the library that
+    all calls share, so do not let two calls overlap on the GPU.  Enqueues on `stream` (a cudaStream_t value; None = legacy
+    default stream) and does not synchronise.  Grids with more than NOALLOC_MAX_COLUMNS retained (kx, ky) columns raise
+    GandalfError(ERR_INVALID).  Make the first call on a device at start-up, outside any stream capture."""
+    import torch
+    lib = load_library()
+    need = 2 * 2 * (2 * (nz // 3) + 1) * (2 * (ny // 3) + 1) * (nx // 3 + 1)
+    for t in (w_raw, out):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.device.index == device
+    assert w_raw.numel() >= need, (w_raw.numel(), need)
+    msg = C.create_string_buffer(320)
+    rc = lib.gandalf_kperp_spectrum_noalloc(int(device), C.c_void_p(int(stream) if stream else None), nx, ny, nz, float(Lx), float(Ly),
+                                            C.c_void_p(w_raw.data_ptr()), int(out.numel()), int(bool(literal_eq26)),
+                                            C.c_void_p(out.data_ptr()), msg, len(msg))
+    if rc != OK:
+        raise GandalfError(rc, msg.value.decode())
     return out
 
 
