@@ -143,6 +143,7 @@ struct oracle_ctx {
   std::vector<cplx> hw[2];                  // half-step (stage) state of Alg. 1 l.3-4 between the two stages of a step
   std::vector<std::vector<cplx>> hg;
   double dt_cur;                            // the step's dt (fixed, or Eq. 16), set by the first stage
+  bool stage_pending = false;               // between oracle_step_stage(.., 0) and (.., 1): (hw, hg) hold a half-step state
   int moff, Mg;                             // shard: global index of local moment 0, global moment count (Q31)
   int own_lo, own_hi;                       // owned local moments [own_lo, own_hi): the rest are halos
   double t; long long step; double last_dt;
@@ -624,6 +625,7 @@ static int step_stage1(oracle_ctx* c, double dt_in) {
   if (exact) propagate(c, sh.g, 0.5 * dt);                  // g_{n+1/2} = P(dt/2) (g_n + dt/2 R_n),  P(tau) = exp(s i kz (I - T) tau)
   c->hw[0].swap(sh.w[0]); c->hw[1].swap(sh.w[1]); c->hg.swap(sh.g);
   c->dt_cur = dt;
+  c->stage_pending = true;
   return 0;
 }
 
@@ -671,6 +673,7 @@ static int step_stage2(oracle_ctx* c) {
   apply_forcing_g(c, s1, dt);
   c->w[0].swap(s1.w[0]); c->w[1].swap(s1.w[1]); c->g.swap(s1.g);
   c->t += dt; c->step += 1; c->last_dt = dt;
+  c->stage_pending = false;
   State cur; cur.w[0] = c->w[0]; cur.w[1] = c->w[1]; cur.g = c->g;
   double e[6]; energies(c, cur, e);
   c->hist.push_back(c->t);
@@ -772,6 +775,7 @@ int oracle_destroy(oracle_ctx* c) { delete c; return 0; }
 
 int oracle_set_state(oracle_ctx* c, const double* zeta_hat, const double* g_hat) {
   if (!c || !zeta_hat || (c->M > 0 && !g_hat)) return -1;
+  c->stage_pending = false;                 // a new state abandons a half-done step (as gandalf_set_state)
   const size_t hp = (size_t)c->nz * c->ny * (c->nx / 2 + 1) * 2;
   for (int a = 0; a < 2; ++a) {
     std::vector<cplx> xi;
@@ -811,6 +815,7 @@ int oracle_rhs(oracle_ctx* c, double* dw_hat, double* dg_hat) {
 
 int oracle_step(oracle_ctx* c, double dt, int nsteps) {
   if (!c || nsteps < 0) return -1;
+  if (c->stage_pending) { c->err = "oracle_step: a step is half done (stage 0 without stage 1)"; return -1; }
   for (int i = 0; i < nsteps; ++i) { int rc = step_once(c, dt); if (rc) return rc; }
   return 0;
 }
@@ -943,6 +948,11 @@ int oracle_bracket_full(oracle_ctx* c, const double* f_hat, const double* g_hat,
 // A moment-sharded run exchanges its halo moments between the stages (Q31); oracle_step(dt, 1) == stage 0 then stage 1.
 int oracle_step_stage(oracle_ctx* c, double dt, int stage) {
   if (!c || (stage != 0 && stage != 1)) return -1;
+  // the stages alternate 0, 1 (as gandalf_step_stage): stage 1 without a half-step state would read empty arrays
+  if ((stage == 1) != c->stage_pending || (stage == 1 && c->hw[0].size() != c->N)) {
+    c->err = "oracle_step_stage: stages must alternate 0, 1";
+    return -1;
+  }
   return stage == 0 ? step_stage1(c, dt) : step_stage2(c);
 }
 // Full-spectrum access to the half-step (stage) state, same field numbering as oracle_get_full.

@@ -117,3 +117,27 @@ def test_shard_parameters_are_validated():
         Oracle(16, 16, 8, M=4, m_offset=1)                             # offset without M_global
     with pytest.raises(Exception):
         Oracle(16, 16, 8, M=4, m_offset=0, M_global=8, hermite_exact=1)
+
+
+def test_oracle_stages_must_alternate():
+    """Stage 1 without a stage 0 has no half-step state to read (it used to index empty arrays); the oracle refuses it the
+    way gandalf_step_stage does, and refuses a full step while one is half done."""
+    prm, z, g, run = config2(16, 16, 8, 2)
+    o = Oracle(16, 16, 8, **prm)
+    o.set_state(z, g)
+    with pytest.raises(Exception):
+        o.step_stage(run["dt"], 1)
+    o.step_stage(run["dt"], 0)
+    with pytest.raises(Exception):
+        o.step_stage(run["dt"], 0)
+    with pytest.raises(Exception):
+        o.step(run["dt"], 1)
+    o.step_stage(run["dt"], 1)
+    ref = Oracle(16, 16, 8, **prm)
+    ref.set_state(z, g)
+    ref.step(run["dt"], 1)
+    assert np.array_equal(o.get_full(2), ref.get_full(2)) and o.time() == ref.time()
+    o.step_stage(run["dt"], 0)
+    o.set_state(z, g)                        # a new state abandons the half-done step
+    o.step(run["dt"], 1)
+    assert np.array_equal(o.get_full(0), ref.get_full(0))
