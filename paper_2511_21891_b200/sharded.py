@@ -89,8 +89,19 @@ class ShardLayout:
 class DistExchange:
     """Halo exchange over a torch.distributed process group (one rank per GPU; NCCL on GPUs, gloo on CPU)."""
 
-    def __init__(self, group=None):
-        self.group = group
+    def __init__(self, group=None, device=None):
+        """`device`: where reduction operands are placed.  None = decided by the backend: NCCL reduces CUDA tensors only, so
+        the operand goes to the current CUDA device (the one the shard's context runs on); gloo reduces on the host."""
+        self.group, self.device = group, device
+
+    def _reduce_device(self):
+        import torch
+        import torch.distributed as dist
+        if self.device is not None:
+            return torch.device(self.device)
+        if dist.get_backend(self.group) == "nccl":
+            return torch.device("cuda", torch.cuda.current_device())
+        return torch.device("cpu")
 
     def halos(self, shard, layout, state):
         import torch.distributed as dist
@@ -112,9 +123,9 @@ class DistExchange:
     def sum(self, x):
         import torch
         import torch.distributed as dist
-        t = x if isinstance(x, torch.Tensor) else torch.as_tensor(x)
+        t = (x if isinstance(x, torch.Tensor) else torch.as_tensor(x)).to(self._reduce_device())
         dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
-        return t
+        return t.cpu()
 
 
 class LocalExchange:

@@ -99,3 +99,38 @@ def test_staged_step_equals_step():
         b.step_stage(run["dt"], 1)
     assert torch.equal(a.get_state_raw(device=True), b.get_state_raw(device=True))
     assert np.array_equal(a.energy_history(), b.energy_history())
+
+
+def _nccl_world1(rank, port, shape, M, nsteps, out_path):
+    """One rank, NCCL backend: the path bench.py --parallelism mshard takes (DistExchange on the library's buffers), as far as
+    one GPU can take it -- no halo moves with a single rank, but W_g goes through an NCCL all-reduce, which accepts CUDA tensors
+    only (the energy record comes back from the library as a host array)."""
+    import os
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", rank=rank, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        prm, z, g, run = config2(*shape, M)
+        lay = sharded.ShardLayout.make(M, 1, 0)
+        sh = sharded.GandalfShard(*shape, lay, device=0, stream=torch.cuda.current_stream().cuda_stream, **prm)
+        sh.set_state(z, g)
+        st = sharded.ShardedStepper(sh, lay, sharded.DistExchange())
+        st.step(run["dt"], nsteps)
+        np.save(out_path, np.stack([st.energy(), sh.energy()]))
+        sh.close()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_stepper_energy_reduces_over_nccl(tmp_path):
+    import socket
+    import torch.multiprocessing as mp
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    out = str(tmp_path / "e.npy")
+    mp.spawn(_nccl_world1, args=(port, (32, 32, 16), 4, 3, out), nprocs=1, join=True)
+    e = np.load(out)
+    assert np.array_equal(e[0], e[1]) and e[0, 5] > 0            # one rank: the reduced record is the shard's own
