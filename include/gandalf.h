@@ -38,6 +38,8 @@ extern "C" {
 
 typedef struct gandalf_ctx gandalf_ctx;   /* opaque */
 
+#define GANDALF_HERMITE_EXACT_MAX_M 256   /* largest M with hermite_exact = 1 (shared-memory rows of the propagator, host eigen-solve) */
+
 typedef struct gandalf_params {
   int    nx, ny, nz;      /* grid; powers of two, 8 <= nx,ny <= 512, 2 <= nz <= 512               */
   int    M;               /* number of Hermite moments g_0..g_{M-1}; 0 = RMHD only (Q10)          */
@@ -73,7 +75,8 @@ typedef struct gandalf_params {
   int    hermite_exact;   /* 0: Hermite moments by plain RK2 [Alg. 1 l.4, l.9] (default).  1: the streaming / phase-mixing
                              operator s i kz (I - T) of Eq. 6 is integrated exactly (matrix exponential in m per kz,
                              integrating-factor midpoint for the brackets) [future work of PAPER.md:657, 829; lifts the
-                             dt < dz/v_th constraint of PAPER.md:214; Q30] */
+                             dt < dz/v_th constraint of PAPER.md:214; Q30].  Needs the absorbing
+                             closure, hermite_coeff = 0 and M <= GANDALF_HERMITE_EXACT_MAX_M (else GANDALF_ERR_UNSUPPORTED) */
   int    m_offset;        /* Moment shard [SURVEY.md 8(e)(i); PAPER.md:832, 975 list multi-device runs as future work; Q31]: */
   int    M_global;        /* this context holds the moments m_offset .. m_offset+M-1 of a hierarchy of M_global moments (0 = not
                              sharded).  If m_offset > 0 its FIRST moment field is a halo copy of the lower neighbour's last owned
@@ -137,8 +140,11 @@ int gandalf_rhs(gandalf_ctx* ctx, double* dw_hat, double* dg_hat, int on_device)
  * corrector (Alg. 1 l.8-9) -> exponential dissipation (Eq. 17-19) -> forcing increment (Eq. 25).
  * dt > 0: fixed step.  dt <= 0: dt = min(dt_max, cfl * min(Lx/nx, Ly/ny) / max|grad_perp Phi|) recomputed every
  * step ON THE DEVICE from the state at t_n (Eq. 16), no host synchronisation.  If the flow vanishes (max = 0) and
- * dt_max = 0 the step and all later ones are no-ops (dt = 0: the state survives, as in the oracle) and every
- * synchronising call returns GANDALF_ERR_CFL until gandalf_set_state.
+ * dt_max = 0 the step and all later ones are no-ops on the state (dt = 0: it survives unchanged, as in the oracle, which
+ * refuses such a step) and every synchronising call returns GANDALF_ERR_CFL until a new state is loaded: gandalf_set_state,
+ * gandalf_set_state_raw and gandalf_set_time clear the flag.  Unlike the oracle, the no-op steps are still COUNTED: the step
+ * number (and with it the forcing counters) moves on and each appends a history record of the unchanged state at the
+ * unchanged time -- the step is enqueued without a host round trip, so the host cannot take it back.
  * One energy record is appended per step to the device-resident history.  The call is
  * asynchronous on the ctx's stream; errors detected on the device (non-finite energy) are
  * reported by gandalf_energy_history / gandalf_energy / gandalf_get_time, which synchronise. */

@@ -238,6 +238,9 @@ int gandalf_create(const gandalf_params* p, gandalf_ctx** out) {
   } else if (p->m_offset != 0) return GANDALF_ERR_INVALID;
   if (p->M > 0 && p->vA != 1.0) return GANDALF_ERR_UNSUPPORTED;
   if (p->hermite_exact && p->M > 0 && (p->closure != 0 || p->hermite_coeff != 0)) return GANDALF_ERR_UNSUPPORTED;   // symmetric coupling matrix only (Q30)
+  // k_hermite_apply keeps 8 rows of the M x M propagator in the default 48 KB of dynamic shared memory (128 M bytes), and the
+  // set-up diagonalises the coupling matrix on the host (O(M^3)) and stores Kz M^2 propagator entries: bounded here, not at the first step
+  if (p->hermite_exact && p->M > GANDALF_HERMITE_EXACT_MAX_M) return GANDALF_ERR_UNSUPPORTED;
   if (cudaSetDevice(p->device) != cudaSuccess) { cudaGetLastError(); return GANDALF_ERR_CUDA; }
 
   gandalf_ctx* c = new (std::nothrow) gandalf_ctx();
@@ -503,6 +506,7 @@ int gandalf_set_state_raw(gandalf_ctx* c, const double* in, int on_device) {
   const size_t bytes = (size_t)c->d.F * c->d.PS * sizeof(cd);
   GD_CUDA(c, cudaMemcpyAsync(c->S0, in, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->st));
   if (!on_device) c->h2d_bytes += (long long)bytes;
+  GD_CUDA(c, cudaMemsetAsync(c->scal + SC_ERR, 0, sizeof(double), c->st));   // a new state: the sticky Eq. 16 flag of the old one goes
   c->stage_pending = false;
   int rc = make_hybrid(c, c->S0);
   if (rc) return rc;
@@ -518,6 +522,7 @@ int gandalf_set_time(gandalf_ctx* c, double t, long long step) {
   const double dstep = (double)step;
   GD_CUDA(c, cudaMemcpyAsync(c->scal + SC_T, &t, sizeof(double), cudaMemcpyHostToDevice, c->st));
   GD_CUDA(c, cudaMemcpyAsync(c->scal + SC_STEP, &dstep, sizeof(double), cudaMemcpyHostToDevice, c->st));
+  GD_CUDA(c, cudaMemsetAsync(c->scal + SC_ERR, 0, sizeof(double), c->st));   // a resumed run starts without the sticky Eq. 16 flag
   GD_CUDA(c, cudaStreamSynchronize(c->st));     // t, dstep live on this stack frame
   c->step = step; c->hist_base = step;          // the history restarts at the resumed step
   return GANDALF_OK;

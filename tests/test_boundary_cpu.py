@@ -66,7 +66,8 @@ def test_unsupported_combination(lib):
 
 
 @pytest.mark.parametrize("combo", [dict(M=4, M_global=8, nspecies=2), dict(M=4, M_global=8, hermite_exact=1),
-                                   dict(M=4, hermite_exact=1, closure=1), dict(M=4, hermite_exact=1, hermite_coeff=1)])
+                                   dict(M=4, hermite_exact=1, closure=1), dict(M=4, hermite_exact=1, hermite_coeff=1),
+                                   dict(M=257, hermite_exact=1)])     # above GANDALF_HERMITE_EXACT_MAX_M: refused at create, not at the first step
 def test_unsupported_shard_and_exact_combinations(lib, combo):
     """Moment shards (Q31) take one species and the RK2 streaming step; the exact propagator (Q30) a symmetric
     coupling matrix."""

@@ -64,6 +64,41 @@ def test_cfl_zero_flow_leaves_state_and_reports():
     assert g.time()[1] == 1
 
 
+def test_cfl_error_is_cleared_by_a_raw_restart():
+    """The sticky Eq. 16 flag belongs to the state that had no flow: loading another state the restart way
+    (set_state_raw + set_time) must clear it, and the run then continues like a context that never saw the error."""
+    from paper_2511_21891_b200.gandalf import Gandalf, GandalfError, ERR_CFL
+    shape, M = (16, 16, 8), 2
+    gm = synth.dense_random(*shape, M, seed=5, decay=2.5)
+    z = synth.dense_random(*shape, 2, seed=6, decay=2.5)
+    z0 = np.zeros_like(z)
+    good = Gandalf(*shape, M=M)
+    good.set_state(z, gm)
+    good.step(-1.0, 2)
+    raw, (t, step, _) = good.get_state_raw(), good.time()
+    g = Gandalf(*shape, M=M)
+    g.set_state(z0, gm)
+    g.step(-1.0, 2)                                   # no flow, no dt_max
+    with pytest.raises(GandalfError) as ei:
+        g.time()
+    assert ei.value.code == ERR_CFL
+    g.set_state_raw(raw)
+    g.set_time(t, step)
+    assert g.time()[:2] == (t, step)                  # no error any more
+    g.step(-1.0, 3); good.step(-1.0, 3)
+    assert g.time() == good.time()
+    assert np.array_equal(g.get_state_raw(), good.get_state_raw())
+    # set_state_raw alone clears it too
+    h = Gandalf(*shape, M=M)
+    h.set_state(z0, gm)
+    h.step(-1.0, 1)
+    with pytest.raises(GandalfError):
+        h.time()
+    h.set_state_raw(raw)
+    h.step(-1.0, 1)
+    assert h.time()[1] == 2 and h.time()[2] > 0       # the no-op step was counted (documented), the new one took a real dt
+
+
 def test_cfl_dt_max_matches_oracle():
     from oracle import Oracle
     from paper_2511_21891_b200.gandalf import Gandalf
