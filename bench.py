@@ -361,6 +361,45 @@ def run_planes_sweep(device=0, planes=(2, 4, 8, 16, 32, 128)):
     return out
 
 
+L2_BYTES = 126e6          # B200 L2 (B200_PROFILING.md)
+CAPTURE_SOURCES = ("pass_x.cu", "passes_zy.cu", "fft.cuh", "common.cuh")      # what the kernels of the committed ncu captures are built from
+
+
+def kernel_sources_sha256():
+    """sha256 over the kernel sources the committed ncu figures (profiles/r0N_traffic.csv, _fp64_instr.csv) were captured from."""
+    import hashlib
+    h = hashlib.sha256()
+    for fn_ in CAPTURE_SOURCES:
+        h.update(open(os.path.join(ROOT, "paper_2511_21891_b200", "csrc", fn_), "rb").read())
+    return h.hexdigest()
+
+
+def captures_stale(tag="r02"):
+    """True when the kernel sources differ from the ones hashed in profiles/<tag>_capture_sources.md at capture time (the
+    committed traffic / instruction counts then describe another build); None when no hash was recorded."""
+    try:
+        txt = open(os.path.join(ROOT, "profiles", f"{tag}_capture_sources.md")).read()
+    except OSError:
+        return None
+    import re
+    m = re.search(r"sha256[^0-9a-f]*([0-9a-f]{64})", txt)
+    return None if not m else m.group(1) != kernel_sources_sha256()
+
+
+def classify_bound(dom_bytes, hbm_floor_ms, alu_floor_ms):
+    """Which roof bounds the dominant kernel, and the L2 note of the timing rules, from the workload itself:
+    a launch whose algorithmic bytes fit the L2 is not an HBM measurement at all (the small grids are launch / latency
+    bound); otherwise the larger of the HBM floor and the fp64-instruction floor (when one is known)."""
+    if dom_bytes <= L2_BYTES:
+        return ("launch/latency",
+                "NOT flushed: the dominant kernel moves %.1f MB per launch, which fits the 126 MB L2 -- this grid is launch / latency bound "
+                "(DESIGN.md 5b) and the HBM fraction below says nothing about the kernels" % (dom_bytes / 1e6))
+    l2 = "no flush needed: the dominant kernel streams %.2f GB per launch, far more than the 126 MB L2" % (dom_bytes / 1e9)
+    if alu_floor_ms is not None and alu_floor_ms > hbm_floor_ms:
+        return "alu", l2
+    return "hbm", l2
+
+
 def run_mshard(args, rank, world, local):
     """ONE run of the workload sharded by Hermite moment over the ranks (strong scaling): xi+- replicated, one halo moment per
     neighbour exchanged twice per step with NCCL point-to-point copies in place on the library's buffers (sharded.py)."""
@@ -409,12 +448,12 @@ def run_mshard(args, rank, world, local):
     ms = max_over_ranks(e0.elapsed_time(e1), world)
     clocks = sampler.stop()
     launches = sum(sh.g.launch_count() for sh in shards) - n0
-    en = np.array([sh.energy() for sh in shards])
-    wg = float(en[:, 5].sum())
     if world > 1:
-        t = torch.tensor([wg], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t)
-        wg = float(t.item())
+        en = np.array([stepper.energy()])                          # W_g summed over the ranks by DistExchange (a CUDA tensor under NCCL)
+        wg = float(en[0, 5])
+    else:
+        en = np.array([sh.energy() for sh in shards])
+        wg = float(en[:, 5].sum())
     if rank == 0:
         steps_per_s = args.steps / (ms * 1e-3)                     # ONE run: the ranks share the work (strong scaling)
         halo_bytes = 16 * (shape[0] // 3 + 1) * (2 * (shape[1] // 3) + 1) * (2 * (shape[2] // 3) + 1)
@@ -604,6 +643,7 @@ def main():
             pass
         if traffic is not None:
             break
+    stale = captures_stale("r02")
     # fp64 side of the dominant kernel: 5 N log2 N flops per complex transform against the DFMA rate
     # measured on this device right now (gandalf_microbench 0)
     alu = None
@@ -634,14 +674,30 @@ def main():
         alu = {"error": repr(exc)[:200]}
     step_ms = ms / args.steps
     bound_note = None
+    hbm_floor = per_launch[dom] / 1e9 / peak_gbs * 1e3
+    alu_floor = None
     if isinstance(alu, dict) and "instr" in alu:
-        hbm_floor = per_launch[dom] / 1e9 / peak_gbs * 1e3
         alu_floor = alu["instr"]["fp64_warp_instructions_per_launch"] * 32 / (alu["measured_fp64_t_instr_per_s"] * 1e12) * 1e3
+    bound, l2_note = classify_bound(per_launch[dom], hbm_floor, alu_floor)
+    hbm_side = {"achieved": kern[dom]["achieved_gbs"], "peak": peak_gbs, "unit": "GB/s", "frac": kern[dom]["achieved_gbs"] / peak_gbs,
+                "floor_ms": hbm_floor}
+    head = dict(hbm_side)
+    if bound == "alu":       # the larger floor is the roof the kernel can actually reach: report against it, keep the HBM side beside it
+        ins = alu["instr"]
+        head = {"achieved": ins["achieved_t_instr_per_s"], "peak": alu["measured_fp64_t_instr_per_s"], "unit": "T fp64 thread-instr/s",
+                "frac": ins["frac_of_measured_issue_rate"], "floor_ms": alu_floor}
+        peak_src = "measured in this run (gandalf_microbench 0: fp64 issue rate of all SMs); the HBM side uses " + peak_src
         bound_note = ("%s sits on the ridge: HBM floor %.2f ms (algorithmic bytes at the measured copy bandwidth), fp64-instruction floor %.2f ms "
-                      "(executed fp64 instructions at the measured issue rate), measured %.2f ms; the path as a whole is HBM-bound, so the "
-                      "fraction is reported against HBM and the ALU side is in roofline.alu" % (dom, hbm_floor, alu_floor, kern[dom]["avg_ms"]))
-    roofline = {"bound": "hbm", "bound_note": bound_note, "kernel": dom, "achieved": kern[dom]["achieved_gbs"], "peak": peak_gbs, "peak_source": peak_src,
-                "unit": "GB/s", "frac": kern[dom]["achieved_gbs"] / peak_gbs, "traffic": traffic, "traffic_source": traffic_src,
+                      "(executed fp64 instructions at the measured issue rate), measured %.2f ms; the larger floor is the bound reported, the HBM "
+                      "side is in roofline.hbm (the step as a whole is HBM-bound: roofline.step)" % (dom, hbm_floor, alu_floor, kern[dom]["avg_ms"]))
+    elif bound == "launch/latency":
+        bound_note = "the dominant kernel's bytes per launch fit the L2: neither roof applies, the step is a chain of short launches (cuda graph replay)"
+    elif alu_floor is not None:
+        bound_note = ("%s: HBM floor %.2f ms, fp64-instruction floor %.2f ms, measured %.2f ms" % (dom, hbm_floor, alu_floor, kern[dom]["avg_ms"]))
+    roofline = {"bound": bound, "bound_note": bound_note, "kernel": dom, "achieved": head["achieved"], "peak": head["peak"], "peak_source": peak_src,
+                "unit": head["unit"], "frac": head["frac"], "floor_ms": head["floor_ms"], "measured_ms": kern[dom]["avg_ms"], "hbm": hbm_side,
+                "traffic": traffic, "traffic_source": traffic_src,
+                "traffic_stale": stale, "traffic_stale_how": "sha256 of csrc/{%s} against profiles/r02_capture_sources.md" % ", ".join(CAPTURE_SOURCES),
                 "algorithmic_bytes_per_launch": per_launch[dom],
                 "note": "per-kernel times come from a second pass of %d steps with CUDA events around every launch (%.3f ms/step); the headline "
                         "ms_per_step is timed without them" % (ksteps, kms / ksteps),
@@ -667,7 +723,7 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl, "grid": list(shape), "M": M, "dt": dt, "fields": F, "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "l2": "no flush needed: every kernel streams inputs far larger than the 126 MB L2 (working set per step > 9 GB at 4a)"},
+                       "l2": l2_note},
             "steps_per_s": steps_per_s, "grid_point_moments_per_s": steps_per_s * shape[0] * shape[1] * shape[2] * F,
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
             "launch_path": ("cuda graph of one step, replayed" if graph_replays else "plain stream launches"), "graph_replays": graph_replays, "roofline": roofline, "cpu_baseline": cpu, "cufft_comparison": cufft, "kperp_spectrum": spectrum,

@@ -73,3 +73,28 @@ def test_moment_shard_layouts_used_by_the_bench():
     lays = [sharded.ShardLayout.make(32, 4, r) for r in range(4)]
     assert [lay.hi - lay.lo for lay in lays] == [8, 8, 8, 8] and [lay.M_local for lay in lays] == [9, 10, 10, 9]
     assert lays[1].params() == dict(M=10, m_offset=7, M_global=32) and sharded.ShardLayout.make(32, 1, 0).params() == dict(M=32)
+
+
+def test_bound_and_l2_note_follow_the_workload():
+    """The bench line must not call a launch-bound small grid 'hbm', nor claim 'no flush needed' for a working set that fits
+    the L2; on the large grids the larger of the two floors is the bound."""
+    import bench
+    per_launch, _ = bench.algorithmic_bytes((32, 32, 16), 0)
+    b, note = bench.classify_bound(max(per_launch.values()), 1e-3, None)
+    assert b == "launch/latency" and note.startswith("NOT flushed")
+    per_launch, _ = bench.algorithmic_bytes((256, 256, 128), 32)
+    dom = per_launch["x_pass_P2"]
+    assert bench.classify_bound(dom, 0.73, 0.79)[0] == "alu"
+    assert bench.classify_bound(dom, 0.73, 0.60)[0] == "hbm"
+    b, note = bench.classify_bound(dom, 0.73, None)
+    assert b == "hbm" and note.startswith("no flush needed") and "4.78 GB" in note
+    per_launch, _ = bench.algorithmic_bytes((128, 128, 64), 32)
+    assert bench.classify_bound(per_launch["x_pass_P2"], 0.1, None)[0] == "hbm"
+
+
+def test_committed_ncu_figures_belong_to_the_current_kernel_sources():
+    """roofline.traffic and roofline.alu.instr are copied from committed captures; the hash beside them must be the one of
+    the kernel sources in this tree (re-capture and update profiles/r02_capture_sources.md after touching a kernel)."""
+    import bench
+    assert bench.captures_stale("r02") is False
+    assert bench.captures_stale("no_such_round") is None
