@@ -66,6 +66,44 @@ def test_dense_same_grid_config4a_size_rhs_and_two_steps():
     assert np.abs(hg[:, 1:] - ho[:, 1:]).max() <= 1e-9 * np.abs(ho[:, 1:]).max()
 
 
+@pytest.mark.slow
+def test_dense_same_grid_config4a_with_all_32_moments_rhs():
+    """BASELINE config 4(a) exactly as bench.py times it -- 256x256x128 with M = 32 -- on a dense
+    spectrum: one RHS against Oracle(256, 256, 128, M=32).  The 34-field sliding window of the x-pass, its 53-job tile ring
+    across line blocks and P4's 34-field block order carry real data in every mode here (the M = 4 test above does not reach
+    them).  The oracle needs about half a minute and ~20 GB of host memory for this one evaluation."""
+    shape, M = (256, 256, 128), 32
+    prm = dict(M=M, nu_coll=1.0, p=2.0, eta=1.0, r=2, eta_normalized=1, eta_g=1.0)
+    o, g = _pair(shape, prm)
+    z = synth.dense_random(*shape, 2, seed=4420, decay=3.0)
+    gm = synth.dense_random(*shape, M, seed=4421, decay=3.0)
+    o.set_state(z, gm); g.set_state(z, gm)
+    del z, gm
+    t0 = time.time()
+    ew, eg = _rhs_err(o, g)
+    print(f"dense 256x256x128 M=32: RHS rel L2 dw {ew:.2e} dg {eg:.2e} (oracle + GPU {time.time() - t0:.0f} s)")
+    assert ew <= 1e-12 and eg <= 1e-12
+
+
+def test_hermite_exact_at_a_grid_with_thousands_of_apply_blocks():
+    """hermite_exact = 1 at BASELINE config 3's size (128x128x64, M = 32): k_hermite_apply launches 29 x 43 x 4 = 4988 blocks
+    here (the other exact-propagator parity cases stay below 64x64x32).  One RHS and two steps against the oracle."""
+    shape, M = (128, 128, 64), 32
+    prm = dict(M=M, hermite_exact=1, nu_coll=1.0, p=2.0, eta=1.0, r=2, eta_normalized=1, eta_g=1.0)
+    o, g = _pair(shape, prm)
+    z = synth.dense_random(*shape, 2, seed=4430, decay=3.0)
+    gm = synth.dense_random(*shape, M, seed=4431, decay=3.0)
+    o.set_state(z, gm); g.set_state(z, gm)
+    ew, eg = _rhs_err(o, g)
+    assert ew <= 1e-12 and eg <= 1e-12
+    o.step(2e-3, 2); g.step(2e-3, 2)
+    ez, egs = _state_err(o, g)
+    print(f"hermite_exact 128x128x64 M=32: RHS dw {ew:.2e} dg {eg:.2e}; state after 2 steps zeta {ez:.2e} g {egs:.2e}")
+    assert ez <= 1e-10 and egs <= 1e-10
+    ho, hg = o.energy_history(), g.energy_history()
+    assert np.abs(hg[:, 1:] - ho[:, 1:]).max() <= 1e-9 * np.abs(ho[:, 1:]).max()
+
+
 def test_dense_same_grid_config4a_size_two_species():
     shape, M = (256, 256, 128), 2
     o, g = _pair(shape, dict(M=M, nspecies=2))
