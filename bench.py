@@ -217,13 +217,27 @@ def cpu_baseline_sample(name, full_shape, full_rhs=False):
     del o1
     oracle.set_num_threads(nthreads)
     if full_rhs:
+        # the slab flatters the oracle (its z transforms shrink with the slab): where the host has the memory, ONE RHS evaluation at
+        # the full grid is the reported value and the slab figure moves to `slab_sample`
         of, _, runf = _oracle_slab(name, full_shape[2])
         t0 = time.perf_counter()
         of.rhs()
         elf = time.perf_counter() - t0
-        out["full_grid_rhs"] = {"value": 1.0 / elf, "unit": "RHS evals/s", "cores": nthreads, "seconds": elf,
-                                "sample": f"one RHS evaluation at the full {full_shape[0]}x{full_shape[1]}x{full_shape[2]} grid, all moments (no scaling)"}
+        del of
+        out["slab_sample"] = {k: out[k] for k in ("value", "seconds", "sample")}
+        out.update({"value": 1.0 / elf, "seconds": elf,
+                    "sample": f"ONE RHS evaluation at the full {full_shape[0]}x{full_shape[1]}x{full_shape[2]} grid, all moments, no scaling "
+                              f"(the slab figure, which --impl reference also uses, is in slab_sample)"})
     return out
+
+
+def host_can_hold_full_oracle(shape, F):
+    """The oracle keeps full complex spectra: about 12 arrays of nx*ny*nz complex per field at the RHS (measured ~20 GB at 4a)."""
+    try:
+        avail = os.sysconf("SC_AVPHYS_PAGES") * os.sysconf("SC_PAGE_SIZE")
+    except (ValueError, OSError):
+        return False
+    return avail > 2.0 * 12 * F * shape[0] * shape[1] * shape[2] * 16
 
 
 def cufft_comparison(sim, stream, shape, prm, reps=3):
@@ -336,31 +350,6 @@ def run_microbench(device=0, which=(0, 1, 2, 3)):
     return out
 
 
-def run_planes_sweep(device=0, planes=(2, 4, 8, 16, 32, 128)):
-    """What z-batching the P1 -> P2 -> P3 chain to keep its intermediates in L2 would have to beat: the same
-    kernels on 256x256xnz grids with all 34 fields.  D + E are 37.6 MB per plane, so nz = 2 is L2-resident and nz >= 8 is not."""
-    import torch
-    from paper_2511_21891_b200.gandalf import Gandalf, KERNEL_CLASSES
-    from paper_2511_21891_b200 import workloads
-    out = {"what": "ms per launch of each pass kernel at 256x256xnz, M = 32, scaled by 128/nz", "D_plus_E_MB_per_plane": 37.6, "rows": {}}
-    for nz in planes:
-        prm, z, g, run = workloads.config4a(nz=nz)
-        stream = torch.cuda.Stream(device=device)
-        sim = Gandalf(*run["shape"], device=device, stream=stream.cuda_stream, **prm)
-        with torch.cuda.stream(stream):
-            sim.set_state(torch.from_numpy(z).cuda(device), torch.from_numpy(g).cuda(device))
-            sim.step(run["dt"], 5)
-        torch.cuda.synchronize()
-        sim.kernel_timing(True)
-        with torch.cuda.stream(stream):
-            sim.step(run["dt"], 20)
-        torch.cuda.synchronize()
-        kt = sim.kernel_times()
-        out["rows"][str(nz)] = {k: round(kt[k][0] / nz * 128, 4) for k in KERNEL_CLASSES if kt[k][1]}
-        sim.close()
-    return out
-
-
 L2_BYTES = 126e6          # B200 L2 (B200_PROFILING.md)
 CAPTURE_SOURCES = ("pass_x.cu", "passes_zy.cu", "fft.cuh", "common.cuh")      # what the kernels of the committed ncu captures are built from
 
@@ -398,6 +387,55 @@ def classify_bound(dom_bytes, hbm_floor_ms, alu_floor_ms):
     if alu_floor_ms is not None and alu_floor_ms > hbm_floor_ms:
         return "alu", l2
     return "hbm", l2
+
+
+def quick_time(workload, local, warmup=10, steps=50):
+    """ms per step and roofline fractions of another workload, timed like the headline (CUDA events on the context's stream, then a
+    per-kernel pass): used to put BASELINE config 4(b) into the default line (extra.config4b)."""
+    import torch
+    from paper_2511_21891_b200.gandalf import Gandalf, KERNEL_CLASSES
+    prm, z, g, run = make_workload(workload)
+    shape, dt, M = run["shape"], run["dt"], prm.get("M", 0) * prm.get("nspecies", 1)
+    stream = torch.cuda.Stream()
+    sim = Gandalf(*shape, device=local, stream=stream.cuda_stream, **prm)
+    zd = torch.from_numpy(z).cuda()
+    gd = torch.from_numpy(g).cuda() if M else None
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        sim.set_state(zd, gd)
+        sim.step(dt, warmup)
+    torch.cuda.synchronize()
+    sampler.start()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        sim.step(dt, steps)
+        e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    sim.kernel_timing(True)
+    with torch.cuda.stream(stream):
+        sim.step(dt, 10)
+    torch.cuda.synchronize()
+    kt = sim.kernel_times()
+    sim.kernel_timing(False)
+    clocks = sampler.stop()
+    assert np.isfinite(sim.energy_history()).all()
+    sim.close()
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = peaks.get("hbm_gbs", 6650.0)
+    per_launch, step_bytes = algorithmic_bytes(shape, M)
+    kern = {k: {"avg_ms": kt[k][0], "frac_of_hbm_peak": per_launch[k] / 1e9 / (kt[k][0] * 1e-3) / peak}
+            for k in KERNEL_CLASSES if kt[k][1] and k != "z_inverse"}
+    dom = max(kern, key=lambda k: kern[k]["avg_ms"])
+    return {"workload": f"BASELINE config {workload}", "grid": list(shape), "M": M, "steps": steps, "warmup": warmup, "ms_per_step": ms,
+            "value": 2e3 / ms, "unit": "RHS evals/s", "step_algorithmic_gb": step_bytes / 1e9,
+            "step_frac_of_measured_hbm_peak": step_bytes / 1e9 / (ms * 1e-3) / peak, "dominant_kernel": dom,
+            "dominant_kernel_frac": kern[dom]["frac_of_hbm_peak"], "kernels": kern, "clocks": clocks}
 
 
 def run_mshard(args, rank, world, local):
@@ -487,13 +525,13 @@ def main():
     ap.add_argument("--no-cufft-compare", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="plain stream launches instead of the replayed CUDA graph of one step")
     ap.add_argument("--oracle-full-rhs", action="store_true", help="also time one oracle RHS evaluation at the FULL grid (slow, ~20 GB host memory at 4a)")
+    ap.add_argument("--no-oracle-full-rhs", action="store_true", help="cpu_baseline from the z-slab sample only (skips the ~30 s full-grid oracle RHS of the default 4a run)")
+    ap.add_argument("--sustained-seconds", type=float, default=3.0, help="after the timed region, run about this many seconds of steps and report them as `sustained` (0 = off)")
+    ap.add_argument("--no-4b", action="store_true", help="do not time BASELINE config 4(b) after the default 4a run")
     ap.add_argument("--microbench", action="store_true", help="print the measured unit ceilings (gandalf_microbench) and exit")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "mshard"],
                     help="N > 1: independent replicas (default; north_star keeps the product on one GPU) or ONE run sharded by Hermite "
                          "moment with halo exchange over NCCL (paper_2511_21891_b200/sharded.py, DESIGN.md Q31)")
-    ap.add_argument("--planes-sweep", action="store_true",
-                    help="time the four pass kernels of config 4(a) restricted to nz = 2, 4, ... planes (working set of the P1->P2->P3 "
-                         "intermediates from inside the 126 MB L2 to far outside it) and print ms per launch scaled to 128 planes")
     ap.add_argument("--emulate-ranks", type=int, default=0, help="mshard on ONE GPU: emulate this many ranks in one process (checks the path; not a scaling number)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -505,10 +543,6 @@ def main():
     if args.microbench:
         if rank == 0:
             print(json.dumps(run_microbench(local)), flush=True)
-        return
-    if args.planes_sweep:
-        if rank == 0:
-            print(json.dumps(run_planes_sweep(local)), flush=True)
         return
     if args.warmup < 3:
         args.warmup = 3
@@ -571,8 +605,24 @@ def main():
     ktimes = sim.kernel_times()
     sim.kernel_timing(False)
     clocks = sampler.stop()             # sampled over the timed region and the per-kernel pass that follows it (same load)
+    # a time stepper runs for minutes: the same steps over a few SECONDS, where the power cap has settled the clock
+    sustained, nsus = None, 0
+    if args.sustained_seconds > 0:
+        nsus = max(args.steps, int(args.sustained_seconds / max(ms / args.steps * 1e-3, 1e-6)))
+        nsus = min(nsus, 20000)
+        s2 = ClockSampler(local)
+        s2.start()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            s0.record(stream)
+            sim.step(dt, nsus)
+            s1.record(stream)
+        torch.cuda.synchronize()
+        sms = max_over_ranks(s0.elapsed_time(s1), world)
+        sustained = {"steps": nsus, "seconds": sms * 1e-3, "ms_per_step": sms / nsus, "value": 2 * whole_job_steps_per_s(sms, nsus, world),
+                     "unit": "RHS evals/s", "clocks": s2.stop()}
     hist = sim.energy_history()
-    assert hist.shape[0] == args.warmup + args.steps + ksteps and np.isfinite(hist).all()
+    assert hist.shape[0] == args.warmup + args.steps + ksteps + nsus and np.isfinite(hist).all()
     spectrum = None
     if args.workload == "3":      # BASELINE config 3 "reports the k_perp energy spectrum" (Eq. 26; unpinned statistics)
         sp = sim.kperp_spectrum(44)
@@ -606,11 +656,35 @@ def main():
         el = time.perf_counter() - t0
         el = max_over_ranks(el, world)
         b1 = sim.transfer_bytes()           # counted by the library at the copies it issues (gandalf_transfer_bytes)
+        energy_only = {"value": 2 * world * args.e2e_steps / el, "unit": "RHS evals/s",
+                       "h2d_bytes_per_step": int((b1[0] - b0[0]) // args.e2e_steps), "d2h_bytes_per_step": int((b1[1] - b0[1]) // args.e2e_steps),
+                       "what": "gandalf_set_state(host pinned) + gandalf_step(dt,1) + gandalf_energy_history(host): only the energy record comes back"}
+        # the result of a step is the new STATE: read it back too, in the library's checkpoint format (gandalf_get_state_raw: the
+        # retained modes of every field, the mirror of what set_state moves in), into pinned host memory
+        rawp = torch.empty(sim.state_raw_doubles(), dtype=torch.float64, pin_memory=True)
+        rawh = rawp.numpy()
+
+        def read_state():
+            sim.get_state_raw(out=rawh)
+        read_state()
+        torch.cuda.synchronize()
+        b0 = sim.transfer_bytes()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            sim.set_state(zh, gh)
+            sim.step(dt, 1)
+            read_state()                    # device -> host: the new state (synchronises)
+            en = sim.energy_history()       # and its energy record
+        torch.cuda.synchronize()
+        el = max_over_ranks(time.perf_counter() - t0, world)
+        b1 = sim.transfer_bytes()
+        assert np.isfinite(rawh).all() and np.abs(rawh).max() > 0
         e2e = {"value": 2 * world * args.e2e_steps / el, "unit": "RHS evals/s", "steps": args.e2e_steps,
                "h2d_bytes_per_step": int((b1[0] - b0[0]) // args.e2e_steps), "d2h_bytes_per_step": int((b1[1] - b0[1]) // args.e2e_steps),
                "host_array_bytes": int(z.nbytes + (g.nbytes if M else 0)),
-               "what": "gandalf_set_state(host pinned) + gandalf_step(dt,1) + gandalf_energy_history(host) per step; set_state copies "
-                       "only the modes Eq. 20 retains (the rest of the host array is never read)"}
+               "what": "gandalf_set_state(host pinned) + gandalf_step(dt,1) + gandalf_get_state_raw(host pinned) + gandalf_energy_history(host) "
+                       "per step: the state goes in and the new state comes back; both directions move only the modes Eq. 20 retains",
+               "energy_only": energy_only}
 
     # ---- roofline of the dominant kernel (largest share of device time in the timed region)
     peaks = {}
@@ -633,7 +707,7 @@ def main():
                           "frac_of_hbm_peak": per_launch[name] / 1e9 / (avg_ms * 1e-3) / peak_gbs}
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"])
     traffic, traffic_src = None, None   # dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)
-    for fn_ in ("r02_traffic.csv", "r01_traffic.csv"):
+    for fn_ in ("r02_traffic.csv",):
         try:
             for ln in open(os.path.join(ROOT, "profiles", fn_)).read().splitlines()[1:]:
                 w, k, b = ln.split(",")
@@ -715,7 +789,8 @@ def main():
     if rank == 0:
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            cpu = cpu_baseline_sample(args.workload, shape, full_rhs=args.oracle_full_rhs)
+            full = args.oracle_full_rhs or (args.workload == "4a" and not args.no_oracle_full_rhs and host_can_hold_full_oracle(shape, F))
+            cpu = cpu_baseline_sample(args.workload, shape, full_rhs=full)
         wl = {"4a": "BASELINE config 4(a)", "4b": "BASELINE config 4(b)",
               "4a2": "BASELINE config 4(a) with both slow-mode species (2+64 fields)"}.get(args.workload, f"BASELINE config {args.workload}")
         line = {
@@ -725,10 +800,19 @@ def main():
             "config": {"workload": wl, "grid": list(shape), "M": M, "dt": dt, "fields": F, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": l2_note},
             "steps_per_s": steps_per_s, "grid_point_moments_per_s": steps_per_s * shape[0] * shape[1] * shape[2] * F,
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+            "clocks": clocks, "sustained": sustained, "e2e": e2e, "gpu_launches": launches,
             "launch_path": ("cuda graph of one step, replayed" if graph_replays else "plain stream launches"), "graph_replays": graph_replays, "roofline": roofline, "cpu_baseline": cpu, "cufft_comparison": cufft, "kperp_spectrum": spectrum,
             "final_energy": {"E_A": float(hist[-1, 1]), "W_g": float(hist[-1, 6])},
         }
+        if args.workload == "4a" and world == 1 and not args.no_4b:
+            # BASELINE config 4 names two sizes: the second one is timed in the same run (the 4a context is released first)
+            sim.close()
+            del zd, gd
+            torch.cuda.empty_cache()
+            try:
+                line["extra"] = {"config4b": quick_time("4b", local)}
+            except Exception as exc:                  # never take the headline down
+                line["extra"] = {"config4b": {"error": repr(exc)[:200]}}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

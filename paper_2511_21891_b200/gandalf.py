@@ -223,9 +223,14 @@ class Gandalf:
         self._ck(self._lib.gandalf_state_raw_doubles(self._h, C.byref(n)))
         return n.value
 
-    def get_state_raw(self, device=False):
-        """The evolved variables w+-, g_m on the retained modes (exact checkpoint), a flat float64 array."""
+    def get_state_raw(self, device=False, out=None):
+        """The evolved variables w+-, g_m on the retained modes (exact checkpoint), a flat float64 array.
+        `out`: a contiguous float64 numpy array of state_raw_doubles() entries to fill instead (e.g. a view of pinned memory)."""
         n = self.state_raw_doubles()
+        if out is not None:
+            assert not device and isinstance(out, np.ndarray) and out.dtype == np.float64 and out.flags.c_contiguous and out.size == n
+            self._ck(self._lib.gandalf_get_state_raw(self._h, C.c_void_p(out.ctypes.data), 0))
+            return out
         if device:
             import torch
             t = torch.empty(n, dtype=torch.float64, device=f"cuda:{self.params.device}")
