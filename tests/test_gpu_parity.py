@@ -389,6 +389,70 @@ def test_config3_full_size_first_steps():
     _check_history(o, g)
 
 
+def _golden_rows(name):
+    import os
+    rows = {"T": [], "H": [], "S": []}
+    for ln in open(os.path.join(os.path.dirname(__file__), "golden", name)):
+        t = ln.split()
+        if t and t[0] in rows:
+            rows[t[0]].append(t[1:])
+    return rows
+
+
+def test_config3_full_size_10_and_100_steps_against_the_oracle_written_golden():
+    """BASELINE config 3 at its full size over the window SURVEY.md 8(d) names ("the first 10 and 100 steps"), against
+    tests/golden/config3_history_oracle.txt, which tests/golden/make_config3_history.py wrote from the oracle alone (about an
+    hour of CPU: too slow to repeat here).  Run A is the config as written (C = 0.3), 10 steps; run B uses C = 0.03 for the
+    100-step window, because as written the run overflows within ~40 steps in the oracle and here alike (Q28).
+    Compared: time and the CFL dt of the last step (1e-12), the energy records (1e-9), 48 sampled coefficients of zeta+- and
+    g_m at step 10 (1e-10 of the largest coefficient of the potentials / of all moments) and at step 100 (1e-9)."""
+    from paper_2511_21891_b200.gandalf import Gandalf
+    prm, z, gm, run = config3()
+    assert run["shape"] == (128, 128, 64) and prm["M"] == 32 and prm["cfl"] == 0.3
+    rows = _golden_rows("config3_history_oracle.txt")
+    seen = {"T": 0, "H": 0, "S": 0}
+
+    def check(g, tag, step, tol_s):
+        t, nstep, last_dt = g.time()
+        assert nstep == step
+        hist = g.energy_history()
+        zeta, gg = g.get_state()
+        allf = np.concatenate([zeta, gg])
+        for r in rows["T"]:
+            if r[0] == tag and int(r[1]) == step:
+                assert abs(t - float(r[2])) <= 1e-12 * float(r[2]) and abs(last_dt - float(r[3])) <= 1e-12 * float(r[3]), (tag, step)
+                seen["T"] += 1
+        for r in rows["H"]:
+            if r[0] == tag and int(r[1]) <= step and (step == 10 or int(r[1]) > 10):
+                want = np.array([float(x) for x in r[2:]])
+                got = hist[int(r[1]) - 1]
+                assert abs(got[0] - want[0]) <= 1e-12 * want[0], (tag, r[1])
+                assert np.abs(got[1:] - want[1:]).max() <= TOL_ENERGY * max(1.0, np.abs(want[1:]).max()), (tag, r[1])
+                seen["H"] += 1
+        for r in rows["S"]:
+            if r[0] == tag and int(r[1]) == step:
+                f, iz, iy, ix = (int(x) for x in r[2:6])
+                want = complex(float(r[6]), float(r[7]))
+                # scale: the largest coefficient of the potentials / of ALL moments, as _check_state's joint relative L2 (a high
+                # moment the cascade has not reached yet sits at 1e-17, the round-off floor of its neighbours' couplings)
+                scale = np.abs(allf[:2]).max() if f < 2 else np.abs(allf[2:]).max()
+                assert abs(allf[f, iz, iy, ix] - want) <= tol_s * scale, (tag, step, f, iz, iy, ix)
+                seen["S"] += 1
+
+    g = Gandalf(*run["shape"], **prm)                      # run A: as written
+    g.set_state(z, gm)
+    g.step(0.0, 10)
+    check(g, "A", 10, TOL_10STEPS)
+    g.close()
+    g = Gandalf(*run["shape"], **dict(prm, cfl=0.03))      # run B: the stable C
+    g.set_state(z, gm)
+    g.step(0.0, 10)
+    check(g, "B", 10, TOL_10STEPS)
+    g.step(0.0, 90)
+    check(g, "B", 100, 1e-9)
+    assert seen == {"T": 3, "H": 1 + 1 + 9, "S": 3 * 48}, seen
+
+
 def test_finding_q28_advective_cfl_is_not_sufficient_with_moments():
     """DESIGN.md Q28: with C = 0.3 on max|grad Phi| alone (Eq. 16) the explicit RK2 of the Hermite couplings
     sqrt(m/2){Psi, g_m+-1} is unstable once enough moments are kept (the oracle blows up with the same digits); C = 0.03
